@@ -1,0 +1,158 @@
+"""Seeded synthetic workloads for the Ultra Flash sparse causal chunk attention path.
+
+This module holds ONLY input generation (shapes, seeds, value distributions, bf16
+rounding).  It contains none of the method's arithmetic (no pooling, scoring, top-k,
+softmax or cache policy) and imports neither `oracle/` nor the CUDA package: it is the
+one module both sides may share (tests and bench.py feed its arrays to both).
+
+Shapes follow BASELINE.json `configs[0..4]`; the value recipe is SURVEY.md §8(d)
+(stated again in DESIGN.md §"Input recipe"): Q/K = N(0,1) + A * smooth sinusoidal
+(t,h,w) positional features, V = N(0,1), rounded to bf16 (round-to-nearest-even).
+The paper's real workloads are DiT activations of a trained Wan2.1-1.3B-shaped SR model
+ which do not exist here; these inputs stand in for them.
+"""
+from __future__ import annotations
+
+import dataclasses
+import math
+
+import numpy as np
+
+
+@dataclasses.dataclass(frozen=True)
+class Workload:
+    """One BASELINE.json config.  `prior_chunks` = chunks appended before the timed one."""
+    name: str
+    n_heads: int
+    head_dim: int
+    block: int
+    frames_per_chunk: int          # latent frames per chunk (F)
+    grid_h: int                    # token grid height (Hg) after VAE /8 and 2x2 patchify
+    grid_w: int                    # token grid width  (Wg)
+    capacity_chunks: int           # C: resident non-sink chunks incl. the current one
+    prior_chunks: int              # chunks in the stream before the measured chunk
+    topk_count: int                # >=0: exact count; -1: use percent
+    topk_percent: int              # percent of |CAND|
+    amp: float                     # positional amplitude A
+    sink_blocks: int = 1
+    k_min: int = 4                 # PAPER.md:818 (k_min = 4), floor in percent mode only
+    n_stream_chunks: int = 0       # >0: rolling-stream config (config 3)
+
+    @property
+    def chunk_tokens(self) -> int:
+        return self.frames_per_chunk * self.grid_h * self.grid_w
+
+    @property
+    def bpc(self) -> int:
+        return -(-self.chunk_tokens // self.block)
+
+
+def token_grid(height_px: int, width_px: int, vae: int = 8, patch: int = 2) -> tuple[int, int]:
+    """Token grid (Hg, Wg) of one latent frame: pixels / VAE stride / spatial patch.
+    PAPER.md:343 ("patch size (1,2,2)"), 8x spatial VAE (BASELINE.json configs[1])."""
+    return height_px // vae // patch, width_px // vae // patch
+
+
+_G1K = token_grid(1088, 1920)   # (68, 120) -> 8160 tokens / latent frame
+_G2K = token_grid(1440, 2560)   # (90, 160) -> 14400 tokens / latent frame
+
+CONFIGS: dict[str, Workload] = {
+    # configs[0]: tiny, 1 head x 64, 3 chunks of 2 frames x 8x8 tokens, block 64, top-2, cache holds all
+    "tiny": Workload("tiny", 1, 64, 64, 2, 8, 8, capacity_chunks=3, prior_chunks=2,
+                     topk_count=2, topk_percent=-1, amp=0.0, n_stream_chunks=3),
+    # configs[1]: 1K step, 1 prior chunk + sink => C = 2
+    "1k": Workload("1k", 12, 128, 128, 3, _G1K[0], _G1K[1], capacity_chunks=2, prior_chunks=1,
+                   topk_count=-1, topk_percent=25, amp=2.0),
+    # configs[2]: 2K step, 2 prior chunks + sink => C = 3
+    "2k": Workload("2k", 12, 128, 128, 3, _G2K[0], _G2K[1], capacity_chunks=3, prior_chunks=2,
+                   topk_count=-1, topk_percent=15, amp=2.0),
+    # configs[3]: 1K rolling stream, 20 chunks, capacity 3 + sink, top 25 %
+    "1k_stream": Workload("1k_stream", 12, 128, 128, 3, _G1K[0], _G1K[1], capacity_chunks=3,
+                          prior_chunks=2, topk_count=-1, topk_percent=25, amp=2.0,
+                          n_stream_chunks=20),
+    # configs[4]: wide model, 40 heads, 2 prior chunks + sink, top 20 %, amplitude 3
+    "wide": Workload("wide", 40, 128, 128, 3, _G1K[0], _G1K[1], capacity_chunks=3, prior_chunks=2,
+                     topk_count=-1, topk_percent=20, amp=3.0),
+}
+
+
+def scaled(w: Workload, name: str, **kw) -> Workload:
+    """A smaller/other variant of a workload with the same recipe (for CPU-seconds parity cases)."""
+    return dataclasses.replace(w, name=name, **kw)
+
+
+# ---------------------------------------------------------------------------
+# bf16 <-> fp32 format conversion (a storage format, not method arithmetic)
+# ---------------------------------------------------------------------------
+
+def f32_to_bf16_bits(x: np.ndarray) -> np.ndarray:
+    """Round float32 to bf16 (round-to-nearest-even); returns uint16 bit patterns."""
+    u = np.ascontiguousarray(x, dtype=np.float32).view(np.uint32)
+    rnd = ((u >> np.uint32(16)) & np.uint32(1)) + np.uint32(0x7FFF)
+    return ((u + rnd) >> np.uint32(16)).astype(np.uint16)
+
+
+def bf16_bits_to_f32(b: np.ndarray) -> np.ndarray:
+    """Exact widening of bf16 bit patterns to float32."""
+    return (np.ascontiguousarray(b, dtype=np.uint16).astype(np.uint32) << np.uint32(16)).view(np.float32)
+
+
+# ---------------------------------------------------------------------------
+# Positional features and chunk generator
+# ---------------------------------------------------------------------------
+
+def _pos_tables(w: Workload):
+    """Frequencies / phases drawn once per run from default_rng(10_000) in the order
+    f_t, f_h, f_w, phi."""
+    g = np.random.default_rng(10_000)
+    d, H = w.head_dim, w.n_heads
+    f_t = g.integers(0, 2, d)
+    f_h = g.integers(0, 3, d)
+    f_w = g.integers(0, 3, d)
+    phi = g.uniform(0.0, 2.0 * math.pi, (H, d))
+    return f_t, f_h, f_w, phi
+
+
+def positional(w: Workload, chunk: int, n_tokens: int | None = None) -> np.ndarray:
+    """p[n, h, j] = sin(2*pi*(f_t[j]*t/24 + f_h[j]*y/Hg + f_w[j]*x/Wg) + phi[h, j]), float32,
+    tokens in raster (t, y, x) order with t = chunk*F + n // (Hg*Wg).
+    Evaluated as sin(a)cos(phi) + cos(a)sin(phi) in float64, then cast to float32."""
+    N = w.chunk_tokens if n_tokens is None else n_tokens
+    f_t, f_h, f_w, phi = _pos_tables(w)
+    n = np.arange(N)
+    per_frame = w.grid_h * w.grid_w
+    t = chunk * w.frames_per_chunk + n // per_frame
+    y = (n % per_frame) // w.grid_w
+    x = n % w.grid_w
+    a = 2.0 * math.pi * (np.outer(t / 24.0, f_t) + np.outer(y / w.grid_h, f_h) + np.outer(x / w.grid_w, f_w))
+    sa, ca = np.sin(a), np.cos(a)                               # [N, d]
+    p = sa[:, None, :] * np.cos(phi)[None] + ca[:, None, :] * np.sin(phi)[None]
+    return p.astype(np.float32)
+
+
+def make_chunk(w: Workload, chunk: int, seed: int | None = None, n_tokens: int | None = None,
+               rng: np.random.Generator | None = None):
+    """Q, K, V of one chunk as bf16 bit patterns, uint16 [N, H, d].
+
+    Seed rule: chunk c of a stream uses seed c unless `rng` is given (config 0
+    draws all chunks in order from one default_rng(0)).  Draw order: Qn, Kn, Vn."""
+    N = w.chunk_tokens if n_tokens is None else n_tokens
+    if rng is None:
+        rng = np.random.default_rng(chunk if seed is None else seed)
+    shape = (N, w.n_heads, w.head_dim)
+    qn = rng.standard_normal(shape, dtype=np.float32)
+    kn = rng.standard_normal(shape, dtype=np.float32)
+    vn = rng.standard_normal(shape, dtype=np.float32)
+    if w.amp != 0.0:
+        p = positional(w, chunk, N)
+        qn += np.float32(w.amp) * p
+        kn += np.float32(w.amp) * p
+    return f32_to_bf16_bits(qn), f32_to_bf16_bits(kn), f32_to_bf16_bits(vn)
+
+
+def make_stream(w: Workload, n_chunks: int):
+    """List of (Q, K, V) bf16-bit chunks 0..n_chunks-1.  'tiny' draws from one rng(0) in order."""
+    if w.name.startswith("tiny"):
+        rng = np.random.default_rng(0)
+        return [make_chunk(w, c, rng=rng) for c in range(n_chunks)]
+    return [make_chunk(w, c) for c in range(n_chunks)]
