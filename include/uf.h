@@ -1,0 +1,162 @@
+/* uf.h — C ABI of the B200-native sparse causal chunk attention path of Ultra Flash
+ * (arxiv/paper_2606_09150).  Library: paper_2606_09150_b200/libuf.so (built by
+ * paper_2606_09150_b200/build.py with nvcc for sm_100a).
+ *
+ * Citations: `P:NNN` = line NNN of the paper text; `BJ` = BASELINE.json
+ * (`north_star`, `configs`); `R-n` = reading n in DESIGN.md §"Readings of the paper".
+ *
+ * What the path computes, per streaming chunk c of one attention layer (P:86-90, P:136 (iii),
+ * P:343; call order "append -> select -> attention" from BJ configs[3]):
+ *
+ *   uf_kv_append        write the chunk's K,V into a bounded rolling cache, evict the oldest
+ *                       chunks under a FIFO window, keep a permanent sink (chunk 0, block 0)
+ *   uf_select_blocks    block-mean pool Q and K, score s_ij = qbar_i . kbar_j / sqrt(d) (Eq. 4,
+ *                       P:88), keep the top-k cached key blocks per (head, query block)
+ *   uf_sparse_attn_fwd  softmax(q k^T / sqrt(d)) v over SINK u TOPK u CUR (the whole current
+ *                       chunk), chunk-causal by construction
+ *
+ * Conventions
+ *   - All calls return an int32 status (UF_OK = 0).  uf_last_error() gives a message.
+ *   - "device pointer" = CUDA device memory on the ctx's device; "host pointer" = ordinary host
+ *     memory.  The caller owns every buffer it passes in; the ctx owns the caches, the pooled-K
+ *     table, the selection workspace and the host slot map, all freed by uf_ctx_destroy.
+ *   - Device work is enqueued on the caller's stream (`void* stream` = cudaStream_t, NULL = the
+ *     legacy default stream) and is asynchronous; host bookkeeping (slot map, candidate set) is
+ *     updated synchronously and is valid on return.  Getters that copy device data synchronise
+ *     the given stream.
+ *   - One ctx = the cache of one (layer, video stream).  A ctx is not thread-safe.
+ *   - Q, K, V, O are bf16, logical shape [n_tokens, n_heads, head_dim], element strides
+ *     (tok_stride, head_stride, 1); the innermost (head_dim) axis must be contiguous, the base
+ *     pointer and both strides*2 bytes must be multiples of 16 bytes.
+ *   - Blocks: flat runs of `block` consecutive tokens aligned to the chunk start; the last
+ *     block of a chunk may be ragged (R-1, R-3).  Global key-block id g = chunk*BPC + b with
+ *     BPC = ceil(chunk_tokens_max / block).
+ *   - There is no CPU fallback: every step runs in CUDA kernels for sm_100a.
+ */
+#ifndef UF_H_
+#define UF_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define UF_OK               0
+#define UF_ERR_INVALID_ARG  1   /* null pointer, bad size/stride/alignment, bad config            */
+#define UF_ERR_STATE        2   /* call order: select before append, attn before select, ...      */
+#define UF_ERR_CAPACITY     3   /* n_tokens > chunk_tokens_max, window > capacity, buffer too small */
+#define UF_ERR_UNSUPPORTED  4   /* shape not covered by any kernel                                 */
+#define UF_ERR_CUDA         5   /* a CUDA runtime/driver call failed (message has the CUDA error)  */
+
+#define UF_MAX_CAPACITY_CHUNKS 16
+
+typedef struct uf_ctx uf_ctx;
+
+typedef struct uf_config {
+  int32_t n_heads;           /* H  (BJ configs: 1, 12, 40)                                        */
+  int32_t head_dim;          /* d  (32, 64 or 128)                                                 */
+  int32_t block;             /* B  query block == key block (64 or 128; multiple of 32, <= 128)   */
+  int32_t chunk_tokens_max;  /* upper bound on tokens per chunk; BPC = ceil(this / block)         */
+  int32_t capacity_chunks;   /* C: resident non-sink chunks INCLUDING the just-appended one (R-16);
+                                1..UF_MAX_CAPACITY_CHUNKS.  P:343 "KV cache: 3 temporal windows"  */
+  int32_t sink_blocks;       /* S: blocks 0..S-1 of chunk 0 kept forever (BJ configs[0]); 0..4    */
+  int32_t k_min;             /* floor on k in percent mode (k_min = 4)                     */
+  int32_t device;            /* CUDA ordinal; -1 = host-only ctx: slot-map bookkeeping works,
+                                every device step returns UF_ERR_STATE (used by CPU tests)        */
+} uf_config;
+
+/* Create a ctx: allocates K cache, V cache ([H][(S + C*BPC)*B][d] bf16, zero-filled), the pooled-K
+ * table and the selection workspace on cfg->device.  *out receives the handle. */
+int32_t uf_ctx_create(const uf_config* cfg, uf_ctx** out);
+
+/* Free everything the ctx owns.  NULL is accepted. */
+int32_t uf_ctx_destroy(uf_ctx* ctx);
+
+/* Start a new video stream: empty cache, no sink, chunk counter back to 0 (R-27).  Re-zeroes the
+ * caches on `stream`. */
+int32_t uf_ctx_reset(uf_ctx* ctx, void* stream);
+
+/* Step a1 — KV append + evict (P:136 (iii) "dynamically selecting a compact cache window",
+ * P:343; BJ configs[3] "eviction of the oldest non-sink chunk after each append").
+ * The chunk gets id c = number of appends since reset.  With window W = window_chunks (0 -> C,
+ * else 1..C) every resident chunk with id <= c - W is evicted, oldest first (FIFO; shrinking W
+ * evicts several, growing never resurrects, R-17); the chunk then takes the lowest-numbered free
+ * slot.  On c == 0 its first S blocks are also copied to the sink region.  Also produces the
+ * block-mean pooled K of the chunk's blocks, used by uf_select_blocks.
+ *   k, v        device pointers, bf16 [n_tokens, H, d] with the given element strides
+ *   n_tokens    1..chunk_tokens_max
+ * With a host-only ctx (device == -1) k, v, stream are ignored and only the slot map advances. */
+int32_t uf_kv_append(uf_ctx* ctx, const void* k, const void* v, int32_t n_tokens,
+                     int64_t tok_stride, int64_t head_stride, int32_t window_chunks, void* stream);
+
+/* Host query: for the current state, the candidate count |CAND| (blocks of resident chunks older
+ * than the newest one, minus the sink ids, R-10/R-15) and the effective budget
+ *   k' = min(k, |CAND|),  k = topk_count if topk_count >= 0,
+ *                         else max(k_min, floor(topk_percent * |CAND| / 100))   (R-8/R-9).
+ * Either output pointer may be NULL. */
+int32_t uf_query_topk(const uf_ctx* ctx, int32_t topk_count, int32_t topk_percent,
+                      int32_t* n_cand, int32_t* k_eff);
+
+/* Steps a2-a4 — block pooling, scoring (Eq. 4: s_ij^h = qbar_i^h . kbar_j^h / sqrt(d_h), fp64,
+ * terms added in index order, no fused multiply-add, R-4) and top-k per (head, query block); equal
+ * scores -> the smaller global id wins (BJ); lists ascending by global id.  The selection is kept
+ * in the ctx for the following uf_sparse_attn_fwd.
+ *   q           device pointer, bf16 [n_tokens, H, d]; n_tokens must equal the last append's
+ *   idx_out     device pointer or NULL: int32 [H, ceil(n_tokens/B), k'] global block ids
+ *   cnt_out     device pointer or NULL: int32 [H, ceil(n_tokens/B)] (= k' for every row)     */
+int32_t uf_select_blocks(uf_ctx* ctx, const void* q, int32_t n_tokens,
+                         int64_t tok_stride, int64_t head_stride,
+                         int32_t topk_count, int32_t topk_percent,
+                         int32_t* idx_out, int32_t* cnt_out, void* stream);
+
+/* Step a5 — block-sparse attention: for every valid query row n of block i and head h
+ *   o_n = sum_m softmax_m(q_n . k_m * scale) v_m   over the valid tokens m of
+ *   KEPT[h,i] = SINK u TOPK[h,i] u CUR   (BJ north_star; R-13/R-14/R-15).
+ * bf16 inputs, fp32 accumulation and softmax, bf16 output (round-to-nearest-even).
+ *   q, o        device pointers, bf16 [n_tokens, H, d] (same strides for both)
+ *   lse         device pointer or NULL: fp32 [H, n_tokens], natural-log sum-exp of the scaled logits
+ *   softmax_scale  0 -> 1/sqrt(d)
+ * Kernels: B == 128 && d == 128 -> TMA + tcgen05/TMEM kernel; other shapes -> the generic CUDA-core
+ * kernel.  uf_set_attn_impl can force the generic kernel (cross-checks). */
+int32_t uf_sparse_attn_fwd(uf_ctx* ctx, const void* q, void* o, float* lse, int32_t n_tokens,
+                           int64_t tok_stride, int64_t head_stride, float softmax_scale,
+                           void* stream);
+
+/* impl: 0 = automatic (default), 1 = force the generic CUDA-core attention kernel. */
+int32_t uf_set_attn_impl(uf_ctx* ctx, int32_t impl);
+
+/* Observability (host outputs).
+ * uf_get_slot_map: slot_chunk[C] = chunk id resident in each slot or -1; n_resident; newest chunk
+ * id (-1 before the first append).  Any pointer may be NULL. */
+int32_t uf_get_slot_map(const uf_ctx* ctx, int32_t* slot_chunk, int32_t* n_resident,
+                        int32_t* newest_chunk);
+
+/* uf_get_cache_block: copy the cached K and V rows of one key block and one head to host memory.
+ * global_block: g = chunk*BPC + b of a resident chunk, or -(s+1) for sink block s.
+ * k_out, v_out: host pointers (or NULL), bf16 [B, d]; rows past the block's valid count are the
+ * cache's zero padding.  Synchronises `stream`. */
+int32_t uf_get_cache_block(uf_ctx* ctx, int32_t global_block, int32_t head,
+                           void* k_out, void* v_out, void* stream);
+
+/* uf_get_pooled_k: copy the block-mean pooled K (fp64 [d]) of one resident key block and head to
+ * host memory (same addressing as uf_get_cache_block).  Synchronises `stream`. */
+int32_t uf_get_pooled_k(uf_ctx* ctx, int32_t global_block, int32_t head, double* out, void* stream);
+
+/* Bytes of device memory the ctx owns. */
+int64_t uf_ctx_device_bytes(const uf_ctx* ctx);
+
+/* Number of kernels the ctx has launched since creation (bench.py's gpu_launches). */
+int64_t uf_ctx_launch_count(const uf_ctx* ctx);
+
+/* Message of the last failing call on this ctx (ctx-owned string; "" if none).  With ctx == NULL:
+ * message of the last failing uf_ctx_create on this thread. */
+const char* uf_last_error(const uf_ctx* ctx);
+
+/* Library version string, e.g. "uf-b200 0.1 (sm_100a)". */
+const char* uf_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* UF_H_ */

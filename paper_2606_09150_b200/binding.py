@@ -1,0 +1,184 @@
+"""ctypes binding of include/uf.h — argument marshalling only.
+
+Every function has the name and the arguments of the C call it wraps; tensors are passed as
+objects with `.data_ptr()` (torch tensors) or as raw integer addresses.  Nothing of the method is
+computed here: pooling, scoring, top-k, cache policy and attention all run inside libuf.so.
+There is no fallback: if the library is missing or a call fails, `UFError` is raised.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from ctypes import POINTER, Structure, byref, c_char_p, c_double, c_float, c_int32, c_int64, c_void_p
+
+_PKG = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_PKG, "libuf.so")
+
+UF_OK, UF_ERR_INVALID_ARG, UF_ERR_STATE, UF_ERR_CAPACITY, UF_ERR_UNSUPPORTED, UF_ERR_CUDA = range(6)
+UF_MAX_CAPACITY_CHUNKS = 16
+_ERR_NAMES = {1: "UF_ERR_INVALID_ARG", 2: "UF_ERR_STATE", 3: "UF_ERR_CAPACITY", 4: "UF_ERR_UNSUPPORTED",
+              5: "UF_ERR_CUDA"}
+
+# every symbol include/uf.h declares (tests check that the library exports all of them)
+SYMBOLS = [
+    "uf_ctx_create", "uf_ctx_destroy", "uf_ctx_reset", "uf_kv_append", "uf_query_topk", "uf_select_blocks",
+    "uf_sparse_attn_fwd", "uf_set_attn_impl", "uf_get_slot_map", "uf_get_cache_block", "uf_get_pooled_k",
+    "uf_ctx_device_bytes", "uf_ctx_launch_count", "uf_last_error", "uf_version",
+]
+
+
+class UFError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"{_ERR_NAMES.get(code, code)}: {msg}")
+        self.code = code
+
+
+class uf_config(Structure):
+    _fields_ = [(n, c_int32) for n in ("n_heads", "head_dim", "block", "chunk_tokens_max", "capacity_chunks",
+                                       "sink_blocks", "k_min", "device")]
+
+
+_lib = None
+
+
+def load_library() -> ctypes.CDLL:
+    """dlopen libuf.so (built in-tree by paper_2606_09150_b200.build); raises if it is missing."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise UFError(UF_ERR_UNSUPPORTED, f"{LIB_PATH} not built: run `python -m paper_2606_09150_b200.build` "
+                                          "(there is no CPU fallback)")
+    lib = ctypes.CDLL(LIB_PATH)
+    P = c_void_p
+    lib.uf_ctx_create.argtypes = [POINTER(uf_config), POINTER(P)]
+    lib.uf_ctx_destroy.argtypes = [P]
+    lib.uf_ctx_reset.argtypes = [P, P]
+    lib.uf_kv_append.argtypes = [P, P, P, c_int32, c_int64, c_int64, c_int32, P]
+    lib.uf_query_topk.argtypes = [P, c_int32, c_int32, POINTER(c_int32), POINTER(c_int32)]
+    lib.uf_select_blocks.argtypes = [P, P, c_int32, c_int64, c_int64, c_int32, c_int32, P, P, P]
+    lib.uf_sparse_attn_fwd.argtypes = [P, P, P, P, c_int32, c_int64, c_int64, c_float, P]
+    lib.uf_set_attn_impl.argtypes = [P, c_int32]
+    lib.uf_get_slot_map.argtypes = [P, POINTER(c_int32), POINTER(c_int32), POINTER(c_int32)]
+    lib.uf_get_cache_block.argtypes = [P, c_int32, c_int32, P, P, P]
+    lib.uf_get_pooled_k.argtypes = [P, c_int32, c_int32, POINTER(c_double), P]
+    lib.uf_ctx_device_bytes.argtypes = [P]
+    lib.uf_ctx_device_bytes.restype = c_int64
+    lib.uf_ctx_launch_count.argtypes = [P]
+    lib.uf_ctx_launch_count.restype = c_int64
+    lib.uf_last_error.argtypes = [P]
+    lib.uf_last_error.restype = c_char_p
+    lib.uf_version.argtypes = []
+    lib.uf_version.restype = c_char_p
+    for name in SYMBOLS:
+        if getattr(lib, name).restype is ctypes.c_int:
+            getattr(lib, name).restype = c_int32
+    _lib = lib
+    return lib
+
+
+def _ptr(x) -> c_void_p:
+    if x is None:
+        return c_void_p(0)
+    if hasattr(x, "data_ptr"):
+        return c_void_p(x.data_ptr())
+    if hasattr(x, "ctypes"):                       # numpy array (host pointers of the getters)
+        return c_void_p(x.ctypes.data)
+    return c_void_p(int(x))
+
+
+def _stream(s) -> c_void_p:
+    if s is None:
+        return c_void_p(0)
+    if hasattr(s, "cuda_stream"):
+        return c_void_p(s.cuda_stream)
+    return c_void_p(int(s))
+
+
+def _check(ctx, code: int):
+    if code != UF_OK:
+        msg = load_library().uf_last_error(ctx)
+        raise UFError(code, msg.decode() if msg else "")
+
+
+def uf_version() -> str:
+    return load_library().uf_version().decode()
+
+
+def uf_ctx_create(n_heads: int, head_dim: int, block: int, chunk_tokens_max: int, capacity_chunks: int,
+                  sink_blocks: int = 1, k_min: int = 4, device: int = 0) -> c_void_p:
+    lib = load_library()
+    cfg = uf_config(n_heads, head_dim, block, chunk_tokens_max, capacity_chunks, sink_blocks, k_min, device)
+    out = c_void_p(0)
+    _check(None, lib.uf_ctx_create(byref(cfg), byref(out)))
+    return out
+
+
+def uf_ctx_destroy(ctx) -> None:
+    _check(None, load_library().uf_ctx_destroy(ctx))
+
+
+def uf_ctx_reset(ctx, stream=None) -> None:
+    _check(ctx, load_library().uf_ctx_reset(ctx, _stream(stream)))
+
+
+def uf_kv_append(ctx, k, v, n_tokens: int, tok_stride: int, head_stride: int, window_chunks: int = 0,
+                 stream=None) -> None:
+    _check(ctx, load_library().uf_kv_append(ctx, _ptr(k), _ptr(v), n_tokens, tok_stride, head_stride,
+                                            window_chunks, _stream(stream)))
+
+
+def uf_query_topk(ctx, topk_count: int = -1, topk_percent: int = -1) -> tuple[int, int]:
+    """-> (|CAND|, k')"""
+    n_cand, k_eff = c_int32(0), c_int32(0)
+    _check(ctx, load_library().uf_query_topk(ctx, topk_count, topk_percent, byref(n_cand), byref(k_eff)))
+    return n_cand.value, k_eff.value
+
+
+def uf_select_blocks(ctx, q, n_tokens: int, tok_stride: int, head_stride: int, topk_count: int = -1,
+                     topk_percent: int = -1, idx_out=None, cnt_out=None, stream=None) -> None:
+    _check(ctx, load_library().uf_select_blocks(ctx, _ptr(q), n_tokens, tok_stride, head_stride, topk_count,
+                                                topk_percent, _ptr(idx_out), _ptr(cnt_out), _stream(stream)))
+
+
+def uf_sparse_attn_fwd(ctx, q, o, lse, n_tokens: int, tok_stride: int, head_stride: int,
+                       softmax_scale: float = 0.0, stream=None) -> None:
+    _check(ctx, load_library().uf_sparse_attn_fwd(ctx, _ptr(q), _ptr(o), _ptr(lse), n_tokens, tok_stride,
+                                                  head_stride, softmax_scale, _stream(stream)))
+
+
+def uf_set_attn_impl(ctx, impl: int) -> None:
+    _check(ctx, load_library().uf_set_attn_impl(ctx, impl))
+
+
+def uf_get_slot_map(ctx, capacity_chunks: int) -> tuple[list[int], int, int]:
+    """-> (slot -> chunk id or -1, number resident, newest chunk id)"""
+    arr = (c_int32 * UF_MAX_CAPACITY_CHUNKS)()
+    n_res, newest = c_int32(0), c_int32(0)
+    _check(ctx, load_library().uf_get_slot_map(ctx, arr, byref(n_res), byref(newest)))
+    return list(arr[:capacity_chunks]), n_res.value, newest.value
+
+
+def uf_get_cache_block(ctx, global_block: int, head: int, k_out, v_out, stream=None) -> None:
+    """k_out, v_out: host buffers (numpy uint16 [B, d]) or None."""
+    _check(ctx, load_library().uf_get_cache_block(ctx, global_block, head, _ptr(k_out), _ptr(v_out),
+                                                  _stream(stream)))
+
+
+def uf_get_pooled_k(ctx, global_block: int, head: int, out, stream=None) -> None:
+    """out: host buffer, numpy float64 [d]."""
+    _check(ctx, load_library().uf_get_pooled_k(ctx, global_block, head,
+                                               ctypes.cast(_ptr(out), POINTER(c_double)), _stream(stream)))
+
+
+def uf_ctx_device_bytes(ctx) -> int:
+    return load_library().uf_ctx_device_bytes(ctx)
+
+
+def uf_ctx_launch_count(ctx) -> int:
+    return load_library().uf_ctx_launch_count(ctx)
+
+
+def uf_last_error(ctx=None) -> str:
+    msg = load_library().uf_last_error(ctx)
+    return msg.decode() if msg else ""

@@ -1,0 +1,369 @@
+// uf_api.cu — the C ABI of include/uf.h: ctx life cycle, cache bookkeeping (slot map, FIFO window,
+// sink), argument checks and kernel dispatch.  No arithmetic of the method runs on the host except
+// the integer cache policy (P:136 (iii), BJ configs[3]; readings R-16/R-17 in DESIGN.md).
+#include "uf_internal.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+namespace {
+
+thread_local std::string g_create_err;
+
+int fail(uf_ctx* c, int code, const std::string& msg) {
+  if (c) c->err = msg; else g_create_err = msg;
+  return code;
+}
+int fail_cuda(uf_ctx* c, cudaError_t e, const char* what) {
+  return fail(c, UF_ERR_CUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+
+#define UF_CUDA(c, call)                                          \
+  do {                                                            \
+    cudaError_t e__ = (call);                                     \
+    if (e__ != cudaSuccess) return fail_cuda((c), e__, #call);    \
+  } while (0)
+
+int n_blocks(const uf_ctx* c, int ntok) { return uf_ceil_div(ntok, c->cfg.block); }
+
+int n_resident(const uf_ctx* c) {
+  int n = 0;
+  for (int s = 0; s < c->cfg.capacity_chunks; ++s) n += (c->slot_chunk[s] >= 0);
+  return n;
+}
+
+// Snapshot of the state for the newest chunk (the "current" one).
+bool make_view(const uf_ctx* c, UfView* v) {
+  const int C = c->cfg.capacity_chunks;
+  int cur = c->next_chunk - 1;
+  if (cur < 0) return false;
+  memset(v, 0, sizeof(*v));
+  v->H = c->cfg.n_heads; v->d = c->cfg.head_dim; v->B = c->cfg.block;
+  v->BPC = c->BPC; v->S = c->cfg.sink_blocks; v->P = c->P;
+  v->cur_chunk = cur; v->cur_slot = -1;
+  v->sink_ntok = c->sink_ntok;
+  const int n_sink_ids = uf_ceil_div(c->sink_ntok, c->cfg.block);   // sink blocks that exist
+  v->n_sink_blocks = cur > 0 ? n_sink_ids : 0;
+  // resident chunks in ascending id
+  int ids[UF_MAXC], slots[UF_MAXC], n = 0;
+  for (int s = 0; s < C; ++s)
+    if (c->slot_chunk[s] >= 0) { ids[n] = c->slot_chunk[s]; slots[n] = s; ++n; }
+  for (int i = 1; i < n; ++i)
+    for (int j = i; j > 0 && ids[j - 1] > ids[j]; --j) {
+      int t = ids[j]; ids[j] = ids[j - 1]; ids[j - 1] = t;
+      t = slots[j]; slots[j] = slots[j - 1]; slots[j - 1] = t;
+    }
+  int np = 0, pref = 0;
+  for (int i = 0; i < n; ++i) {
+    if (ids[i] == cur) { v->cur_slot = slots[i]; v->cur_ntok = c->slot_ntok[slots[i]]; continue; }
+    int nb = n_blocks(c, c->slot_ntok[slots[i]]);
+    int first = (ids[i] == 0) ? (n_sink_ids < nb ? n_sink_ids : nb) : 0;   // CAND excludes SINK ids
+    v->prior_chunk[np] = ids[i]; v->prior_slot[np] = slots[i];
+    v->prior_ntok[np] = c->slot_ntok[slots[i]]; v->prior_first_b[np] = first;
+    v->cand_prefix[np] = pref;
+    pref += nb - first;
+    ++np;
+  }
+  v->cand_prefix[np] = pref;
+  for (int i = np + 1; i <= UF_MAXC; ++i) v->cand_prefix[i] = pref;
+  v->n_prior = np; v->n_cand = pref;
+  return v->cur_slot >= 0;
+}
+
+int topk_budget(const uf_ctx* c, int n_cand, int topk_count, int topk_percent, int* k_eff) {
+  int64_t k;
+  if (topk_count >= 0) k = topk_count;
+  else {
+    if (topk_percent < 0 || topk_percent > 100) return UF_ERR_INVALID_ARG;
+    k = ((int64_t)topk_percent * n_cand) / 100;
+    if (k < c->cfg.k_min) k = c->cfg.k_min;
+  }
+  if (k > n_cand) k = n_cand;
+  *k_eff = (int)k;
+  return UF_OK;
+}
+
+int check_tensor_args(uf_ctx* c, const void* p, int64_t tok_stride, int64_t head_stride, const char* name) {
+  if (!p) return fail(c, UF_ERR_INVALID_ARG, std::string(name) + ": null pointer");
+  if (((uintptr_t)p & 15) != 0) return fail(c, UF_ERR_INVALID_ARG, std::string(name) + ": pointer not 16-byte aligned");
+  if (tok_stride < c->cfg.head_dim || head_stride < c->cfg.head_dim || (tok_stride % 8) || (head_stride % 8))
+    return fail(c, UF_ERR_INVALID_ARG, std::string(name) + ": strides must be >= head_dim and multiples of 8 elements");
+  return UF_OK;
+}
+
+void clear_host_state(uf_ctx* c) {
+  for (int s = 0; s < UF_MAXC; ++s) { c->slot_chunk[s] = -1; c->slot_ntok[s] = 0; }
+  c->next_chunk = 0; c->sink_ntok = 0; c->sel_valid = false; c->sel_k = 0; c->sel_ntok = 0;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* uf_version(void) { return "uf-b200 0.1 (sm_100a)"; }
+
+const char* uf_last_error(const uf_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_err.c_str(); }
+
+int32_t uf_ctx_create(const uf_config* cfg, uf_ctx** out) {
+  if (!cfg || !out) return fail(nullptr, UF_ERR_INVALID_ARG, "uf_ctx_create: null argument");
+  *out = nullptr;
+  if (cfg->n_heads < 1 || (cfg->head_dim != 32 && cfg->head_dim != 64 && cfg->head_dim != 128) ||
+      cfg->block < 32 || cfg->block > 128 || (cfg->block % 32) || cfg->chunk_tokens_max < 1 ||
+      cfg->capacity_chunks < 1 || cfg->capacity_chunks > UF_MAXC || cfg->sink_blocks < 0 ||
+      cfg->sink_blocks > 4 || cfg->k_min < 0)
+    return fail(nullptr, UF_ERR_INVALID_ARG, "uf_ctx_create: config out of range (see uf.h)");
+  uf_ctx* c = new (std::nothrow) uf_ctx();
+  if (!c) return fail(nullptr, UF_ERR_CAPACITY, "uf_ctx_create: out of host memory");
+  c->cfg = *cfg;
+  c->BPC = uf_ceil_div(cfg->chunk_tokens_max, cfg->block);
+  c->P = cfg->sink_blocks + cfg->capacity_chunks * c->BPC;
+  c->kcap = (cfg->capacity_chunks - 1) * c->BPC;
+  if (c->kcap < 1) c->kcap = 1;
+  if (c->P >= (1 << 20)) { delete c; return fail(nullptr, UF_ERR_CAPACITY, "uf_ctx_create: too many physical blocks"); }
+  clear_host_state(c);
+  c->host_only = cfg->device < 0;
+  if (c->host_only) { *out = c; return UF_OK; }
+
+  cudaError_t e = cudaSetDevice(cfg->device);
+  if (e != cudaSuccess) { int r = fail_cuda(nullptr, e, "cudaSetDevice"); delete c; return r; }
+  cudaDeviceProp prop;
+  e = cudaGetDeviceProperties(&prop, cfg->device);
+  if (e != cudaSuccess) { int r = fail_cuda(nullptr, e, "cudaGetDeviceProperties"); delete c; return r; }
+  if (prop.major != 10) {
+    delete c;
+    return fail(nullptr, UF_ERR_UNSUPPORTED, "uf_ctx_create: this library is built for sm_100a (B200) only");
+  }
+  c->sm_count = prop.multiProcessorCount;
+  const int64_t H = cfg->n_heads, d = cfg->head_dim, B = cfg->block, P = c->P, BPC = c->BPC;
+  const int64_t NP = (BPC + 1) / 2;
+  const int64_t cache_bytes = H * P * B * d * 2;
+  struct { void** p; int64_t bytes; } allocs[] = {
+      {(void**)&c->kc, cache_bytes},
+      {(void**)&c->vc, cache_bytes},
+      {(void**)&c->kpool, H * d * P * 8},
+      {(void**)&c->qbar, H * BPC * d * 8},
+      {(void**)&c->sel_q, H * BPC * (int64_t)c->kcap * 4},
+      {(void**)&c->sel_rank, H * BPC * (int64_t)c->kcap * 4},
+      {(void**)&c->sel_pair, H * NP * 2 * (int64_t)c->kcap * 4},
+      {(void**)&c->pair_cnt, H * NP * 4},
+  };
+  for (auto& a : allocs) {
+    e = cudaMalloc(a.p, (size_t)a.bytes);
+    if (e != cudaSuccess) {
+      int r = fail_cuda(nullptr, e, "cudaMalloc");
+      uf_ctx_destroy(c);
+      return r;
+    }
+    c->dev_bytes += a.bytes;
+  }
+  e = cudaMemset(c->kc, 0, (size_t)cache_bytes);
+  if (e == cudaSuccess) e = cudaMemset(c->vc, 0, (size_t)cache_bytes);
+  if (e == cudaSuccess) e = cudaMemset(c->kpool, 0, (size_t)(H * d * P * 8));
+  if (e == cudaSuccess) e = cudaDeviceSynchronize();
+  if (e != cudaSuccess) { int r = fail_cuda(nullptr, e, "cudaMemset"); uf_ctx_destroy(c); return r; }
+  if (cfg->block == 128 && cfg->head_dim == 128) {
+    int r = uf_sm100_make_cache_maps(c);
+    if (r != UF_OK) { g_create_err = c->err; uf_ctx_destroy(c); return r; }
+  }
+  *out = c;
+  return UF_OK;
+}
+
+int32_t uf_ctx_destroy(uf_ctx* c) {
+  if (!c) return UF_OK;
+  if (!c->host_only) {
+    cudaSetDevice(c->cfg.device);
+    cudaFree(c->kc); cudaFree(c->vc); cudaFree(c->kpool); cudaFree(c->qbar);
+    cudaFree(c->sel_q); cudaFree(c->sel_rank); cudaFree(c->sel_pair); cudaFree(c->pair_cnt);
+  }
+  delete c;
+  return UF_OK;
+}
+
+int32_t uf_ctx_reset(uf_ctx* c, void* stream) {
+  if (!c) return UF_ERR_INVALID_ARG;
+  clear_host_state(c);
+  if (c->host_only) return UF_OK;
+  UF_CUDA(c, cudaSetDevice(c->cfg.device));
+  cudaStream_t s = (cudaStream_t)stream;
+  const int64_t H = c->cfg.n_heads, d = c->cfg.head_dim, B = c->cfg.block, P = c->P;
+  UF_CUDA(c, cudaMemsetAsync(c->kc, 0, (size_t)(H * P * B * d * 2), s));
+  UF_CUDA(c, cudaMemsetAsync(c->vc, 0, (size_t)(H * P * B * d * 2), s));
+  UF_CUDA(c, cudaMemsetAsync(c->kpool, 0, (size_t)(H * d * P * 8), s));
+  return UF_OK;
+}
+
+int32_t uf_kv_append(uf_ctx* c, const void* k, const void* v, int32_t n_tokens,
+                     int64_t tok_stride, int64_t head_stride, int32_t window_chunks, void* stream) {
+  if (!c) return UF_ERR_INVALID_ARG;
+  const int C = c->cfg.capacity_chunks;
+  if (n_tokens < 1) return fail(c, UF_ERR_INVALID_ARG, "uf_kv_append: n_tokens < 1");
+  if (n_tokens > c->cfg.chunk_tokens_max) return fail(c, UF_ERR_CAPACITY, "uf_kv_append: n_tokens > chunk_tokens_max");
+  if (window_chunks < 0 || window_chunks > C) return fail(c, UF_ERR_CAPACITY, "uf_kv_append: window_chunks outside 0..capacity_chunks");
+  if (!c->host_only) {
+    int r = check_tensor_args(c, k, tok_stride, head_stride, "uf_kv_append k");
+    if (r) return r;
+    r = check_tensor_args(c, v, tok_stride, head_stride, "uf_kv_append v");
+    if (r) return r;
+  }
+  // --- cache policy (host, integers only) ---
+  const int cid = c->next_chunk;
+  const int W = window_chunks == 0 ? C : window_chunks;
+  for (;;) {   // evict ids <= cid - W, oldest first
+    int oldest = -1;
+    for (int s = 0; s < C; ++s)
+      if (c->slot_chunk[s] >= 0 && (oldest < 0 || c->slot_chunk[s] < c->slot_chunk[oldest])) oldest = s;
+    if (oldest < 0 || c->slot_chunk[oldest] > cid - W) break;
+    c->slot_chunk[oldest] = -1; c->slot_ntok[oldest] = 0;
+  }
+  int slot = -1;
+  for (int s = 0; s < C; ++s) if (c->slot_chunk[s] < 0) { slot = s; break; }   // lowest free slot
+  if (slot < 0) return fail(c, UF_ERR_STATE, "uf_kv_append: no free slot (internal)");
+  c->slot_chunk[slot] = cid; c->slot_ntok[slot] = n_tokens;
+  if (cid == 0) {
+    int ns = c->cfg.sink_blocks * c->cfg.block;
+    c->sink_ntok = ns < n_tokens ? ns : n_tokens;
+  }
+  c->next_chunk = cid + 1;
+  c->sel_valid = false;
+  if (c->host_only) return UF_OK;
+  // --- device: copy + pooled K ---
+  UF_CUDA(c, cudaSetDevice(c->cfg.device));
+  UfView view;
+  make_view(c, &view);
+  cudaError_t e = uf_launch_append(c, view, (const __nv_bfloat16*)k, (const __nv_bfloat16*)v,
+                                   tok_stride, head_stride, (cudaStream_t)stream);
+  if (e != cudaSuccess) return fail_cuda(c, e, "uf_kv_append kernel launch");
+  return UF_OK;
+}
+
+int32_t uf_query_topk(const uf_ctx* c, int32_t topk_count, int32_t topk_percent, int32_t* n_cand, int32_t* k_eff) {
+  if (!c) return UF_ERR_INVALID_ARG;
+  UfView v;
+  if (!make_view(c, &v)) return UF_ERR_STATE;
+  int k = 0;
+  int r = topk_budget(c, v.n_cand, topk_count, topk_percent, &k);
+  if (r) return r;
+  if (n_cand) *n_cand = v.n_cand;
+  if (k_eff) *k_eff = k;
+  return UF_OK;
+}
+
+int32_t uf_select_blocks(uf_ctx* c, const void* q, int32_t n_tokens, int64_t tok_stride, int64_t head_stride,
+                         int32_t topk_count, int32_t topk_percent, int32_t* idx_out, int32_t* cnt_out,
+                         void* stream) {
+  if (!c) return UF_ERR_INVALID_ARG;
+  if (c->host_only) return fail(c, UF_ERR_STATE, "uf_select_blocks: host-only ctx has no device path");
+  UfView v;
+  if (!make_view(c, &v)) return fail(c, UF_ERR_STATE, "uf_select_blocks: no chunk appended yet");
+  if (n_tokens != v.cur_ntok) return fail(c, UF_ERR_INVALID_ARG, "uf_select_blocks: n_tokens differs from the last append");
+  int r = check_tensor_args(c, q, tok_stride, head_stride, "uf_select_blocks q");
+  if (r) return r;
+  int k = 0;
+  r = topk_budget(c, v.n_cand, topk_count, topk_percent, &k);
+  if (r) return fail(c, r, "uf_select_blocks: topk_percent outside 0..100");
+  if (k > c->kcap) return fail(c, UF_ERR_CAPACITY, "uf_select_blocks: k exceeds workspace (internal)");
+  UF_CUDA(c, cudaSetDevice(c->cfg.device));
+  cudaError_t e = uf_launch_select(c, v, (const __nv_bfloat16*)q, tok_stride, head_stride, k, idx_out, cnt_out,
+                                   (cudaStream_t)stream);
+  if (e != cudaSuccess) return fail_cuda(c, e, "uf_select_blocks kernel launch");
+  c->sel_valid = true; c->sel_k = k; c->sel_ntok = n_tokens;
+  return UF_OK;
+}
+
+int32_t uf_sparse_attn_fwd(uf_ctx* c, const void* q, void* o, float* lse, int32_t n_tokens,
+                           int64_t tok_stride, int64_t head_stride, float softmax_scale, void* stream) {
+  if (!c) return UF_ERR_INVALID_ARG;
+  if (c->host_only) return fail(c, UF_ERR_STATE, "uf_sparse_attn_fwd: host-only ctx has no device path");
+  UfView v;
+  if (!make_view(c, &v)) return fail(c, UF_ERR_STATE, "uf_sparse_attn_fwd: no chunk appended yet");
+  if (!c->sel_valid) return fail(c, UF_ERR_STATE, "uf_sparse_attn_fwd: uf_select_blocks must run after the last append");
+  if (n_tokens != c->sel_ntok) return fail(c, UF_ERR_INVALID_ARG, "uf_sparse_attn_fwd: n_tokens differs from the selection's");
+  int r = check_tensor_args(c, q, tok_stride, head_stride, "uf_sparse_attn_fwd q");
+  if (r) return r;
+  r = check_tensor_args(c, o, tok_stride, head_stride, "uf_sparse_attn_fwd o");
+  if (r) return r;
+  if (!(softmax_scale >= 0.0f) || std::isinf(softmax_scale)) return fail(c, UF_ERR_INVALID_ARG, "uf_sparse_attn_fwd: bad softmax_scale");
+  float scale = softmax_scale == 0.0f ? (float)(1.0 / std::sqrt((double)c->cfg.head_dim)) : softmax_scale;
+  UF_CUDA(c, cudaSetDevice(c->cfg.device));
+  const bool fast = (c->cfg.block == 128 && c->cfg.head_dim == 128 && c->attn_impl == 0 && c->tm_ok);
+  if (fast)
+    return uf_launch_attn_sm100(c, v, (const __nv_bfloat16*)q, (__nv_bfloat16*)o, lse, tok_stride, head_stride,
+                                scale, (cudaStream_t)stream);
+  cudaError_t e = uf_launch_attn_generic(c, v, (const __nv_bfloat16*)q, (__nv_bfloat16*)o, lse, tok_stride,
+                                         head_stride, scale, (cudaStream_t)stream);
+  if (e != cudaSuccess) return fail_cuda(c, e, "uf_sparse_attn_fwd kernel launch");
+  return UF_OK;
+}
+
+int32_t uf_set_attn_impl(uf_ctx* c, int32_t impl) {
+  if (!c || impl < 0 || impl > 1) return UF_ERR_INVALID_ARG;
+  c->attn_impl = impl;
+  return UF_OK;
+}
+
+int32_t uf_get_slot_map(const uf_ctx* c, int32_t* slot_chunk, int32_t* n_res, int32_t* newest) {
+  if (!c) return UF_ERR_INVALID_ARG;
+  if (slot_chunk) for (int s = 0; s < c->cfg.capacity_chunks; ++s) slot_chunk[s] = c->slot_chunk[s];
+  if (n_res) *n_res = n_resident(c);
+  if (newest) *newest = c->next_chunk - 1;
+  return UF_OK;
+}
+
+static int resolve_phys(uf_ctx* c, int32_t g, int* phys) {
+  if (g < 0) {
+    int s = -g - 1;
+    if (s >= uf_ceil_div(c->sink_ntok, c->cfg.block)) return fail(c, UF_ERR_INVALID_ARG, "sink block does not exist");
+    *phys = s;
+    return UF_OK;
+  }
+  int cid = g / c->BPC, b = g % c->BPC;
+  for (int s = 0; s < c->cfg.capacity_chunks; ++s)
+    if (c->slot_chunk[s] == cid) {
+      if (b >= n_blocks(c, c->slot_ntok[s])) return fail(c, UF_ERR_INVALID_ARG, "block index past the chunk's last block");
+      *phys = c->cfg.sink_blocks + s * c->BPC + b;
+      return UF_OK;
+    }
+  return fail(c, UF_ERR_STATE, "chunk of the requested block is not resident");
+}
+
+int32_t uf_get_cache_block(uf_ctx* c, int32_t g, int32_t head, void* k_out, void* v_out, void* stream) {
+  if (!c) return UF_ERR_INVALID_ARG;
+  if (c->host_only) return fail(c, UF_ERR_STATE, "uf_get_cache_block: host-only ctx");
+  if (head < 0 || head >= c->cfg.n_heads) return fail(c, UF_ERR_INVALID_ARG, "uf_get_cache_block: bad head");
+  int phys = 0;
+  int r = resolve_phys(c, g, &phys);
+  if (r) return r;
+  UF_CUDA(c, cudaSetDevice(c->cfg.device));
+  const int64_t B = c->cfg.block, d = c->cfg.head_dim;
+  const int64_t off = ((int64_t)head * c->P + phys) * B * d;
+  cudaStream_t s = (cudaStream_t)stream;
+  if (k_out) UF_CUDA(c, cudaMemcpyAsync(k_out, c->kc + off, (size_t)(B * d * 2), cudaMemcpyDeviceToHost, s));
+  if (v_out) UF_CUDA(c, cudaMemcpyAsync(v_out, c->vc + off, (size_t)(B * d * 2), cudaMemcpyDeviceToHost, s));
+  UF_CUDA(c, cudaStreamSynchronize(s));
+  return UF_OK;
+}
+
+int32_t uf_get_pooled_k(uf_ctx* c, int32_t g, int32_t head, double* out, void* stream) {
+  if (!c || !out) return UF_ERR_INVALID_ARG;
+  if (c->host_only) return fail(c, UF_ERR_STATE, "uf_get_pooled_k: host-only ctx");
+  if (head < 0 || head >= c->cfg.n_heads) return fail(c, UF_ERR_INVALID_ARG, "uf_get_pooled_k: bad head");
+  int phys = 0;
+  int r = resolve_phys(c, g, &phys);
+  if (r) return r;
+  UF_CUDA(c, cudaSetDevice(c->cfg.device));
+  cudaStream_t s = (cudaStream_t)stream;
+  const int64_t d = c->cfg.head_dim;
+  // kpool is [H][d][P]: a strided gather of d doubles
+  UF_CUDA(c, cudaMemcpy2DAsync(out, 8, c->kpool + ((int64_t)head * d) * c->P + phys, (size_t)c->P * 8, 8, (size_t)d,
+                               cudaMemcpyDeviceToHost, s));
+  UF_CUDA(c, cudaStreamSynchronize(s));
+  return UF_OK;
+}
+
+int64_t uf_ctx_device_bytes(const uf_ctx* c) { return c ? c->dev_bytes : 0; }
+int64_t uf_ctx_launch_count(const uf_ctx* c) { return c ? c->launches : 0; }
+
+}  // extern "C"

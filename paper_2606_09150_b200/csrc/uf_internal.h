@@ -1,0 +1,104 @@
+// uf_internal.h — shared declarations of the CUDA path (not part of the ABI; see include/uf.h).
+// Notation follows DESIGN.md: H heads, d head_dim, B block, BPC blocks per chunk slot, C capacity,
+// S sink blocks, P = S + C*BPC physical key blocks per head, g = chunk*BPC + b global block id.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <cuda_bf16.h>
+#include <cuda.h>
+#include <stdint.h>
+
+#include <string>
+
+#include "uf.h"
+
+#define UF_MAXC UF_MAX_CAPACITY_CHUNKS
+
+// Physical layout of the K cache and of the V cache (ctx-owned):
+//   [head h][physical token row = phys*B + r][d] bf16,  phys in [0, P):
+//   phys 0..S-1 = sink region, phys S + slot*BPC + b = block b of the chunk resident in `slot`.
+// Every key block is one contiguous B x d tile, so a single tiled TMA load at token coordinate
+// phys*B fetches it.  Rows past a block's valid count are zero.
+
+// A key-block reference handed to the attention kernels, packed in one int32:
+//   bits  0..19  phys     physical block index
+//   bits 20..27  nvalid-1 valid key rows in the block (1..B)
+//   bits 28..29  mask     which of the CTA's two query tiles attend it (sm100 kernel only)
+__host__ __device__ inline int32_t uf_entry_pack(int phys, int nvalid, int mask) {
+  return (int32_t)((uint32_t)phys | ((uint32_t)(nvalid - 1) << 20) | ((uint32_t)mask << 28));
+}
+__host__ __device__ inline int uf_entry_phys(int32_t e)   { return (int)((uint32_t)e & 0xFFFFFu); }
+__host__ __device__ inline int uf_entry_nvalid(int32_t e) { return (int)(((uint32_t)e >> 20) & 0xFFu) + 1; }
+__host__ __device__ inline int uf_entry_mask(int32_t e)   { return (int)(((uint32_t)e >> 28) & 0x3u); }
+
+// Snapshot of the cache state for one step, passed by value to kernels.
+struct UfView {
+  int H, d, B, BPC, S, P;
+  int n_prior;                    // resident chunks older than the current one, ascending id
+  int prior_chunk[UF_MAXC];       // chunk id
+  int prior_slot[UF_MAXC];        // slot it lives in
+  int prior_ntok[UF_MAXC];        // its token count
+  int prior_first_b[UF_MAXC];     // first block that is a candidate (sink ids are skipped, R-15)
+  int cand_prefix[UF_MAXC + 1];   // candidates contributed by priors [0, i)
+  int n_cand;                     // |CAND|
+  int cur_chunk, cur_slot, cur_ntok;
+  int n_sink_blocks;              // sink blocks attended this step (0 for chunk 0: inside CUR)
+  int sink_ntok;                  // valid tokens in the sink region
+};
+
+__host__ __device__ inline int uf_ceil_div(int a, int b) { return (a + b - 1) / b; }
+
+// candidate j (ascending global id) -> global id, physical block, valid rows
+__host__ __device__ inline void uf_cand_lookup(const UfView& v, int j, int* g, int* phys, int* nvalid) {
+  int i = 0;
+  while (i + 1 < v.n_prior && j >= v.cand_prefix[i + 1]) ++i;
+  int b = v.prior_first_b[i] + (j - v.cand_prefix[i]);
+  *g = v.prior_chunk[i] * v.BPC + b;
+  *phys = v.S + v.prior_slot[i] * v.BPC + b;
+  int rem = v.prior_ntok[i] - b * v.B;
+  *nvalid = rem < v.B ? rem : v.B;
+}
+
+struct uf_ctx {
+  uf_config cfg;
+  int BPC = 0, P = 0;
+  bool host_only = false;
+  // device buffers
+  __nv_bfloat16* kc = nullptr;    // K cache [H][P*B][d]
+  __nv_bfloat16* vc = nullptr;    // V cache [H][P*B][d]
+  double* kpool = nullptr;        // block-mean pooled K, [H][d][P] (transposed for coalesced scoring)
+  double* qbar = nullptr;         // block-mean pooled Q of the current chunk, [H][BPC][d]
+  int32_t* sel_q = nullptr;       // per (h, q-block): k' packed entries, ascending global id; [H][BPC][kcap]
+  int32_t* sel_rank = nullptr;    // candidate index of every sel_q entry (merge key); [H][BPC][kcap]
+  int32_t* sel_pair = nullptr;    // per (h, q-block pair): merged union list with tile masks; [H][NP][2*kcap]
+  int32_t* pair_cnt = nullptr;    // [H][NP]
+  int kcap = 0;                   // (C-1)*BPC
+  int64_t dev_bytes = 0;
+  // host state
+  int slot_chunk[UF_MAXC];
+  int slot_ntok[UF_MAXC];
+  int next_chunk = 0;
+  int sink_ntok = 0;
+  bool sel_valid = false;
+  int sel_k = 0, sel_ntok = 0;
+  int attn_impl = 0;
+  int64_t launches = 0;
+  int sm_count = 0;
+  CUtensorMap tm_k, tm_v;         // K / V cache maps for the sm100 kernel (valid when B == d == 128)
+  bool tm_ok = false;
+  std::string err;
+};
+
+// --- kernels (each launcher returns cudaGetLastError()) -------------------------------------------
+cudaError_t uf_launch_append(uf_ctx* c, const UfView& v, const __nv_bfloat16* k, const __nv_bfloat16* vv,
+                             int64_t tok_stride, int64_t head_stride, cudaStream_t s);
+cudaError_t uf_launch_select(uf_ctx* c, const UfView& v, const __nv_bfloat16* q, int64_t tok_stride,
+                             int64_t head_stride, int k_eff, int32_t* idx_out, int32_t* cnt_out,
+                             cudaStream_t s);
+cudaError_t uf_launch_attn_generic(uf_ctx* c, const UfView& v, const __nv_bfloat16* q, __nv_bfloat16* o,
+                                   float* lse, int64_t tok_stride, int64_t head_stride, float scale,
+                                   cudaStream_t s);
+// returns UF_* status (tensor-map encoding can fail); message in c->err
+int uf_launch_attn_sm100(uf_ctx* c, const UfView& v, const __nv_bfloat16* q, __nv_bfloat16* o, float* lse,
+                         int64_t tok_stride, int64_t head_stride, float scale, cudaStream_t s);
+int uf_sm100_make_cache_maps(uf_ctx* c);

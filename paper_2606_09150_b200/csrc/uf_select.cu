@@ -1,0 +1,241 @@
+// uf_select.cu — steps a2-a4: block-mean pooling of Q, block scores (Eq. 4) and exact
+// top-k per (head, query block) with ties to the lower global id (BJ), plus the merge of the two
+// lists of a query-block pair that the sm100 attention kernel walks.
+//
+// Arithmetic that decides indices is fp64 and follows the order stated in DESIGN.md R-4: the pooled
+// sums are exact (order-free), the mean is one IEEE division, the dot product adds its d products in
+// index order with separately rounded multiply and add (no FMA), then one IEEE division by sqrt(d).
+#include "uf_internal.h"
+
+namespace {
+
+constexpr int kPoolThreads = 256;
+constexpr int kScoreThreads = 256;
+
+__device__ __forceinline__ uint4 ld_stream(const uint4* p) {
+  uint4 r;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+  return r;
+}
+
+// ---- a2: pooled Q.  grid (query blocks, H) -------------------------------------------------------
+template <int D>
+__global__ void __launch_bounds__(kPoolThreads)
+uf_pool_q_kernel(const __nv_bfloat16* __restrict__ q, int64_t tok_stride, int64_t head_stride,
+                 double* __restrict__ qbar, int B, int BPC, int ntok) {
+  constexpr int VPR = D / 8;
+  constexpr int RPP = kPoolThreads / VPR;
+  __shared__ double red[RPP][D + 2];
+  const int i = blockIdx.x, h = blockIdx.y;
+  const int vcx = threadIdx.x % VPR, rg = threadIdx.x / VPR;
+  const int row0 = i * B;
+  const int nvalid = min(B, ntok - row0);
+  double acc[8];
+#pragma unroll
+  for (int t = 0; t < 8; ++t) acc[t] = 0.0;
+#pragma unroll 4
+  for (int r = rg; r < nvalid; r += RPP) {
+    const int64_t src = (int64_t)(row0 + r) * tok_stride + (int64_t)h * head_stride + vcx * 8;
+    const uint4 u = ld_stream(reinterpret_cast<const uint4*>(q + src));
+    const uint32_t w[4] = {u.x, u.y, u.z, u.w};
+#pragma unroll
+    for (int t = 0; t < 4; ++t) {
+      acc[2 * t]     += (double)__uint_as_float(w[t] << 16);
+      acc[2 * t + 1] += (double)__uint_as_float(w[t] & 0xFFFF0000u);
+    }
+  }
+#pragma unroll
+  for (int t = 0; t < 8; ++t) red[rg][vcx * 8 + t] = acc[t];
+  __syncthreads();
+  if (threadIdx.x < D) {
+    double s = 0.0;
+#pragma unroll
+    for (int g = 0; g < RPP; ++g) s += red[g][threadIdx.x];
+    qbar[((int64_t)h * BPC + i) * D + threadIdx.x] = s / (double)nvalid;
+  }
+}
+
+// order-preserving map double -> uint64 (no NaNs; -0.0 was normalised to +0.0 by the caller)
+__device__ __forceinline__ unsigned long long sortable(double x) {
+  unsigned long long u = (unsigned long long)__double_as_longlong(x);
+  return (u & 0x8000000000000000ull) ? ~u : (u | 0x8000000000000000ull);
+}
+
+// ---- a3 + a4: scores and top-k.  grid (ceil(nqb / kQG), H) ------------------------------------------
+// kQG query blocks are scored per CTA (each pooled-K load is re-used kQG times).
+// dynamic smem: double qs[kQG][D]; unsigned long long key[kQG][n_cand]
+template <int D, int kQG>
+__global__ void __launch_bounds__(kScoreThreads)
+uf_score_topk_kernel(UfView v, const double* __restrict__ qbar, const double* __restrict__ kpool,
+                     int nqb, int k_eff, int32_t* __restrict__ sel_q, int32_t* __restrict__ sel_rank, int kcap,
+                     int32_t* __restrict__ idx_out, int32_t* __restrict__ cnt_out) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  double* qs = reinterpret_cast<double*>(smem_raw);                                  // [kQG][D]
+  unsigned long long* key = reinterpret_cast<unsigned long long*>(qs + kQG * D);     // [kQG][n_cand]
+  __shared__ int warp_cnt[kScoreThreads / 32];
+  const int h = blockIdx.y;
+  const int i0 = blockIdx.x * kQG;
+  const int ng = min(kQG, nqb - i0);
+  const int nc = v.n_cand;
+  const int tid = threadIdx.x;
+
+  for (int x = tid; x < kQG * D; x += kScoreThreads) {
+    const int g = x / D, t = x % D;
+    qs[x] = g < ng ? qbar[((int64_t)h * v.BPC + i0 + g) * D + t] : 0.0;
+  }
+  __syncthreads();
+
+  const double inv = sqrt((double)D);
+  for (int j = tid; j < nc; j += kScoreThreads) {
+    int gid, phys, nval;
+    uf_cand_lookup(v, j, &gid, &phys, &nval);
+    const double* kp = kpool + (int64_t)h * D * v.P + phys;
+    double acc[kQG];
+#pragma unroll
+    for (int g = 0; g < kQG; ++g) acc[g] = 0.0;
+#pragma unroll 4
+    for (int t = 0; t < D; ++t) {
+      const double kv = kp[(int64_t)t * v.P];
+#pragma unroll
+      for (int g = 0; g < kQG; ++g) acc[g] = __dadd_rn(acc[g], __dmul_rn(qs[g * D + t], kv));
+    }
+#pragma unroll
+    for (int g = 0; g < kQG; ++g) key[(int64_t)g * nc + j] = sortable(__ddiv_rn(acc[g], inv) + 0.0);
+  }
+  __syncthreads();
+
+  // rank of candidate j = #{j' : s[j'] > s[j]} + #{j' < j : s[j'] == s[j]}; kept iff rank < k'.
+  // Candidates are in ascending global id, so an ordered compaction emits ascending ids.
+  for (int g = 0; g < ng; ++g) {
+    const unsigned long long* kg = key + (int64_t)g * nc;
+    const int i = i0 + g;
+    int base = 0;
+    for (int j0 = 0; j0 < nc; j0 += kScoreThreads) {
+      const int j = j0 + tid;
+      bool keep = false;
+      if (j < nc) {
+        const unsigned long long mine = kg[j];
+        int rank = 0;
+        for (int jj = 0; jj < nc; ++jj) {
+          const unsigned long long o = kg[jj];
+          rank += (o > mine) || (o == mine && jj < j);
+        }
+        keep = rank < k_eff;
+      }
+      const unsigned ball = __ballot_sync(0xffffffffu, keep);
+      const int lane = tid & 31, w = tid >> 5;
+      if (lane == 0) warp_cnt[w] = __popc(ball);
+      __syncthreads();
+      int off = base;
+      for (int ww = 0; ww < w; ++ww) off += warp_cnt[ww];
+      int total = 0;
+      for (int ww = 0; ww < kScoreThreads / 32; ++ww) total += warp_cnt[ww];
+      if (keep) {
+        const int pos = off + __popc(ball & ((1u << lane) - 1u));
+        int gid, phys, nval;
+        uf_cand_lookup(v, j, &gid, &phys, &nval);
+        sel_q[((int64_t)h * v.BPC + i) * kcap + pos] = uf_entry_pack(phys, nval, 0);
+        sel_rank[((int64_t)h * v.BPC + i) * kcap + pos] = j;       // candidate index: the merge key
+        if (idx_out) idx_out[((int64_t)h * nqb + i) * k_eff + pos] = gid;
+      }
+      base += total;
+      __syncthreads();
+    }
+    if (tid == 0 && cnt_out) cnt_out[(int64_t)h * nqb + i] = k_eff;
+  }
+}
+
+// ---- merge the lists of query blocks (2p, 2p+1) into one ascending union with tile masks ----------
+// One thread per (h, pair).  Both lists are subsequences of CAND in candidate order (sel_rank holds the
+// candidate index of every kept entry), so a two-pointer merge yields the union in that order; bit 0 of
+// the mask = tile 0 (block 2p) attends the entry, bit 1 = tile 1 (block 2p+1).
+__global__ void uf_pair_merge_kernel(const int32_t* __restrict__ sel_q, const int32_t* __restrict__ sel_rank,
+                                     int32_t* __restrict__ sel_pair, int32_t* __restrict__ pair_cnt,
+                                     int H, int BPC, int nqb, int k_eff, int kcap) {
+  const int NP = (BPC + 1) / 2;
+  const int np_cur = (nqb + 1) / 2;
+  const int x = blockIdx.x * blockDim.x + threadIdx.x;
+  if (x >= H * np_cur) return;
+  const int h = x / np_cur, p = x % np_cur;
+  const int i0 = 2 * p, i1 = 2 * p + 1;
+  const int32_t* a = sel_q + ((int64_t)h * BPC + i0) * kcap;
+  const int32_t* ra = sel_rank + ((int64_t)h * BPC + i0) * kcap;
+  const bool has1 = i1 < nqb;
+  const int32_t* b = sel_q + ((int64_t)h * BPC + i1) * kcap;
+  const int32_t* rb = sel_rank + ((int64_t)h * BPC + i1) * kcap;
+  int32_t* out = sel_pair + ((int64_t)h * NP + p) * 2 * kcap;
+  int ia = 0, ib = 0, n = 0;
+  const int na = k_eff, nb = has1 ? k_eff : 0;
+  while (ia < na || ib < nb) {
+    const int ka = ia < na ? ra[ia] : 0x7fffffff;
+    const int kb = ib < nb ? rb[ib] : 0x7fffffff;
+    if (ka == kb)      { out[n++] = a[ia] | (3 << 28); ++ia; ++ib; }
+    else if (ka < kb)  { out[n++] = a[ia] | (1 << 28); ++ia; }
+    else               { out[n++] = b[ib] | (2 << 28); ++ib; }
+  }
+  pair_cnt[(int64_t)h * NP + p] = n;
+}
+
+}  // namespace
+
+cudaError_t uf_launch_select(uf_ctx* c, const UfView& v, const __nv_bfloat16* q, int64_t tok_stride,
+                             int64_t head_stride, int k_eff, int32_t* idx_out, int32_t* cnt_out,
+                             cudaStream_t s) {
+  const int nqb = uf_ceil_div(v.cur_ntok, v.B);
+  const int NP = (v.BPC + 1) / 2;
+  if (k_eff == 0) {
+    // no candidates (chunk 0, or window 1): counts are zero, nothing to score
+    if (cnt_out) {
+      cudaError_t e = cudaMemsetAsync(cnt_out, 0, (size_t)v.H * nqb * sizeof(int32_t), s);
+      if (e != cudaSuccess) return e;
+    }
+    return cudaMemsetAsync(c->pair_cnt, 0, (size_t)v.H * NP * sizeof(int32_t), s);
+  }
+  dim3 gp(nqb, v.H);
+  cudaError_t e = cudaSuccess;
+  int qg = 8;
+  auto smem_for = [&](int g) { return (size_t)g * v.d * 8 + (size_t)g * v.n_cand * 8; };
+  while (qg > 1 && smem_for(qg) > 160 * 1024) qg >>= 1;
+  const size_t smem = smem_for(qg);
+  if (smem > 200 * 1024) return cudaErrorInvalidConfiguration;     // > ~25k candidates: not supported
+  dim3 gs(uf_ceil_div(nqb, qg), v.H);
+#define UF_SCORE_LAUNCH(DD, QG)                                                                              \
+  {                                                                                                          \
+    if (smem > 48 * 1024)                                                                                    \
+      e = cudaFuncSetAttribute(uf_score_topk_kernel<DD, QG>, cudaFuncAttributeMaxDynamicSharedMemorySize,    \
+                               (int)smem);                                                                   \
+    if (e != cudaSuccess) return e;                                                                          \
+    uf_score_topk_kernel<DD, QG><<<gs, kScoreThreads, smem, s>>>(v, c->qbar, c->kpool, nqb, k_eff, c->sel_q, \
+                                                                 c->sel_rank, c->kcap, idx_out, cnt_out);    \
+  }
+#define UF_SELECT_CASE(DD)                                                                                   \
+  case DD:                                                                                                   \
+    uf_pool_q_kernel<DD><<<gp, kPoolThreads, 0, s>>>(q, tok_stride, head_stride, c->qbar, v.B, v.BPC,        \
+                                                     v.cur_ntok);                                            \
+    if (qg == 8) UF_SCORE_LAUNCH(DD, 8)                                                                      \
+    else if (qg == 4) UF_SCORE_LAUNCH(DD, 4)                                                                 \
+    else if (qg == 2) UF_SCORE_LAUNCH(DD, 2)                                                                 \
+    else UF_SCORE_LAUNCH(DD, 1)                                                                              \
+    break;
+  switch (v.d) {
+    UF_SELECT_CASE(32)
+    UF_SELECT_CASE(64)
+    UF_SELECT_CASE(128)
+    default: return cudaErrorInvalidValue;
+  }
+#undef UF_SELECT_CASE
+#undef UF_SCORE_LAUNCH
+  c->launches += 2;
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  if (v.B == 128 && v.d == 128) {
+    const int np_cur = (nqb + 1) / 2;
+    uf_pair_merge_kernel<<<uf_ceil_div(v.H * np_cur, 128), 128, 0, s>>>(c->sel_q, c->sel_rank, c->sel_pair,
+                                                                        c->pair_cnt, v.H, v.BPC, nqb, k_eff,
+                                                                        c->kcap);
+    c->launches += 1;
+    e = cudaGetLastError();
+  }
+  return e;
+}

@@ -1,0 +1,223 @@
+"""GPU parity tests: the CUDA path (through the C ABI) against the fp64 oracle, element by element on
+the same seeded inputs.  Bar (BASELINE.json north_star): slot maps and selected block ids bit-exact,
+attention outputs within max-abs 2e-2 / mean-abs 2e-3.  Run with `-m gpu` on a B200."""
+from __future__ import annotations
+
+import dataclasses
+
+import numpy as np
+import pytest
+
+import uf_workloads as wl
+import uf_harness as hz
+
+pytestmark = pytest.mark.gpu
+
+
+def _run_stream(w, chunks, topk_count=-1, topk_percent=-1, windows=None, impl=0, nmax=None, attn=True,
+                heads=None, qblocks=None, check_cache=True):
+    cu = hz.CudaStream(w, nmax)
+    orc = hz.make_oracle(w, nmax)
+    worst = (0.0, 0.0)
+    try:
+        for c, (Qb, Kb, Vb) in enumerate(chunks):
+            win = 0 if windows is None else windows[c]
+            got = cu.step(Qb, Kb, Vb, topk_count, topk_percent, win, impl=impl)
+            ref = hz.oracle_step(orc, Qb, Kb, Vb, topk_count, topk_percent, win, heads=heads, qblocks=qblocks,
+                                 attn=attn)
+            r = hz.compare_step(got, ref, where=f"[{w.name} chunk {c}]")
+            if r:
+                worst = (max(worst[0], r[0]), max(worst[1], r[1]))
+        if check_cache:
+            _check_cache(cu, orc, w)
+    finally:
+        cu.close()
+    return worst
+
+
+def _check_cache(cu, orc, w):
+    """Cache bytes of resident blocks (first, last of each chunk) and the sink equal the inputs; pooled K
+    equals the oracle's block means bit for bit."""
+    H = w.n_heads
+    for ch in orc.resident:
+        nb = orc.n_blocks(ch["n"])
+        for b in sorted({0, nb - 1}):
+            g = ch["id"] * orc.BPC + b
+            for h in sorted({0, H - 1}):
+                kb, vb = cu.cache_block(g, h)
+                kr, vr = orc.block_kv(g)
+                r = kr.shape[0]
+                assert np.array_equal(hz.bits_to_f64(kb[:r]), kr[:, h, :])
+                assert np.array_equal(hz.bits_to_f64(vb[:r]), vr[:, h, :])
+                assert not kb[r:].any() and not vb[r:].any(), "pad rows of a ragged block must be zero"
+                pk = cu.pooled_k(g, h)
+                assert np.array_equal(pk, kr[:, h, :].sum(axis=0) / float(r))
+    for s in orc.sink_ids():
+        kb, vb = cu.cache_block(-(s + 1), 0)
+        kr, vr = orc.block_kv(s, from_sink=True)
+        r = kr.shape[0]
+        assert np.array_equal(hz.bits_to_f64(kb[:r]), kr[:, 0, :]) and np.array_equal(hz.bits_to_f64(vb[:r]), vr[:, 0, :])
+
+
+# ---------------------------------------------------------------------------------------------------
+def test_config0_tiny_full():
+    """BASELINE.json configs[0]: 1 head x 64, block 64, 3 chunks of 128 tokens, top-2 + sink + current."""
+    w = wl.CONFIGS["tiny"]
+    _run_stream(w, wl.make_stream(w, 3), topk_count=2)
+
+
+@pytest.mark.parametrize("impl", [0, 1])
+def test_small_b128_stream_ragged(impl):
+    """B = d = 128 (tcgen05 kernel when impl = 0; generic kernel when impl = 1): 6 chunks, capacity 3,
+    5 query blocks (odd: the last pair has one tile) with a ragged 40-token tail, 2 heads, top 50 %."""
+    w = wl.scaled(wl.CONFIGS["1k"], "small128", n_heads=2, frames_per_chunk=1, grid_h=23, grid_w=24,
+                  capacity_chunks=3, topk_percent=50)
+    assert w.chunk_tokens == 552 and w.bpc == 5
+    _run_stream(w, wl.make_stream(w, 6), topk_percent=50, impl=impl)
+
+
+def test_small_b128_even_blocks_count_mode():
+    w = wl.scaled(wl.CONFIGS["1k"], "small128e", n_heads=3, frames_per_chunk=1, grid_h=32, grid_w=32,
+                  capacity_chunks=2)
+    assert w.chunk_tokens == 1024 and w.bpc == 8
+    _run_stream(w, wl.make_stream(w, 4), topk_count=3)
+
+
+def test_dense_limit_k_saturates():
+    """k >= |CAND| keeps every candidate: the sparse path equals dense chunk-causal attention."""
+    w = wl.scaled(wl.CONFIGS["1k"], "dense128", n_heads=1, frames_per_chunk=1, grid_h=16, grid_w=20,
+                  capacity_chunks=3)
+    _run_stream(w, wl.make_stream(w, 4), topk_count=10_000)
+
+
+def test_window_shrink_and_variable_chunk_length():
+    """FIFO window shrink evicts several chunks; a slot reused by a shorter chunk must not leak stale rows."""
+    w = wl.scaled(wl.CONFIGS["1k"], "var128", n_heads=2, frames_per_chunk=1, grid_h=20, grid_w=20,
+                  capacity_chunks=4)
+    lens = [400, 333, 400, 129, 1, 257, 400]
+    windows = [0, 0, 0, 2, 4, 1, 3]
+    chunks = [wl.make_chunk(w, c, n_tokens=n) for c, n in enumerate(lens)]
+    _run_stream(w, chunks, topk_percent=60, windows=windows, nmax=400)
+
+
+def test_ties_duplicate_blocks_lower_id_wins():
+    """Bitwise-duplicated key blocks score equal; the lower global id must be selected (BJ)."""
+    w = wl.scaled(wl.CONFIGS["1k"], "ties128", n_heads=2, frames_per_chunk=1, grid_h=16, grid_w=32,
+                  capacity_chunks=3)
+    assert w.chunk_tokens == 512
+    chunks = wl.make_stream(w, 3)
+    Q1, K1, V1 = chunks[1]
+    K0 = chunks[0][1]
+    K1 = K1.copy()
+    K1[0:128] = K0[128:256]          # chunk1 block0 == chunk0 block1
+    K1[256:384] = K0[128:256]        # chunk1 block2 == chunk0 block1
+    K1[384:512] = K1[128:256]        # chunk1 block3 == chunk1 block1
+    chunks[1] = (Q1, K1, V1)
+    _run_stream(w, chunks, topk_count=2)
+    _run_stream(w, chunks, topk_count=3)
+
+
+def test_no_sink_and_small_dims_generic():
+    """S = 0 (no sink) and the d = 32 / B = 32 generic shapes."""
+    w = wl.scaled(wl.CONFIGS["tiny"], "tiny32", n_heads=3, head_dim=32, block=32, frames_per_chunk=1, grid_h=7,
+                  grid_w=11, capacity_chunks=2, sink_blocks=0, amp=1.0)
+    _run_stream(w, [wl.make_chunk(w, c) for c in range(4)], topk_count=1)
+
+
+def test_custom_scale_and_no_lse():
+    w = wl.scaled(wl.CONFIGS["1k"], "scale128", n_heads=1, frames_per_chunk=1, grid_h=16, grid_w=16,
+                  capacity_chunks=2)
+    cu, orc = hz.CudaStream(w), hz.make_oracle(w)
+    try:
+        for c in range(2):
+            Qb, Kb, Vb = wl.make_chunk(w, c)
+            got = cu.step(Qb, Kb, Vb, topk_count=1, want_lse=False, scale=0.05)
+            ref = hz.oracle_step(orc, Qb, Kb, Vb, topk_count=1, scale=0.05)
+            hz.compare_step(got, ref, f"[scale chunk {c}]")
+    finally:
+        cu.close()
+
+
+def test_error_codes_and_call_order():
+    import torch
+    import paper_2606_09150_b200 as uf
+    w = wl.scaled(wl.CONFIGS["1k"], "err128", n_heads=1, frames_per_chunk=1, grid_h=16, grid_w=16, capacity_chunks=2)
+    cu = hz.CudaStream(w)
+    try:
+        Qb, Kb, Vb = wl.make_chunk(w, 0)
+        q, k, v = cu.to_dev(Qb), cu.to_dev(Kb), cu.to_dev(Vb)
+        o = torch.empty_like(q)
+        with pytest.raises(uf.UFError) as ei:
+            uf.uf_select_blocks(cu.ctx, q, 256, 128, 128, 1, -1, None, None, cu.stream)
+        assert ei.value.code == uf.binding.UF_ERR_STATE
+        uf.uf_kv_append(cu.ctx, k, v, 256, 128, 128, 0, cu.stream)
+        with pytest.raises(uf.UFError) as ei:
+            uf.uf_sparse_attn_fwd(cu.ctx, q, o, None, 256, 128, 128, 0.0, cu.stream)
+        assert ei.value.code == uf.binding.UF_ERR_STATE
+        with pytest.raises(uf.UFError) as ei:
+            uf.uf_kv_append(cu.ctx, k, v, 257, 128, 128, 0, cu.stream)
+        assert ei.value.code == uf.binding.UF_ERR_CAPACITY
+        with pytest.raises(uf.UFError) as ei:
+            uf.uf_kv_append(cu.ctx, k, v, 256, 130, 128, 0, cu.stream)
+        assert ei.value.code == uf.binding.UF_ERR_INVALID_ARG
+        with pytest.raises(uf.UFError):
+            uf.uf_kv_append(cu.ctx, None, v, 256, 128, 128, 0, cu.stream)
+        assert uf.uf_ctx_launch_count(cu.ctx) == 1 and uf.uf_ctx_device_bytes(cu.ctx) > 0
+    finally:
+        cu.close()
+
+
+# ----------------------------------------------------------------------------- full-size configs
+def _sampled_pairs(w, n_random, seed):
+    rng = np.random.default_rng(seed)
+    nqb = w.bpc
+    qblocks = sorted({0, 1, nqb - 2, nqb - 1} | set(int(x) for x in rng.integers(0, nqb, n_random)))
+    heads = sorted({0, w.n_heads - 1} | set(int(x) for x in rng.integers(0, w.n_heads, 2)))
+    return heads, qblocks
+
+
+@pytest.mark.parametrize("name", ["1k", "2k"])
+def test_full_size_step(name):
+    """BASELINE.json configs[1] / configs[2] at full size, in the launch configuration bench.py times:
+    slot maps and ALL selected block ids bit-exact; attention compared on sampled (head, query block)
+    pairs the oracle computes one by one (first, second, last two blocks incl. the ragged one, + random)."""
+    w = wl.CONFIGS[name]
+    heads, qblocks = _sampled_pairs(w, 6, seed=1)
+    cu, orc = hz.CudaStream(w), hz.make_oracle(w)
+    try:
+        for c in range(w.prior_chunks + 1):
+            Qb, Kb, Vb = wl.make_chunk(w, c)
+            last = c == w.prior_chunks
+            got = cu.step(Qb, Kb, Vb, topk_percent=w.topk_percent)
+            ref = hz.oracle_step(orc, Qb, Kb, Vb, topk_percent=w.topk_percent, heads=heads, qblocks=qblocks,
+                                 attn=last)
+            r = hz.compare_step(got, ref, f"[{name} chunk {c}]")
+            if last:
+                assert not np.isnan(got["O"]).any(), "every output row must be written"
+                assert np.isfinite(got["lse"]).all()
+                print(f"{name}: sampled O max-abs {r[0]:.3e} mean-abs {r[1]:.3e}, oracle min top-k gap {ref['min_gap']:.3e}")
+    finally:
+        cu.close()
+
+
+def test_sm100_kernel_matches_generic_kernel_medium():
+    """Two independent CUDA implementations of step a5 (tcgen05 vs CUDA-core) agree on every row of a
+    medium case that spans many tiles (property check at a size the oracle would take minutes for)."""
+    import torch
+    w = wl.scaled(wl.CONFIGS["1k"], "medium128", n_heads=4, frames_per_chunk=1, grid_h=50, grid_w=60,
+                  capacity_chunks=3, topk_percent=25)
+    cu = hz.CudaStream(w)
+    try:
+        for c in range(3):
+            Qb, Kb, Vb = wl.make_chunk(w, c)
+            a = cu.step(Qb, Kb, Vb, topk_percent=25, impl=0)
+        q = cu.to_dev(Qb)
+        o2 = torch.empty_like(q)
+        n, H, d = Qb.shape
+        cu.uf.uf_set_attn_impl(cu.ctx, 1)
+        cu.uf.uf_sparse_attn_fwd(cu.ctx, q, o2, None, n, H * d, d, 0.0, cu.stream)
+        torch.cuda.synchronize()
+        diff = np.abs(a["O"] - o2.float().cpu().numpy())
+        assert diff.max() <= 2e-2 and diff.mean() <= 2e-3, (diff.max(), diff.mean())
+    finally:
+        cu.close()
