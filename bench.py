@@ -1,0 +1,436 @@
+#!/usr/bin/env python
+"""bench.py — measure the sparse causal chunk attention hot path (append -> select -> attention) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 1k|2k|wide|1k_stream] [--impl reference]
+
+One "step" = one pass of the whole hot path over one chunk of synthetic
+input shaped like BASELINE.json configs[1] (default; `--workload` picks another).  Prints ONE JSON line
+(the contract is in DESIGN.md §"Measurement").  `value` = effective TFLOP/s counting only kept blocks,
+over the whole step with inputs resident in HBM; `ms_per_step` = ms/chunk; `e2e` = the same through the
+C ABI with pinned HOST buffers (H2D of Q,K,V and D2H of O inside the timed region); `roofline` = the
+attention kernel alone against the measured bf16 tensor peak; `cpu_baseline` = the fp64 oracle timed on
+this box's host cores on a bounded sample.  Multi-GPU = independent replicas (the path does
+not shard by contract), one rank per GPU, max-over-ranks timing.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import uf_workloads as wl  # noqa: E402
+
+METRIC = "effective TFLOP/s on kept blocks, sparse causal chunk attention step (ms/chunk in ms_per_step)"
+UNIT = "TFLOP/s"
+
+
+# --------------------------------------------------------------------------------------------------
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        p = json.load(open(path))
+        return {"bf16_burst": float(p["bf16_tflops"]), "bf16_sustained": float(p["bf16_tflops_sustained"]),
+                "hbm_gbs": float(p["hbm_gbs"]), "source": "measured (MEASURED_PEAKS.json)"}
+    return {"bf16_burst": 1590.0, "bf16_sustained": 1400.0, "hbm_gbs": 6650.0,
+            "source": "fallback (B200_PROFILING.md)"}
+
+
+def kept_flop(w: wl.Workload, n_tok: int, idx: np.ndarray, sink_tok: int, prior_ntok: dict[int, int]) -> int:
+    """4*d*sum over (h, i) of valid q rows x valid kept keys; bookkeeping from the index
+    lists the library returned — no method arithmetic."""
+    B, d, bpc = w.block, w.head_dim, -(-w.chunk_tokens // w.block)
+    nqb = -(-n_tok // B)
+    rows = np.minimum(B, n_tok - np.arange(nqb) * B).astype(np.int64)             # [nqb]
+    if idx.size:
+        cid, b = idx // bpc, idx % bpc
+        ntok = np.vectorize(lambda c: prior_ntok[int(c)])(cid)
+        keys_topk = np.minimum(B, ntok - b * B).astype(np.int64).sum(axis=2)      # [H, nqb]
+    else:
+        keys_topk = np.zeros((w.n_heads, nqb), dtype=np.int64)
+    keys = keys_topk + sink_tok + n_tok
+    return int(4 * d * (rows[None, :] * keys).sum())
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, device: int):
+        self.rows, self.proc, self.device = [], None, device
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.device}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+        return self
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def __exit__(self, *a):
+        if self.proc:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=2)
+            except Exception:
+                self.proc.kill()
+
+    def summary(self):
+        sm, mx, reasons = [], 0.0, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx = max(mx, float(r[1]))
+                for n, v in zip(names, r[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(n)
+            except Exception:
+                pass
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        hi = [x for x in sm if x >= 0.5 * max(sm)] or sm
+        return {"sm_mhz": float(np.median(hi)), "sm_max_mhz": mx, "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# --------------------------------------------------------------------------------------------------
+def dist_setup(n_gpus: int):
+    """One process per GPU under torchrun; returns (rank, world, local_rank)."""
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        import torch.distributed as dist
+        if not dist.is_initialized():
+            backend = os.environ.get("UF_DIST_BACKEND", "nccl")
+            dist.init_process_group(backend=backend)
+    return rank, world, local
+
+
+def aggregate_over_ranks(elapsed_ms: float, units: float, device=None):
+    """Replicas only: time = max over ranks, units = sum over ranks (no data-path collective)."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return elapsed_ms, units
+    dev = device if device is not None else torch.device("cpu")
+    t = torch.tensor([elapsed_ms], dtype=torch.float64, device=dev)
+    u = torch.tensor([units], dtype=torch.float64, device=dev)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
+def barrier():
+    import torch.distributed as dist
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.barrier()
+
+
+# --------------------------------------------------------------------------------------------------
+class HotPath:
+    """The step bench.py times: uf_kv_append -> uf_select_blocks -> uf_sparse_attn_fwd via the C ABI."""
+
+    def __init__(self, w: wl.Workload, device: int, n_distinct: int):
+        import torch
+        import paper_2606_09150_b200 as uf
+        self.torch, self.uf, self.w = torch, uf, w
+        self.dev = torch.device("cuda", device)
+        torch.cuda.set_device(self.dev)
+        self.ctx = uf.uf_ctx_create(w.n_heads, w.head_dim, w.block, w.chunk_tokens, w.capacity_chunks,
+                                    w.sink_blocks, w.k_min, device)
+        self.stream = torch.cuda.current_stream(self.dev)
+        self.n, self.H, self.d = w.chunk_tokens, w.n_heads, w.head_dim
+        self.ts, self.hs = self.H * self.d, self.d
+        self.host = []      # pinned host chunks (int16 views of bf16 bits)
+        self.devc = []      # device-resident chunks
+        for c in range(n_distinct):
+            qb, kb, vb = wl.make_chunk(w, c)
+            hq, hk, hv = (torch.from_numpy(x.view(np.int16)).pin_memory() for x in (qb, kb, vb))
+            self.host.append((hq, hk, hv))
+            self.devc.append(tuple(t.to(self.dev, non_blocking=True).view(torch.bfloat16) for t in (hq, hk, hv)))
+        nqb = -(-self.n // w.block)
+        kmax = max(1, (w.capacity_chunks - 1) * w.bpc)
+        self.idx = torch.zeros((self.H, nqb, kmax), dtype=torch.int32, device=self.dev)
+        self.cnt = torch.zeros((self.H, nqb), dtype=torch.int32, device=self.dev)
+        self.o = torch.zeros((self.n, self.H, self.d), dtype=torch.bfloat16, device=self.dev)
+        self.lse = torch.zeros((self.H, self.n), dtype=torch.float32, device=self.dev)
+        # e2e staging: device inputs filled by H2D, pinned host output
+        self.stage = tuple(torch.empty((self.n, self.H, self.d), dtype=torch.bfloat16, device=self.dev) for _ in range(3))
+        self.o_host = torch.empty((self.n, self.H, self.d), dtype=torch.bfloat16).pin_memory()
+        self.step_no = 0
+        torch.cuda.synchronize(self.dev)
+
+    def close(self):
+        self.uf.uf_ctx_destroy(self.ctx)
+
+    def step(self, q, k, v, ev=None):
+        uf, w = self.uf, self.w
+        uf.uf_kv_append(self.ctx, k, v, self.n, self.ts, self.hs, 0, self.stream)
+        uf.uf_select_blocks(self.ctx, q, self.n, self.ts, self.hs, w.topk_count, w.topk_percent,
+                            self.idx, self.cnt, self.stream)
+        if ev is not None:
+            ev[0].record(self.stream)
+        uf.uf_sparse_attn_fwd(self.ctx, q, self.o, self.lse, self.n, self.ts, self.hs, 0.0, self.stream)
+        if ev is not None:
+            ev[1].record(self.stream)
+        self.step_no += 1
+
+    def step_resident(self, ev=None):
+        q, k, v = self.devc[self.step_no % len(self.devc)]
+        self.step(q, k, v, ev)
+
+    def step_e2e(self):
+        hq, hk, hv = self.host[self.step_no % len(self.host)]
+        sq, sk, sv = self.stage
+        sq.view(self.torch.int16).copy_(hq, non_blocking=True)
+        sk.view(self.torch.int16).copy_(hk, non_blocking=True)
+        sv.view(self.torch.int16).copy_(hv, non_blocking=True)
+        self.step(sq, sk, sv)
+        self.o_host.copy_(self.o, non_blocking=True)
+
+    def current_kept_flop(self):
+        """FLOP of the step just run, from the returned index lists."""
+        uf, w = self.uf, self.w
+        self.torch.cuda.synchronize(self.dev)
+        n_cand, k_eff = uf.uf_query_topk(self.ctx, w.topk_count, w.topk_percent)
+        idx = self.idx.cpu().numpy().reshape(-1)[: self.H * self.idx.shape[1] * k_eff].reshape(self.H, self.idx.shape[1], k_eff)
+        slot_map, _, newest = uf.uf_get_slot_map(self.ctx, w.capacity_chunks)
+        prior = {c: self.n for c in slot_map if c >= 0}
+        sink_tok = min(w.sink_blocks * w.block, self.n) if newest > 0 else 0
+        return kept_flop(w, self.n, idx, sink_tok, prior), n_cand, k_eff
+
+
+def time_steps(hp: HotPath, steps: int, warmup: int, e2e: bool):
+    torch = hp.torch
+    for _ in range(warmup):
+        hp.step_e2e() if e2e else hp.step_resident()
+    torch.cuda.synchronize(hp.dev)
+    barrier()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    attn_ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    launches0 = hp.uf.uf_ctx_launch_count(hp.ctx)
+    ev0.record(hp.stream)
+    for i in range(steps):
+        if e2e:
+            hp.step_e2e()
+        else:
+            hp.step_resident(attn_ev[i])
+    ev1.record(hp.stream)
+    torch.cuda.synchronize(hp.dev)
+    barrier()
+    total_ms = ev0.elapsed_time(ev1)
+    attn_ms = None if e2e else float(np.mean([a.elapsed_time(b) for a, b in attn_ev]))
+    launches = hp.uf.uf_ctx_launch_count(hp.ctx) - launches0
+    return total_ms, attn_ms, launches
+
+
+def stream_percentiles(hp: HotPath, repeats: int):
+    """configs[3]: 20-chunk rolling stream, per-chunk ms; p50/p99 over steady-state chunks (c >= C)."""
+    torch, w = hp.torch, hp.w
+    per = []
+    for rep in range(repeats + 1):
+        hp.uf.uf_ctx_reset(hp.ctx, hp.stream)
+        hp.step_no = 0
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(w.n_stream_chunks)]
+        for c in range(w.n_stream_chunks):
+            evs[c][0].record(hp.stream)
+            hp.step_resident()
+            evs[c][1].record(hp.stream)
+        torch.cuda.synchronize(hp.dev)
+        if rep:
+            per.append([a.elapsed_time(b) for a, b in evs])
+    per = np.asarray(per)
+    steady = per[:, w.capacity_chunks:].reshape(-1)
+    return {"p50_ms": float(np.percentile(steady, 50)), "p99_ms": float(np.percentile(steady, 99)),
+            "rampup_ms": [float(x) for x in per[:, :w.capacity_chunks].mean(axis=0)], "repeats": repeats}
+
+
+# --------------------------------------------------------------------------------------------------
+def cpu_oracle_sample(w: wl.Workload, budget_s: float = 20.0, max_pairs: int = 16):
+    """The fp64 oracle as it stands, on this box's host cores, on a bounded sample of the workload:
+    all prior appends + full selection of the timed chunk + attention on sampled (head, query-block) pairs.
+    Returns (TFLOP/s over the sample's kept FLOP, cores, description)."""
+    from oracle.uf_oracle import UFOracle
+    cores = len(os.sched_getaffinity(0))
+    orc = UFOracle(w.n_heads, w.head_dim, w.block, w.chunk_tokens, w.capacity_chunks, w.sink_blocks, w.k_min)
+    f64 = lambda b: wl.bf16_bits_to_f32(b).astype(np.float64)  # noqa: E731
+    for c in range(w.prior_chunks):
+        _, kb, vb = wl.make_chunk(w, c)
+        orc.kv_append(f64(kb), f64(vb))
+    qb, kb, vb = wl.make_chunk(w, w.prior_chunks)
+    Q, K, V = f64(qb), f64(kb), f64(vb)
+    t0 = time.perf_counter()
+    orc.kv_append(K, V)
+    t_app = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    orc.select_blocks(Q, w.topk_count, w.topk_percent)
+    t_sel = time.perf_counter() - t0
+    rng = np.random.default_rng(0)
+    nqb = w.bpc
+    t_attn, flop, pairs = 0.0, 0, 0
+    while pairs < max_pairs and (t_attn < budget_s or pairs < 2):
+        h, i = int(rng.integers(0, w.n_heads)), int(rng.integers(0, nqb))
+        t0 = time.perf_counter()
+        orc.sparse_attn(Q, heads=[h], qblocks=[i])
+        t_attn += time.perf_counter() - t0
+        rows = min((i + 1) * w.block, w.chunk_tokens) - i * w.block
+        keys = sum(orc.block_kv(g, fs)[0].shape[0] for g, fs in orc.kept_blocks(h, i))
+        flop += 4 * w.head_dim * rows * keys
+        pairs += 1
+    desc = (f"oracle/uf_oracle.py (NumPy fp64): append {t_app:.2f}s + full selection {t_sel:.2f}s (not in value) + "
+            f"attention on {pairs} random (head, query-block) pairs of {w.n_heads * nqb} in {t_attn:.2f}s; "
+            f"value = sampled kept FLOP / attention time")
+    return flop / t_attn / 1e12, cores, desc, t_attn, pairs
+
+
+def run_reference(args, w):
+    """--impl reference: the oracle timed on host cores; rank 0 only."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    vals = []
+    for _ in range(args.warmup if args.warmup < 1 else 1):
+        cpu_oracle_sample(w, budget_s=1.0, max_pairs=2)
+    t_all = 0.0
+    for _ in range(max(1, min(args.steps, 3))):
+        v, cores, desc, t, pairs = cpu_oracle_sample(w, budget_s=8.0, max_pairs=8)
+        vals.append(v); t_all += t
+    value = float(np.mean(vals))
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": len(vals), "warmup": 1, "ms_per_step": 1e3 * t_all / len(vals), "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w.name, "note": "each step = a bounded sample of the workload (see cpu_baseline.sample)"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# --------------------------------------------------------------------------------------------------
+def measure_workload(w, device, steps, warmup, with_e2e=True):
+    n_distinct = w.capacity_chunks + 1 if not w.n_stream_chunks else min(w.n_stream_chunks, 4)
+    hp = HotPath(w, device, n_distinct)
+    try:
+        # reach steady state (chunk 0 evicted, all slots used) before anything is timed
+        for _ in range(w.capacity_chunks + 1):
+            hp.step_resident()
+        with ClockSampler(device) as cs:
+            total_ms, attn_ms, launches = time_steps(hp, steps, warmup, e2e=False)
+        flop, n_cand, k_eff = hp.current_kept_flop()
+        out = {"total_ms": total_ms, "attn_ms": attn_ms, "launches": launches, "flop": flop, "n_cand": n_cand,
+               "k_eff": k_eff, "clocks": cs.summary(), "device_bytes": hp.uf.uf_ctx_device_bytes(hp.ctx)}
+        if with_e2e:
+            e2e_ms, _, _ = time_steps(hp, steps, min(warmup, 3), e2e=True)
+            out["e2e_ms"] = e2e_ms
+            out["h2d"] = 3 * hp.n * hp.H * hp.d * 2
+            out["d2h"] = hp.n * hp.H * hp.d * 2
+        if w.n_stream_chunks:
+            out["stream"] = stream_percentiles(hp, repeats=3)
+        return out
+    finally:
+        hp.close()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--workload", default="1k", choices=["1k", "2k", "wide", "1k_stream"])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-also", action="store_true", help="skip the secondary 2K measurement")
+    args = ap.parse_args()
+    w = wl.CONFIGS[args.workload]
+    if args.impl == "reference":
+        run_reference(args, w)
+        return
+    warmup = max(3, args.warmup)
+
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    rank, world, local = dist_setup(args.gpus)
+    device = local if world > 1 else 0
+    peaks = load_peaks()
+
+    m = measure_workload(w, device, args.steps, warmup)
+    dev = torch.device("cuda", device)
+    total_ms, units = aggregate_over_ranks(m["total_ms"], float(m["flop"]) * args.steps, dev)
+    e2e_ms, _ = aggregate_over_ranks(m["e2e_ms"], 0.0, dev)
+    n_ranks = world
+    value = units / (total_ms * 1e-3) / 1e12
+    e2e_value = units / (e2e_ms * 1e-3) / 1e12
+    attn_tflops = m["flop"] / (m["attn_ms"] * 1e-3) / 1e12
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": n_ranks, "steps": args.steps, "warmup": warmup,
+        "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "bf16", "data": "synthetic",
+        "config": {
+            "workload": f"{w.name} (BASELINE.json configs: {w.n_heads} heads x {w.head_dim}, chunk {w.chunk_tokens} tokens, "
+                        f"block {w.block}, capacity {w.capacity_chunks} chunks + sink, keep {w.topk_percent}% of {m['n_cand']} "
+                        f"cache blocks = {m['k_eff']})",
+            "step": "uf_kv_append -> uf_select_blocks -> uf_sparse_attn_fwd, steady-state rolling cache",
+            "kept_tflop_per_step": m["flop"] / 1e12,
+            "l2": "inputs larger than L2 (Q,K,V 3 x %.0f MB + cache %.0f MB per step; no explicit flush)" % (
+                m["d2h"] / 1e6, 2 * m["d2h"] * w.capacity_chunks / 1e6),
+            "parallelism": "replicas only" if n_ranks > 1 else "single GPU",
+            "attn_ms": m["attn_ms"], "append_select_ms": total_ms / args.steps - m["attn_ms"] if n_ranks == 1 else None,
+            "ctx_device_bytes": m["device_bytes"],
+        },
+        "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms / args.steps,
+                "h2d_bytes_per_step": m["h2d"], "d2h_bytes_per_step": m["d2h"]},
+        "gpu_launches": m["launches"],
+        "clocks": m["clocks"],
+        "roofline": {
+            "kernel": "uf_attn_sm100_kernel", "bound": "tensor", "achieved": attn_tflops, "peak": peaks["bf16_burst"],
+            "unit": "TFLOP/s", "frac": attn_tflops / peaks["bf16_burst"], "traffic": None,
+            "peak_source": peaks["source"] + ", bf16 burst; sustained %.1f -> frac %.3f" % (
+                peaks["bf16_sustained"], attn_tflops / peaks["bf16_sustained"]),
+            "algorithmic_flop_per_launch": m["flop"],
+        },
+    }
+    if rank == 0 and not args.no_also and args.workload == "1k":
+        m2 = measure_workload(wl.CONFIGS["2k"], device, max(3, args.steps // 2), 3, with_e2e=False)
+        t2 = m2["flop"] / (m2["attn_ms"] * 1e-3) / 1e12
+        line["also"] = {"2k": {"ms_per_step": m2["total_ms"] / max(3, args.steps // 2), "attn_ms": m2["attn_ms"],
+                               "kept_tflop_per_step": m2["flop"] / 1e12,
+                               "value": m2["flop"] / (m2["total_ms"] / max(3, args.steps // 2) * 1e-3) / 1e12,
+                               "attn_tflops": t2, "attn_frac_of_burst_peak": t2 / peaks["bf16_burst"],
+                               "k_eff": m2["k_eff"], "n_cand": m2["n_cand"], "clocks": m2["clocks"]}}
+    if "stream" in m:
+        line["stream"] = m["stream"]
+    if rank == 0 and n_ranks == 1 and not args.no_cpu_baseline:
+        v, cores, desc, _, _ = cpu_oracle_sample(w)
+        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
