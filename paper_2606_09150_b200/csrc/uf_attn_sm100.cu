@@ -23,6 +23,7 @@
 #include "uf_internal.h"
 
 #include <cstdio>
+#include <cstdlib>
 
 namespace {
 
@@ -32,6 +33,11 @@ constexpr int kTile = 128 * 128 * 2;   // bytes of one 128 x 128 bf16 tile
 constexpr int kHalf = kTile / 2;       // one 64-column box
 constexpr int kThreads = 384;
 constexpr float kRescaleThreshold = 8.0f;   // log2 units
+#ifdef UF_ARRIVE_ALL
+constexpr uint32_t kPArrivals = 128;        // every softmax thread arrives on P_FULL
+#else
+constexpr uint32_t kPArrivals = 4;          // one elected lane per softmax warp arrives on P_FULL
+#endif
 
 // smem carve-up (offsets from a 1024-aligned base)
 constexpr int kOffQ = 0;                          // 2 tiles
@@ -140,18 +146,151 @@ __device__ __forceinline__ void mma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_
         "r"(a[o + 30]), "r"(a[o + 31])                                                                         \
       : "memory")
 
+// One lane of a converged warp (the same one every time).  tcgen05.mma / tcgen05.commit / TMA take their
+// operands from uniform registers: issued under elect.sync from warp-uniform control flow, ptxas emits them
+// straight-line; issued from an `if (lane == 0)` region it wraps EACH one in an ELECT/R2UR/BRA loop
+// (~13 instructions, ~70 cycles per MMA: slower than the 64-cycle MMA itself).
+__device__ __forceinline__ bool elect_one() {
+  uint32_t pred;
+  asm volatile(
+      "{\n\t"
+      ".reg .pred p;\n\t"
+      "elect.sync _|p, 0xffffffff;\n\t"
+      "selp.b32 %0, 1, 0, p;\n\t"
+      "}" : "=r"(pred));
+  return pred != 0;
+}
+// a loaded value every lane holds anyway, made provably warp-uniform for the compiler
+__device__ __forceinline__ int32_t uniform_i32(int32_t v) { return __shfl_sync(0xffffffffu, v, 0); }
+
 __device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 
 __device__ __forceinline__ float ex2(float x) {
   float y;
+#ifdef UF_DBG_NOMUFU
+  y = x * 0.5f;
+#else
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+#endif
   return y;
 }
 __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
   uint32_t r;
   asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
   return r;
+}
+
+// ---- packed fp32x2 arithmetic (FFMA2 / FADD2: two lanes per issue slot) and 3-input max (FMNMX3) ----
+__device__ __forceinline__ uint64_t pack2(float lo, float hi) {
+  uint64_t r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ void unpack2(uint64_t v, float& lo, float& hi) {
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ uint64_t fma2(uint64_t a, uint64_t b, uint64_t c) {
+  uint64_t d;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+  return d;
+}
+__device__ __forceinline__ uint64_t add2(uint64_t a, uint64_t b) {
+  uint64_t d;
+  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+  return d;
+}
+__device__ __forceinline__ uint64_t add2_rm(uint64_t a, uint64_t b) {
+  uint64_t d;
+  asm("add.rm.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+  return d;
+}
+__device__ __forceinline__ uint64_t sub2(uint64_t a, uint64_t b) {
+  uint64_t d;
+  asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+  return d;
+}
+__device__ __forceinline__ float max3(float a, float b, float c) {
+  float d;
+  asm("max.f32 %0, %1, %2, %3;" : "=f"(d) : "f"(a), "f"(b), "f"(c));
+  return d;
+}
+
+// The MUFU (16 ex2 / cycle / SM) needs as many cycles per 128 x 128 tile as the tensor pipe needs for
+// its two MMAs, so a share of the exponentials is computed on the FMA pipe instead: kEmuPairs of every
+// 8 column pairs.  2^x = 2^floor(x) * 2^frac(x): floor via the round-down magic-number add (the integer
+// lands in the low mantissa bits), 2^frac by a degree-3 minimax polynomial on [0,1) (max relative error
+// 7.5e-5, far below the bf16 rounding of P), the exponent added into the float's bits by one LEA.
+// Valid for -126 <= x (clamped: the polynomial can return 1 - 7.5e-5, exponent field 126) and x <= 8 (guaranteed by the lazy-rescale invariant).
+#ifndef UF_EMU_PAIRS
+#define UF_EMU_PAIRS 3
+#endif
+constexpr int kEmuPairs = UF_EMU_PAIRS;
+__device__ __forceinline__ constexpr bool pair_emulated(int j) { return ((j & 7) * kEmuPairs) % 8 < kEmuPairs; }
+
+__device__ __forceinline__ uint64_t ex2_pair(uint64_t x, bool emulate) {
+  float x0, x1;
+  unpack2(x, x0, x1);
+  if (!emulate) return pack2(ex2(x0), ex2(x1));
+  const uint64_t magic = pack2(12582912.0f, 12582912.0f);            // 2^23 + 2^22
+  x = pack2(fmaxf(x0, -126.0f), fmaxf(x1, -126.0f));
+  const uint64_t r = add2_rm(x, magic);
+  const uint64_t fr = sub2(x, sub2(r, magic));
+  uint64_t p = fma2(fr, pack2(0.07802452147006989f, 0.07802452147006989f), pack2(0.22606715559959412f, 0.22606715559959412f));
+  p = fma2(p, fr, pack2(0.6958335638046265f, 0.6958335638046265f));
+  p = fma2(p, fr, pack2(0.9999251961708069f, 0.9999251961708069f));
+  float p0, p1, r0, r1;
+  unpack2(p, p0, p1);
+  unpack2(r, r0, r1);
+  p0 = __int_as_float((__float_as_int(r0) << 23) + __float_as_int(p0));
+  p1 = __int_as_float((__float_as_int(r1) << 23) + __float_as_int(p1));
+  return pack2(p0, p1);
+}
+
+// One softmax pass over a loaded S row (128 logits in s[]): p = 2^(s*sl2 - m) into bf16 pairs pk[],
+// returns the fp32 row sum; with kWithMax also the raw row max (computed beside the exponentials, not
+// before them: the running max m used here is the one from the previous key blocks).
+template <bool kWithMax>
+__device__ __forceinline__ float exp_pass(const uint32_t (&s)[128], uint32_t (&pk)[64], float m, float sl2, float& rowmax) {
+  const uint64_t nm2 = pack2(-m, -m), sl22 = pack2(sl2, sl2);
+  uint64_t acc0 = pack2(0.f, 0.f), acc1 = acc0;
+  float mx0 = -INFINITY, mx1 = -INFINITY, mx2 = -INFINITY, mx3 = -INFINITY;
+#pragma unroll
+  for (int c = 0; c < 128; c += 8) {
+#pragma unroll
+    for (int u = 0; u < 8; u += 2) {
+      const int j = (c + u) >> 1;
+      const uint64_t x = fma2(pack2(__uint_as_float(s[c + u]), __uint_as_float(s[c + u + 1])), sl22, nm2);
+      const uint64_t p = ex2_pair(x, pair_emulated(j));
+      if (j & 1) acc1 = add2(acc1, p); else acc0 = add2(acc0, p);
+      float p0, p1;
+      unpack2(p, p0, p1);
+      pk[j] = pack_bf16x2(p0, p1);
+    }
+    if (kWithMax) {
+      mx0 = max3(mx0, __uint_as_float(s[c + 0]), __uint_as_float(s[c + 1]));
+      mx1 = max3(mx1, __uint_as_float(s[c + 2]), __uint_as_float(s[c + 3]));
+      mx2 = max3(mx2, __uint_as_float(s[c + 4]), __uint_as_float(s[c + 5]));
+      mx3 = max3(mx3, __uint_as_float(s[c + 6]), __uint_as_float(s[c + 7]));
+    }
+  }
+  if (kWithMax) rowmax = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3));
+  float a0, a1, b0, b1;
+  unpack2(acc0, a0, a1);
+  unpack2(acc1, b0, b1);
+  return (a0 + a1) + (b0 + b1);
+}
+
+__device__ __forceinline__ float max_pass(const uint32_t (&s)[128]) {
+  float mx0 = -INFINITY, mx1 = -INFINITY, mx2 = -INFINITY, mx3 = -INFINITY;
+#pragma unroll
+  for (int c = 0; c < 128; c += 8) {
+    mx0 = max3(mx0, __uint_as_float(s[c + 0]), __uint_as_float(s[c + 1]));
+    mx1 = max3(mx1, __uint_as_float(s[c + 2]), __uint_as_float(s[c + 3]));
+    mx2 = max3(mx2, __uint_as_float(s[c + 4]), __uint_as_float(s[c + 5]));
+    mx3 = max3(mx3, __uint_as_float(s[c + 6]), __uint_as_float(s[c + 7]));
+  }
+  return fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3));
 }
 
 // shared-memory matrix descriptor, 128-byte swizzle
@@ -163,6 +302,15 @@ __device__ __forceinline__ uint64_t make_desc(uint32_t saddr, uint32_t lbo_bytes
 // instruction descriptor kind::f16: D fp32, A/B bf16, M = N = 128; B MN-major for P V
 constexpr uint32_t kIdescQK = (1u << 4) | (1u << 7) | (1u << 10) | ((128u >> 3) << 17) | ((128u >> 4) << 24);
 constexpr uint32_t kIdescPV = kIdescQK | (1u << 16);
+
+#ifdef UF_DBG_TRACE
+// debug only: clock64 timestamps of CTA 0's first kTraceSteps steps; roles: 0 = MMA thread, 1 = softmax tile 0, 2 = softmax tile 1
+constexpr int kTraceSteps = 600;
+__device__ long long uf_trace[3][kTraceSteps][8];
+#define UF_TR(role, step, slot) do { if (blockIdx.x == 0 && (step) < kTraceSteps) uf_trace[role][step][slot] = clock64(); } while (0)
+#else
+#define UF_TR(role, step, slot) do { } while (0)
+#endif
 
 struct AttnParams {
   const int32_t* sel_pair;   // [H][NP][2*kcap]
@@ -180,20 +328,22 @@ struct Item {
   const int32_t* ulist;
 };
 
+template <bool kUniform = false>
 __device__ __forceinline__ Item get_item(const AttnParams& a, int it) {
   Item x;
   x.h = it / a.np_cur;
   x.p = it % a.np_cur;
   const int64_t pi = (int64_t)x.h * a.NP + x.p;
-  x.n_u = a.pair_cnt[pi];
+  x.n_u = kUniform ? uniform_i32(a.pair_cnt[pi]) : a.pair_cnt[pi];
   x.ulist = a.sel_pair + pi * 2 * a.kcap;
   x.n_steps = x.n_u + a.n_sink + a.nqb;
   x.full_mask = (2 * x.p + 1 < a.nqb) ? 3 : 1;
   return x;
 }
 
+template <bool kUniform = false>
 __device__ __forceinline__ int32_t get_entry(const AttnParams& a, const Item& x, int st) {
-  if (st < x.n_u) return __ldg(x.ulist + st);
+  if (st < x.n_u) return kUniform ? uniform_i32(__ldg(x.ulist + st)) : __ldg(x.ulist + st);
   st -= x.n_u;
   if (st < a.n_sink) return uf_entry_pack(st, min(128, a.sink_ntok - st * 128), x.full_mask);
   st -= a.n_sink;
@@ -222,7 +372,7 @@ uf_attn_sm100_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_cons
   if (warp == 9 && lane == 0) {
     for (int i = 0; i < kNumBars; ++i) {
       const bool softmax_arrives = (i == P_FULL0 || i == P_FULL1);
-      mbar_init(bars + i * 8, softmax_arrives ? 128u : 1u);
+      mbar_init(bars + i * 8, softmax_arrives ? kPArrivals : 1u);
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     fence_proxy_async();
@@ -235,57 +385,77 @@ uf_attn_sm100_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_cons
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = *tmem_ptr_smem;
+#ifdef UF_DBG_CLOCK
+  unsigned long long dbg_c0 = 0, dbg_t0 = 0;
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    dbg_c0 = clock64();
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(dbg_t0));
+  }
+#endif
 
   if (warp >= 8) {
-    asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
-    if (warp == 8 && lane == 0) {
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 80;");
+    if (warp == 8) {
       // ================================ TMA producer ================================
+      // (whole warp runs the control flow; the elected lane issues expect_tx + TMA)
       uint32_t kcount = 0, vcount = 0, qn[2] = {0, 0};
       for (int it = blockIdx.x; it < n_items; it += gridDim.x) {
-        const Item x = get_item(a, it);
+        const Item x = get_item<true>(a, it);
         for (int t = 0; t < 2; ++t) {
           if (!(x.full_mask & (1 << t))) continue;
           const uint32_t bq = bars + (Q_FULL0 + t) * 8;
           mbar_wait(bars + (Q_EMPTY0 + t) * 8, (qn[t] & 1) ^ 1);
-          mbar_expect_tx(bq, kTile);
           const int row0 = (2 * x.p + t) * 128;
-          tma_load_3d(base + kOffQ + t * kTile, &tm_q, bq, 0, row0, x.h);
-          tma_load_3d(base + kOffQ + t * kTile + kHalf, &tm_q, bq, 64, row0, x.h);
+          if (elect_one()) {
+            mbar_expect_tx(bq, kTile);
+            tma_load_3d(base + kOffQ + t * kTile, &tm_q, bq, 0, row0, x.h);
+            tma_load_3d(base + kOffQ + t * kTile + kHalf, &tm_q, bq, 64, row0, x.h);
+          }
           ++qn[t];
         }
-        int32_t e = get_entry(a, x, 0);
+        int32_t e = get_entry<true>(a, x, 0);
         for (int st = 0; st < x.n_steps; ++st) {
-          const int32_t en = (st + 1 < x.n_steps) ? get_entry(a, x, st + 1) : 0;
+          const int32_t en = (st + 1 < x.n_steps) ? get_entry<true>(a, x, st + 1) : 0;
           const int row = uf_entry_phys(e) * 128;
           {
             const uint32_t s = kcount % kNK, n = kcount / kNK;
             const uint32_t bf = bars + (K_FULL0 + s) * 8;
             mbar_wait(bars + (K_EMPTY0 + s) * 8, (n & 1) ^ 1);
+#ifdef UF_DBG_NOTMA
+            if (kcount >= kNK) { if (elect_one()) mbar_arrive(bf); } else
+#endif
+            if (elect_one()) {
             mbar_expect_tx(bf, kTile);
             tma_load_3d(base + kOffK + s * kTile, &tm_k, bf, 0, row, x.h);
             tma_load_3d(base + kOffK + s * kTile + kHalf, &tm_k, bf, 64, row, x.h);
+            }
             ++kcount;
           }
           {
             const uint32_t s = vcount % kNV, n = vcount / kNV;
             const uint32_t bf = bars + (V_FULL0 + s) * 8;
             mbar_wait(bars + (V_EMPTY0 + s) * 8, (n & 1) ^ 1);
+#ifdef UF_DBG_NOTMA
+            if (vcount >= kNV) { if (elect_one()) mbar_arrive(bf); } else
+#endif
+            if (elect_one()) {
             mbar_expect_tx(bf, kTile);
             tma_load_3d(base + kOffV + s * kTile, &tm_v, bf, 0, row, x.h);
             tma_load_3d(base + kOffV + s * kTile + kHalf, &tm_v, bf, 64, row, x.h);
+            }
             ++vcount;
           }
           e = en;
         }
       }
-    } else if (warp == 9 && lane == 0) {
+    } else if (warp == 9) {
       // ================================ MMA issuer ==================================
+      // (whole warp runs the control flow and the barrier waits; the elected lane issues MMAs and commits)
       uint32_t kcount = 0, vcount = 0, qn[2] = {0, 0}, pn[2] = {0, 0};
-      int vrem[kNV];
-#pragma unroll
-      for (int i = 0; i < kNV; ++i) vrem[i] = 0;
+      static_assert(kNV == 2, "vrem0/vrem1 below assume a 2-stage V ring");
+      int vrem0 = 0, vrem1 = 0;                      // tiles that still have to consume V stage 0 / 1
       for (int it = blockIdx.x; it < n_items; it += gridDim.x) {
-        const Item x = get_item(a, it);
+        const Item x = get_item<true>(a, it);
         bool pend[2] = {false, false};
         uint32_t pend_vs[2] = {0, 0}, pend_vpar[2] = {0, 0};
         bool first_pv[2] = {true, true};
@@ -293,32 +463,43 @@ uf_attn_sm100_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_cons
           if (x.full_mask & (1 << t)) { mbar_wait(bars + (Q_FULL0 + t) * 8, qn[t] & 1); ++qn[t]; }
 
         auto do_pv = [&](int t) {
+          UF_TR(0, (int)kcount, t * 2);
           mbar_wait(bars + (P_FULL0 + t) * 8, pn[t] & 1); ++pn[t];
+          UF_TR(0, (int)kcount, t * 2 + 1);
           const uint32_t vs = pend_vs[t];
           mbar_wait(bars + (V_FULL0 + vs) * 8, pend_vpar[t]);
           tc_fence_after();
           const uint32_t vaddr = base + kOffV + vs * kTile;
           const uint32_t d_tmem = tmem + 256 + t * 128;
           const uint32_t p_tmem = tmem + t * 128;
+          const int left = (vs == 0) ? --vrem0 : --vrem1;
+          if (elect_one()) {
 #pragma unroll
-          for (int k = 0; k < 8; ++k) {
-            // B = V tile, MN-major: 8-key groups 1024 B apart (SBO), the two 64-column halves 16 KB apart (LBO)
-            const uint64_t bd = make_desc(vaddr + k * 2048, kHalf, 1024);
-            mma_ts(d_tmem, p_tmem + k * 8, bd, kIdescPV, (first_pv[t] && k == 0) ? 0u : 1u);
+            for (int k = 0; k < 8; ++k) {
+              // B = V tile, MN-major: 8-key groups 1024 B apart (SBO), the two 64-column halves 16 KB apart (LBO)
+              const uint64_t bd = make_desc(vaddr + k * 2048, kHalf, 1024);
+#ifndef UF_DBG_NOPV
+              mma_ts(d_tmem, p_tmem + k * 8, bd, kIdescPV, (first_pv[t] && k == 0) ? 0u : 1u);
+#endif
+            }
+            if (left == 0) tc_commit(bars + (V_EMPTY0 + vs) * 8);
           }
+          __syncwarp();
           first_pv[t] = false;
-          if (--vrem[vs] == 0) tc_commit(bars + (V_EMPTY0 + vs) * 8);
           pend[t] = false;
         };
 
-        int32_t e = get_entry(a, x, 0);
+        int32_t e = get_entry<true>(a, x, 0);
         for (int st = 0; st < x.n_steps; ++st) {
-          const int32_t en = (st + 1 < x.n_steps) ? get_entry(a, x, st + 1) : 0;
+          const int32_t en = (st + 1 < x.n_steps) ? get_entry<true>(a, x, st + 1) : 0;
           const int m = uf_entry_mask(e);
           const uint32_t ks = kcount % kNK, kpar = (kcount / kNK) & 1;
           const uint32_t vs = vcount % kNV, vpar = (vcount / kNV) & 1;
+          UF_TR(0, (int)kcount, 6);
           mbar_wait(bars + (K_FULL0 + ks) * 8, kpar);
+          UF_TR(0, (int)kcount, 7);
           tc_fence_after();
+          UF_TR(0, (int)kcount, 4);
           const uint32_t kaddr = base + kOffK + ks * kTile;
           int users = 0;
 #pragma unroll
@@ -326,19 +507,26 @@ uf_attn_sm100_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_cons
             if (!(m & (1 << t))) continue;
             if (pend[t]) do_pv(t);
             const uint32_t qaddr = base + kOffQ + t * kTile;
+            if (elect_one()) {
 #pragma unroll
-            for (int k = 0; k < 8; ++k) {
-              // K-major operands: 8-row groups 1024 B apart (SBO); 16 elements = 32 B along K, second half +16 KB
-              const uint32_t koff = (k & 3) * 32 + (k >> 2) * kHalf;
-              mma_ss(tmem + t * 128, make_desc(qaddr + koff, 16, 1024), make_desc(kaddr + koff, 16, 1024), kIdescQK,
-                     k == 0 ? 0u : 1u);
+              for (int k = 0; k < 8; ++k) {
+                // K-major operands: 8-row groups 1024 B apart (SBO); 16 elements = 32 B along K, second half +16 KB
+                const uint32_t koff = (k & 3) * 32 + (k >> 2) * kHalf;
+#ifndef UF_DBG_NOQK
+                mma_ss(tmem + t * 128, make_desc(qaddr + koff, 16, 1024), make_desc(kaddr + koff, 16, 1024), kIdescQK,
+                       k == 0 ? 0u : 1u);
+#endif
+              }
+              tc_commit(bars + (S_FULL0 + t) * 8);
             }
-            tc_commit(bars + (S_FULL0 + t) * 8);
+            __syncwarp();
             pend[t] = true; pend_vs[t] = vs; pend_vpar[t] = vpar;
             ++users;
           }
-          tc_commit(bars + (K_EMPTY0 + ks) * 8);
-          vrem[vs] = users;
+          if (elect_one()) tc_commit(bars + (K_EMPTY0 + ks) * 8);
+          __syncwarp();
+          UF_TR(0, (int)kcount, 5);
+          if (vs == 0) vrem0 = users; else vrem1 = users;
           ++kcount; ++vcount;
 #pragma unroll
           for (int t = 0; t < 2; ++t)
@@ -348,13 +536,16 @@ uf_attn_sm100_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_cons
 #pragma unroll
         for (int t = 0; t < 2; ++t) {
           if (pend[t]) do_pv(t);
-          if (x.full_mask & (1 << t)) tc_commit(bars + (O_FULL0 + t) * 8);
+          if (x.full_mask & (1 << t)) {
+            if (elect_one()) tc_commit(bars + (O_FULL0 + t) * 8);
+            __syncwarp();
+          }
         }
       }
     }
   } else {
     // ================================== softmax + epilogue ==================================
-    asm volatile("setmaxnreg.inc.sync.aligned.u32 224;");
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 208;");
     const int t = warp >> 2;                           // tile
     const int wq = warp & 3;                           // TMEM lane quarter
     const int row = wq * 32 + lane;                    // row in the tile == TMEM lane
@@ -379,32 +570,49 @@ uf_attn_sm100_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_cons
         e = en;
         if (!(uf_entry_mask(ecur) & (1 << t))) continue;
         const int nvalid = uf_entry_nvalid(ecur);
+        if (wq == 0 && lane == 0) UF_TR(1 + t, (int)sn, 0);
         mbar_wait(b_sfull, sn & 1); ++sn;
         tc_fence_after();
+        if (wq == 0 && lane == 0) UF_TR(1 + t, (int)sn - 1, 1);
+#ifdef UF_DBG_NOSOFTMAX
+        l = 1.f;
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(b_pfull);
+        if (wq == 0 && lane == 0) UF_TR(1 + t, (int)sn - 1, 2);
+        continue;
+#endif
         uint32_t s[128];
-        UF_TMEM_LD32(s_tmem + 0, s, 0);
-        UF_TMEM_LD32(s_tmem + 32, s, 32);
-        UF_TMEM_LD32(s_tmem + 64, s, 64);
-        UF_TMEM_LD32(s_tmem + 96, s, 96);
-        tmem_wait_ld();
-        if (nvalid < 128) {
+        uint32_t pk[64];
+        auto load_s = [&]() {
+          UF_TMEM_LD32(s_tmem + 0, s, 0);
+          UF_TMEM_LD32(s_tmem + 32, s, 32);
+          UF_TMEM_LD32(s_tmem + 64, s, 64);
+          UF_TMEM_LD32(s_tmem + 96, s, 96);
+          tmem_wait_ld();
+          if (nvalid < 128) {
 #pragma unroll
-          for (int c = 0; c < 128; ++c)
-            if (c >= nvalid) s[c] = 0xff800000u;       // -inf: ragged key block (R-3)
-        }
-        float mx0 = __uint_as_float(s[0]), mx1 = __uint_as_float(s[1]), mx2 = __uint_as_float(s[2]), mx3 = __uint_as_float(s[3]);
+            for (int c = 0; c < 128; ++c)
+              if (c >= nvalid) s[c] = 0xff800000u;     // -inf: ragged key block (R-3)
+          }
+        };
+        load_s();
+        float lsum, rowmax = 0.f;
+#ifdef UF_DBG_NOEXP
+        lsum = 1.f;
 #pragma unroll
-        for (int c = 4; c < 128; c += 4) {
-          mx0 = fmaxf(mx0, __uint_as_float(s[c]));
-          mx1 = fmaxf(mx1, __uint_as_float(s[c + 1]));
-          mx2 = fmaxf(mx2, __uint_as_float(s[c + 2]));
-          mx3 = fmaxf(mx3, __uint_as_float(s[c + 3]));
-        }
-        const float m_new = fmaxf(m, fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * a.sl2);
+        for (int c = 0; c < 64; ++c) pk[c] = s[c] ^ s[c + 64];
+#else
         if (first) {
-          m = m_new;
+          m = max_pass(s) * a.sl2;
           first = false;
+          lsum = exp_pass<false>(s, pk, m, a.sl2, rowmax);
         } else {
+          // Exponentials against the running max of the EARLIER blocks, the row max of this block
+          // computed beside them: the max -> exp dependency leaves the critical path.  Valid while
+          // the new max exceeds m by at most 2^8 (the lazy-rescale invariant); otherwise redo.
+          lsum = exp_pass<true>(s, pk, m, a.sl2, rowmax);
+          const float m_new = fmaxf(m, rowmax * a.sl2);
           const bool need = (m_new - m) > kRescaleThreshold;
           if (__any_sync(0xffffffffu, need)) {
             // O_t is quiescent here: S_t's commit covers the earlier O_t += P_t V
@@ -419,26 +627,23 @@ uf_attn_sm100_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_cons
               for (int c = 0; c < 32; ++c) ov[c] = __float_as_uint(__uint_as_float(ov[c]) * f);
               UF_TMEM_ST32(o_tmem + cc, ov, 0);
             }
+            load_s();
+            lsum = exp_pass<false>(s, pk, m, a.sl2, rowmax);
           }
         }
-        float l0 = 0.f, l1 = 0.f, l2 = 0.f, l3 = 0.f;
-        uint32_t pk[64];
-#pragma unroll
-        for (int c = 0; c < 128; c += 4) {
-          const float p0 = ex2(fmaf(__uint_as_float(s[c]), a.sl2, -m));
-          const float p1 = ex2(fmaf(__uint_as_float(s[c + 1]), a.sl2, -m));
-          const float p2 = ex2(fmaf(__uint_as_float(s[c + 2]), a.sl2, -m));
-          const float p3 = ex2(fmaf(__uint_as_float(s[c + 3]), a.sl2, -m));
-          l0 += p0; l1 += p1; l2 += p2; l3 += p3;
-          pk[c / 2] = pack_bf16x2(p0, p1);
-          pk[c / 2 + 1] = pack_bf16x2(p2, p3);
-        }
-        l += (l0 + l1) + (l2 + l3);
+#endif
+        l += lsum;
         UF_TMEM_ST32(s_tmem + 0, pk, 0);
         UF_TMEM_ST32(s_tmem + 32, pk, 32);
         tmem_wait_st();
         tc_fence_before();
+#ifdef UF_ARRIVE_ALL
         mbar_arrive(b_pfull);
+#else
+        __syncwarp();
+        if (lane == 0) mbar_arrive(b_pfull);
+#endif
+        if (wq == 0 && lane == 0) UF_TR(1 + t, (int)sn - 1, 2);
       }
       // ---- epilogue: O_t / l -> bf16 -> swizzled staging (Q_t buffer) -> TMA store ----
       mbar_wait(b_ofull, on & 1); ++on;
@@ -480,6 +685,13 @@ uf_attn_sm100_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_cons
 
   tc_fence_before();
   __syncthreads();
+#ifdef UF_DBG_CLOCK
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    unsigned long long c1 = clock64(), t1;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1));
+    printf("UFCLK cycles %llu ns %llu MHz %.1f\n", c1 - dbg_c0, t1 - dbg_t0, 1e3 * (double)(c1 - dbg_c0) / (double)(t1 - dbg_t0));
+  }
+#endif
   if (warp == 10) {
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem) : "memory");
   }
@@ -551,6 +763,14 @@ int uf_launch_attn_sm100(uf_ctx* c, const UfView& v, const __nv_bfloat16* q, __n
   const int grid = n_items < c->sm_count ? n_items : c->sm_count;
   uf_attn_sm100_kernel<<<grid, kThreads, kSmemBytes, s>>>(tm_q, tm_o, c->tm_k, c->tm_v, a);
   c->launches += 1;
+#ifdef UF_DBG_TRACE
+  if (const char* path = getenv("UF_TRACE_PATH")) {
+    cudaDeviceSynchronize();
+    static long long host[3][kTraceSteps][8];
+    cudaMemcpyFromSymbol(host, uf_trace, sizeof(host));
+    if (FILE* f = fopen(path, "wb")) { fwrite(host, 1, sizeof(host), f); fclose(f); }
+  }
+#endif
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) {
     c->err = std::string("uf_attn_sm100_kernel launch: ") + cudaGetErrorString(e);
