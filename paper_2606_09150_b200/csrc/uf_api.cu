@@ -148,6 +148,8 @@ int32_t uf_ctx_create(const uf_config* cfg, uf_ctx** out) {
       {(void**)&c->sel_rank, H * BPC * (int64_t)c->kcap * 4},
       {(void**)&c->sel_pair, H * NP * 2 * (int64_t)c->kcap * 4},
       {(void**)&c->pair_cnt, H * NP * 4},
+      {(void**)&c->panic_item, H * NP * 4},
+      {(void**)&c->panic_last, 4},
   };
   for (auto& a : allocs) {
     e = cudaMalloc(a.p, (size_t)a.bytes);
@@ -161,6 +163,8 @@ int32_t uf_ctx_create(const uf_config* cfg, uf_ctx** out) {
   e = cudaMemset(c->kc, 0, (size_t)cache_bytes);
   if (e == cudaSuccess) e = cudaMemset(c->vc, 0, (size_t)cache_bytes);
   if (e == cudaSuccess) e = cudaMemset(c->kpool, 0, (size_t)(H * d * P * 8));
+  if (e == cudaSuccess) e = cudaMemset(c->panic_item, 0, (size_t)(H * NP * 4));
+  if (e == cudaSuccess) e = cudaMemset(c->panic_last, 0, 4);
   if (e == cudaSuccess) e = cudaDeviceSynchronize();
   if (e != cudaSuccess) { int r = fail_cuda(nullptr, e, "cudaMemset"); uf_ctx_destroy(c); return r; }
   if (cfg->block == 128 && cfg->head_dim == 128) {
@@ -177,6 +181,7 @@ int32_t uf_ctx_destroy(uf_ctx* c) {
     cudaSetDevice(c->cfg.device);
     cudaFree(c->kc); cudaFree(c->vc); cudaFree(c->kpool); cudaFree(c->qbar);
     cudaFree(c->sel_q); cudaFree(c->sel_rank); cudaFree(c->sel_pair); cudaFree(c->pair_cnt);
+    cudaFree(c->panic_item); cudaFree(c->panic_last);
   }
   delete c;
   return UF_OK;

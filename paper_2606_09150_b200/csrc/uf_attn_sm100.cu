@@ -9,10 +9,29 @@
 //                           (128 x 128 bf16, two 64-column boxes, 128-byte swizzle) into smem rings
 //   warp 9   MMA issuer   : S_t = Q_t K^T  (tcgen05.mma, SS, M=N=K=128) into TMEM,
 //                           O_t += P_t V   (tcgen05.mma, A = P_t from TMEM, B = V tile MN-major)
-//   warps 0-3 / 4-7       : softmax of tile 0 / tile 1, one thread per query row: tcgen05.ld the
-//                           S row, running max (lazy rescale of O_t in TMEM only when the max grew
-//                           by more than 2^8), exp2, row sum, bf16 P back to TMEM over S_t's columns
+//   warps 0-3 / 4-7       : softmax of tile 0 / tile 1, one thread per query row, S read from TMEM
+//                           in 32-column chunks (next chunk in flight while this one is processed),
+//                           bf16 P written back over S_t's columns chunk by chunk
 //   epilogue (same warps) : O_t / l -> bf16 -> swizzled smem (the Q_t buffer) -> TMA store
+//
+// Warps 8 and 9 run their control flow warp-uniformly and issue TMA / tcgen05.mma / tcgen05.commit
+// from the lane elect.sync picks: those instructions take uniform-register operands, and issued from
+// an `if (lane == 0)` region ptxas wraps EACH one in an ELECT/R2UR/BRA loop (measured: ~70 cycles per
+// MMA, slower than the 64-cycle MMA).  The tensor pipe's command queue is shallow (issue blocks while
+// it is full), so whatever the MMA warp executes between two MMA groups is exposed: descriptors are
+// a precomputed 32-bit base plus a constant, stage counters are incremental, entries are prefetched.
+//
+// Softmax (R-20): p = 2^(s*scale*log2e - m).  The reference max m of a row is the one of the EARLIER
+// key blocks; the row max of the current block is computed beside the exponentials and checked
+// afterwards, so the max -> exp dependency is off the critical path:
+//   growth <= 2^8   : nothing to do (lazy rescale; the final O/l uses the same m, so this is exact)
+//   growth <= 2^100 : this block's P and row sum stay relative to the old m (exact); before the next
+//                     block m is raised and O_t (TMEM) and l are multiplied by f = 2^(m_old - m_new)
+//   growth >  2^100 : (exponentials may have overflowed) the item is flagged and redone by the
+//                     kSafe instantiation of this kernel, which takes the exact row max before the
+//                     exponentials of every block; it is launched right after and returns at once
+//                     when nothing was flagged.
+// The first key block of an item always takes the exact-max path.
 //
 // TMEM (512 columns): S_0 [0,128)  S_1 [128,256)  O_0 [256,384)  O_1 [384,512); P_t aliases the
 // first 64 columns of S_t (tensor-pipe ops run in issue order, so S_t(next) is issued after
@@ -32,12 +51,9 @@ constexpr int kNV = 2;                 // V ring stages
 constexpr int kTile = 128 * 128 * 2;   // bytes of one 128 x 128 bf16 tile
 constexpr int kHalf = kTile / 2;       // one 64-column box
 constexpr int kThreads = 384;
-constexpr float kRescaleThreshold = 8.0f;   // log2 units
-#ifdef UF_ARRIVE_ALL
-constexpr uint32_t kPArrivals = 128;        // every softmax thread arrives on P_FULL
-#else
+constexpr float kRescaleThreshold = 8.0f;   // log2 units: below this growth of the row max, keep m
+constexpr float kPanicThreshold = 100.0f;   // log2 units: above this growth, redo the item in the safe kernel
 constexpr uint32_t kPArrivals = 4;          // one elected lane per softmax warp arrives on P_FULL
-#endif
 
 // smem carve-up (offsets from a 1024-aligned base)
 constexpr int kOffQ = 0;                          // 2 tiles
@@ -101,23 +117,35 @@ __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::
 __device__ __forceinline__ void tc_commit(uint32_t bar) {
   asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
 }
+// Shared-memory matrix descriptors, 128-byte swizzle.  The upper 32 bits are the same for every operand
+// here (SBO = 1024 B between 8-row groups, version 1, swizzle mode 2); the lower 32 bits are
+// (address >> 4) | (LBO >> 4) << 16, i.e. a per-buffer base plus a small constant per K step.
+constexpr uint32_t kDescHi = (1024u >> 4) | (1u << 14) | (2u << 29);
+__device__ __forceinline__ uint32_t desc_lo(uint32_t saddr, uint32_t lbo_bytes) {
+  return ((saddr & 0x3FFFFu) >> 4) | ((lbo_bytes >> 4) << 16);
+}
 // D[tmem] (+)= A[smem] * B[smem]
-__device__ __forceinline__ void mma_ss(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t acc) {
+__device__ __forceinline__ void mma_ss(uint32_t d_tmem, uint32_t a_lo, uint32_t b_lo, uint32_t idesc, uint32_t acc) {
   asm volatile(
       "{\n\t"
       ".reg .pred p;\n\t"
+      ".reg .b64 da, db;\n\t"
       "setp.ne.b32 p, %4, 0;\n\t"
-      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t"
-      "}" ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(acc) : "memory");
+      "mov.b64 da, {%1, %5};\n\t"
+      "mov.b64 db, {%2, %5};\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], da, db, %3, p;\n\t"
+      "}" ::"r"(d_tmem), "r"(a_lo), "r"(b_lo), "r"(idesc), "r"(acc), "r"(kDescHi) : "memory");
 }
 // D[tmem] (+)= A[tmem] * B[smem]
-__device__ __forceinline__ void mma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc, uint32_t acc) {
+__device__ __forceinline__ void mma_ts(uint32_t d_tmem, uint32_t a_tmem, uint32_t b_lo, uint32_t idesc, uint32_t acc) {
   asm volatile(
       "{\n\t"
       ".reg .pred p;\n\t"
+      ".reg .b64 db;\n\t"
       "setp.ne.b32 p, %4, 0;\n\t"
-      "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t"
-      "}" ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(acc) : "memory");
+      "mov.b64 db, {%2, %5};\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], db, %3, p;\n\t"
+      "}" ::"r"(d_tmem), "r"(a_tmem), "r"(b_lo), "r"(idesc), "r"(acc), "r"(kDescHi) : "memory");
 }
 
 #define UF_TMEM_LD32(taddr, a, o)                                                                              \
@@ -146,6 +174,25 @@ __device__ __forceinline__ void mma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_
         "r"(a[o + 30]), "r"(a[o + 31])                                                                         \
       : "memory")
 
+#define UF_TMEM_ST16(taddr, a)                                                                                 \
+  asm volatile(                                                                                                \
+      "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], "                                                          \
+      "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};"                               \
+      ::"r"(taddr), "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(a[4]), "r"(a[5]), "r"(a[6]), "r"(a[7]),    \
+        "r"(a[8]), "r"(a[9]), "r"(a[10]), "r"(a[11]), "r"(a[12]), "r"(a[13]), "r"(a[14]), "r"(a[15])           \
+      : "memory")
+
+// tcgen05.wait::ld that also names the 32 destination registers of the load it completes, so that no use
+// of them can be scheduled above it (the load itself returns before its registers are written).
+#define UF_TMEM_WAIT_LD32(a)                                                                                   \
+  asm volatile("tcgen05.wait::ld.sync.aligned;"                                                                \
+      : "+r"(a[0]), "+r"(a[1]), "+r"(a[2]), "+r"(a[3]), "+r"(a[4]), "+r"(a[5]), "+r"(a[6]), "+r"(a[7]),        \
+        "+r"(a[8]), "+r"(a[9]), "+r"(a[10]), "+r"(a[11]), "+r"(a[12]), "+r"(a[13]), "+r"(a[14]), "+r"(a[15]),  \
+        "+r"(a[16]), "+r"(a[17]), "+r"(a[18]), "+r"(a[19]), "+r"(a[20]), "+r"(a[21]), "+r"(a[22]),             \
+        "+r"(a[23]), "+r"(a[24]), "+r"(a[25]), "+r"(a[26]), "+r"(a[27]), "+r"(a[28]), "+r"(a[29]),             \
+        "+r"(a[30]), "+r"(a[31])                                                                               \
+      :: "memory")
+
 // One lane of a converged warp (the same one every time).  tcgen05.mma / tcgen05.commit / TMA take their
 // operands from uniform registers: issued under elect.sync from warp-uniform control flow, ptxas emits them
 // straight-line; issued from an `if (lane == 0)` region it wraps EACH one in an ELECT/R2UR/BRA loop
@@ -160,19 +207,12 @@ __device__ __forceinline__ bool elect_one() {
       "}" : "=r"(pred));
   return pred != 0;
 }
-// a loaded value every lane holds anyway, made provably warp-uniform for the compiler
-__device__ __forceinline__ int32_t uniform_i32(int32_t v) { return __shfl_sync(0xffffffffu, v, 0); }
 
-__device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 
 __device__ __forceinline__ float ex2(float x) {
   float y;
-#ifdef UF_DBG_NOMUFU
-  y = x * 0.5f;
-#else
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-#endif
   return y;
 }
 __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
@@ -221,7 +261,8 @@ __device__ __forceinline__ float max3(float a, float b, float c) {
 // 8 column pairs.  2^x = 2^floor(x) * 2^frac(x): floor via the round-down magic-number add (the integer
 // lands in the low mantissa bits), 2^frac by a degree-3 minimax polynomial on [0,1) (max relative error
 // 7.5e-5, far below the bf16 rounding of P), the exponent added into the float's bits by one LEA.
-// Valid for -126 <= x (clamped: the polynomial can return 1 - 7.5e-5, exponent field 126) and x <= 8 (guaranteed by the lazy-rescale invariant).
+// Valid for x >= -126 (clamped: the polynomial can return 1 - 7.5e-5, i.e. exponent field 126) and x < 128
+// (larger x means the row max grew by more than 2^100: the panic path).
 #ifndef UF_EMU_PAIRS
 #define UF_EMU_PAIRS 3
 #endif
@@ -247,56 +288,33 @@ __device__ __forceinline__ uint64_t ex2_pair(uint64_t x, bool emulate) {
   return pack2(p0, p1);
 }
 
-// One softmax pass over a loaded S row (128 logits in s[]): p = 2^(s*sl2 - m) into bf16 pairs pk[],
-// returns the fp32 row sum; with kWithMax also the raw row max (computed beside the exponentials, not
-// before them: the running max m used here is the one from the previous key blocks).
-template <bool kWithMax>
-__device__ __forceinline__ float exp_pass(const uint32_t (&s)[128], uint32_t (&pk)[64], float m, float sl2, float& rowmax) {
-  const uint64_t nm2 = pack2(-m, -m), sl22 = pack2(sl2, sl2);
-  uint64_t acc0 = pack2(0.f, 0.f), acc1 = acc0;
-  float mx0 = -INFINITY, mx1 = -INFINITY, mx2 = -INFINITY, mx3 = -INFINITY;
+// One 32-column chunk of a softmax pass: p = 2^(s*sl2 - m) as bf16 pairs into pk[], fp32 row sums into
+// the two packed accumulators, and the raw max of the chunk into mx0/mx1 (computed beside the
+// exponentials: the m used here is the running max of the EARLIER key blocks).  `chunk` selects which
+// column pairs take the polynomial; `nvalid_left` < 32 masks the tail of a ragged key block (R-3).
+__device__ __forceinline__ void exp_chunk(uint32_t (&s)[32], uint32_t (&pk)[16], int chunk, int nvalid_left,
+                                          uint64_t sl22, uint64_t nm2, uint64_t& acc0, uint64_t& acc1,
+                                          float& mx0, float& mx1) {
+  if (nvalid_left < 32) {
 #pragma unroll
-  for (int c = 0; c < 128; c += 8) {
-#pragma unroll
-    for (int u = 0; u < 8; u += 2) {
-      const int j = (c + u) >> 1;
-      const uint64_t x = fma2(pack2(__uint_as_float(s[c + u]), __uint_as_float(s[c + u + 1])), sl22, nm2);
-      const uint64_t p = ex2_pair(x, pair_emulated(j));
-      if (j & 1) acc1 = add2(acc1, p); else acc0 = add2(acc0, p);
-      float p0, p1;
-      unpack2(p, p0, p1);
-      pk[j] = pack_bf16x2(p0, p1);
-    }
-    if (kWithMax) {
-      mx0 = max3(mx0, __uint_as_float(s[c + 0]), __uint_as_float(s[c + 1]));
-      mx1 = max3(mx1, __uint_as_float(s[c + 2]), __uint_as_float(s[c + 3]));
-      mx2 = max3(mx2, __uint_as_float(s[c + 4]), __uint_as_float(s[c + 5]));
-      mx3 = max3(mx3, __uint_as_float(s[c + 6]), __uint_as_float(s[c + 7]));
-    }
+    for (int c = 0; c < 32; ++c)
+      if (c >= nvalid_left) s[c] = 0xff800000u;          // -inf
   }
-  if (kWithMax) rowmax = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3));
-  float a0, a1, b0, b1;
-  unpack2(acc0, a0, a1);
-  unpack2(acc1, b0, b1);
-  return (a0 + a1) + (b0 + b1);
-}
-
-__device__ __forceinline__ float max_pass(const uint32_t (&s)[128]) {
-  float mx0 = -INFINITY, mx1 = -INFINITY, mx2 = -INFINITY, mx3 = -INFINITY;
 #pragma unroll
-  for (int c = 0; c < 128; c += 8) {
-    mx0 = max3(mx0, __uint_as_float(s[c + 0]), __uint_as_float(s[c + 1]));
-    mx1 = max3(mx1, __uint_as_float(s[c + 2]), __uint_as_float(s[c + 3]));
-    mx2 = max3(mx2, __uint_as_float(s[c + 4]), __uint_as_float(s[c + 5]));
-    mx3 = max3(mx3, __uint_as_float(s[c + 6]), __uint_as_float(s[c + 7]));
+  for (int u = 0; u < 32; u += 2) {
+    const int j = chunk * 16 + (u >> 1);
+    const uint64_t x = fma2(pack2(__uint_as_float(s[u]), __uint_as_float(s[u + 1])), sl22, nm2);
+    const uint64_t p = ex2_pair(x, pair_emulated(j));
+    if (j & 1) acc1 = add2(acc1, p); else acc0 = add2(acc0, p);
+    float p0, p1;
+    unpack2(p, p0, p1);
+    pk[u >> 1] = pack_bf16x2(p0, p1);
   }
-  return fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3));
-}
-
-// shared-memory matrix descriptor, 128-byte swizzle
-__device__ __forceinline__ uint64_t make_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
-  return (uint64_t)((saddr & 0x3FFFFu) >> 4) | ((uint64_t)(lbo_bytes >> 4) << 16) | ((uint64_t)(sbo_bytes >> 4) << 32) |
-         (1ull << 46) | (2ull << 61);
+#pragma unroll
+  for (int u = 0; u < 32; u += 4) {
+    mx0 = max3(mx0, __uint_as_float(s[u + 0]), __uint_as_float(s[u + 1]));
+    mx1 = max3(mx1, __uint_as_float(s[u + 2]), __uint_as_float(s[u + 3]));
+  }
 }
 
 // instruction descriptor kind::f16: D fp32, A/B bf16, M = N = 128; B MN-major for P V
@@ -304,10 +322,10 @@ constexpr uint32_t kIdescQK = (1u << 4) | (1u << 7) | (1u << 10) | ((128u >> 3) 
 constexpr uint32_t kIdescPV = kIdescQK | (1u << 16);
 
 #ifdef UF_DBG_TRACE
-// debug only: clock64 timestamps of CTA 0's first kTraceSteps steps; roles: 0 = MMA thread, 1 = softmax tile 0, 2 = softmax tile 1
+// debug only: clock64 timestamps of CTA 0's first kTraceSteps steps; roles: 0 = MMA warp, 1 / 2 = softmax tile 0 / 1
 constexpr int kTraceSteps = 600;
 __device__ long long uf_trace[3][kTraceSteps][8];
-#define UF_TR(role, step, slot) do { if (blockIdx.x == 0 && (step) < kTraceSteps) uf_trace[role][step][slot] = clock64(); } while (0)
+#define UF_TR(role, step, slot) do { if (blockIdx.x == 0 && (int)(step) < kTraceSteps) uf_trace[role][step][slot] = clock64(); } while (0)
 #else
 #define UF_TR(role, step, slot) do { } while (0)
 #endif
@@ -316,6 +334,9 @@ struct AttnParams {
   const int32_t* sel_pair;   // [H][NP][2*kcap]
   const int32_t* pair_cnt;   // [H][NP]
   float* lse;                // [H][ntok] or null
+  int32_t* panic_item;       // [H * np_cur]: == seq when the item must be redone by the safe kernel
+  int32_t* panic_last;       // == seq when any item of this launch was flagged
+  int32_t seq;               // launch sequence number (never 0)
   int H, NP, kcap, np_cur;
   int ntok, nqb;
   int n_sink, sink_ntok;
@@ -323,37 +344,12 @@ struct AttnParams {
   float sl2;                 // softmax scale * log2(e)
 };
 
-struct Item {
-  int h, p, n_u, n_steps, full_mask;
-  const int32_t* ulist;
-};
-
-template <bool kUniform = false>
-__device__ __forceinline__ Item get_item(const AttnParams& a, int it) {
-  Item x;
-  x.h = it / a.np_cur;
-  x.p = it % a.np_cur;
-  const int64_t pi = (int64_t)x.h * a.NP + x.p;
-  x.n_u = kUniform ? uniform_i32(a.pair_cnt[pi]) : a.pair_cnt[pi];
-  x.ulist = a.sel_pair + pi * 2 * a.kcap;
-  x.n_steps = x.n_u + a.n_sink + a.nqb;
-  x.full_mask = (2 * x.p + 1 < a.nqb) ? 3 : 1;
-  return x;
-}
-
-template <bool kUniform = false>
-__device__ __forceinline__ int32_t get_entry(const AttnParams& a, const Item& x, int st) {
-  if (st < x.n_u) return kUniform ? uniform_i32(__ldg(x.ulist + st)) : __ldg(x.ulist + st);
-  st -= x.n_u;
-  if (st < a.n_sink) return uf_entry_pack(st, min(128, a.sink_ntok - st * 128), x.full_mask);
-  st -= a.n_sink;
-  return uf_entry_pack(a.cur_phys0 + st, min(128, a.ntok - st * 128), x.full_mask);
-}
-
+template <bool kSafe>
 __global__ void __launch_bounds__(kThreads, 1)
 uf_attn_sm100_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_o,
                      const __grid_constant__ CUtensorMap tm_k, const __grid_constant__ CUtensorMap tm_v,
                      const AttnParams a) {
+  if (kSafe && *a.panic_last != a.seq) return;         // nothing was flagged: the usual case
   extern __shared__ unsigned char smem_raw[];
   const uint32_t raw = smem_u32(smem_raw);
   const uint32_t base = (raw + 1023u) & ~1023u;
@@ -385,163 +381,165 @@ uf_attn_sm100_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_cons
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = *tmem_ptr_smem;
-#ifdef UF_DBG_CLOCK
-  unsigned long long dbg_c0 = 0, dbg_t0 = 0;
-  if (blockIdx.x == 0 && threadIdx.x == 0) {
-    dbg_c0 = clock64();
-    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(dbg_t0));
-  }
-#endif
+
+  // An item = (head h, query-block pair p).  Its key blocks: the pair's merged TOPK list (n_u entries,
+  // loaded 32 at a time, one per lane, and broadcast by shuffle), then n_sink SINK blocks, then nqb CUR
+  // blocks.  The safe kernel only takes the items the fast kernel flagged.
+#define UF_ITEM_LOOP_BEGIN                                                                      \
+  for (int it = blockIdx.x; it < n_items; it += gridDim.x) {                                    \
+    if (kSafe && a.panic_item[it] != a.seq) continue;                                           \
+    const int h = it / a.np_cur, p = it % a.np_cur;                                             \
+    const int64_t pi = (int64_t)h * a.NP + p;                                                   \
+    const int n_u = __shfl_sync(0xffffffffu, a.pair_cnt[pi], 0);                                \
+    const int32_t* ulist = a.sel_pair + pi * 2 * a.kcap;                                        \
+    const int full_mask = (2 * p + 1 < a.nqb) ? 3 : 1;
+#define UF_ITEM_LOOP_END }
 
   if (warp >= 8) {
     asm volatile("setmaxnreg.dec.sync.aligned.u32 80;");
     if (warp == 8) {
       // ================================ TMA producer ================================
-      // (whole warp runs the control flow; the elected lane issues expect_tx + TMA)
-      uint32_t kcount = 0, vcount = 0, qn[2] = {0, 0};
-      for (int it = blockIdx.x; it < n_items; it += gridDim.x) {
-        const Item x = get_item<true>(a, it);
+      uint32_t ks = 0, kph = 0, vs = 0, vph = 0, qph0 = 0, qph1 = 0;
+      auto load_kv = [&](int phys, int h) {
+        const int row = phys * 128;
+        {
+          const uint32_t bf = bars + (K_FULL0 + ks) * 8, dst = base + kOffK + ks * kTile;
+          mbar_wait(bars + (K_EMPTY0 + ks) * 8, kph ^ 1);
+          if (elect_one()) {
+            mbar_expect_tx(bf, kTile);
+            tma_load_3d(dst, &tm_k, bf, 0, row, h);
+            tma_load_3d(dst + kHalf, &tm_k, bf, 64, row, h);
+          }
+          if (++ks == kNK) { ks = 0; kph ^= 1; }
+        }
+        {
+          const uint32_t bf = bars + (V_FULL0 + vs) * 8, dst = base + kOffV + vs * kTile;
+          mbar_wait(bars + (V_EMPTY0 + vs) * 8, vph ^ 1);
+          if (elect_one()) {
+            mbar_expect_tx(bf, kTile);
+            tma_load_3d(dst, &tm_v, bf, 0, row, h);
+            tma_load_3d(dst + kHalf, &tm_v, bf, 64, row, h);
+          }
+          if (++vs == kNV) { vs = 0; vph ^= 1; }
+        }
+      };
+      UF_ITEM_LOOP_BEGIN
+        int32_t nxt = (lane < n_u) ? __ldg(ulist + lane) : 0;
+#pragma unroll
         for (int t = 0; t < 2; ++t) {
-          if (!(x.full_mask & (1 << t))) continue;
+          if (!(full_mask & (1 << t))) continue;
           const uint32_t bq = bars + (Q_FULL0 + t) * 8;
-          mbar_wait(bars + (Q_EMPTY0 + t) * 8, (qn[t] & 1) ^ 1);
-          const int row0 = (2 * x.p + t) * 128;
+          uint32_t& qph = t ? qph1 : qph0;
+          mbar_wait(bars + (Q_EMPTY0 + t) * 8, qph ^ 1);
+          qph ^= 1;
+          const int row0 = (2 * p + t) * 128;
           if (elect_one()) {
             mbar_expect_tx(bq, kTile);
-            tma_load_3d(base + kOffQ + t * kTile, &tm_q, bq, 0, row0, x.h);
-            tma_load_3d(base + kOffQ + t * kTile + kHalf, &tm_q, bq, 64, row0, x.h);
+            tma_load_3d(base + kOffQ + t * kTile, &tm_q, bq, 0, row0, h);
+            tma_load_3d(base + kOffQ + t * kTile + kHalf, &tm_q, bq, 64, row0, h);
           }
-          ++qn[t];
         }
-        int32_t e = get_entry<true>(a, x, 0);
-        for (int st = 0; st < x.n_steps; ++st) {
-          const int32_t en = (st + 1 < x.n_steps) ? get_entry<true>(a, x, st + 1) : 0;
-          const int row = uf_entry_phys(e) * 128;
-          {
-            const uint32_t s = kcount % kNK, n = kcount / kNK;
-            const uint32_t bf = bars + (K_FULL0 + s) * 8;
-            mbar_wait(bars + (K_EMPTY0 + s) * 8, (n & 1) ^ 1);
-#ifdef UF_DBG_NOTMA
-            if (kcount >= kNK) { if (elect_one()) mbar_arrive(bf); } else
-#endif
-            if (elect_one()) {
-            mbar_expect_tx(bf, kTile);
-            tma_load_3d(base + kOffK + s * kTile, &tm_k, bf, 0, row, x.h);
-            tma_load_3d(base + kOffK + s * kTile + kHalf, &tm_k, bf, 64, row, x.h);
-            }
-            ++kcount;
-          }
-          {
-            const uint32_t s = vcount % kNV, n = vcount / kNV;
-            const uint32_t bf = bars + (V_FULL0 + s) * 8;
-            mbar_wait(bars + (V_EMPTY0 + s) * 8, (n & 1) ^ 1);
-#ifdef UF_DBG_NOTMA
-            if (vcount >= kNV) { if (elect_one()) mbar_arrive(bf); } else
-#endif
-            if (elect_one()) {
-            mbar_expect_tx(bf, kTile);
-            tma_load_3d(base + kOffV + s * kTile, &tm_v, bf, 0, row, x.h);
-            tma_load_3d(base + kOffV + s * kTile + kHalf, &tm_v, bf, 64, row, x.h);
-            }
-            ++vcount;
-          }
-          e = en;
+        for (int st0 = 0; st0 < n_u; st0 += 32) {
+          const int32_t mine = nxt;
+          if (st0 + 32 + lane < n_u) nxt = __ldg(ulist + st0 + 32 + lane);
+          const int cnt = min(32, n_u - st0);
+          for (int j = 0; j < cnt; ++j) load_kv(uf_entry_phys(__shfl_sync(0xffffffffu, mine, j)), h);
         }
-      }
+        for (int j = 0; j < a.n_sink; ++j) load_kv(j, h);
+        for (int j = 0; j < a.nqb; ++j) load_kv(a.cur_phys0 + j, h);
+      UF_ITEM_LOOP_END
     } else if (warp == 9) {
       // ================================ MMA issuer ==================================
-      // (whole warp runs the control flow and the barrier waits; the elected lane issues MMAs and commits)
-      uint32_t kcount = 0, vcount = 0, qn[2] = {0, 0}, pn[2] = {0, 0};
+      // Per key block and attending tile t: O_t += P_t V of the PREVIOUS block of that tile (once its
+      // P is ready), then S_t = Q_t K^T of this block.  Tensor-pipe order per step with both tiles:
+      // PV_0(n-1) QK_0(n) PV_1(n-1) QK_1(n): while the softmax warps of one tile work, the pipe runs
+      // the other tile.
+      const uint32_t q_lo0 = desc_lo(base + kOffQ, 16), q_lo1 = desc_lo(base + kOffQ + kTile, 16);
+      const uint32_t k_lo_base = desc_lo(base + kOffK, 16);
+      const uint32_t v_lo_base = desc_lo(base + kOffV, kHalf);
       static_assert(kNV == 2, "vrem0/vrem1 below assume a 2-stage V ring");
+      uint32_t ks = 0, kph = 0, vs = 0, vph = 0, qph0 = 0, qph1 = 0, pph0 = 0, pph1 = 0;
       int vrem0 = 0, vrem1 = 0;                      // tiles that still have to consume V stage 0 / 1
-      for (int it = blockIdx.x; it < n_items; it += gridDim.x) {
-        const Item x = get_item<true>(a, it);
-        bool pend[2] = {false, false};
-        uint32_t pend_vs[2] = {0, 0}, pend_vpar[2] = {0, 0};
-        bool first_pv[2] = {true, true};
-        for (int t = 0; t < 2; ++t)
-          if (x.full_mask & (1 << t)) { mbar_wait(bars + (Q_FULL0 + t) * 8, qn[t] & 1); ++qn[t]; }
+      int trc = 0; (void)trc;                        // UF_DBG_TRACE step counter
+      bool pend[2] = {false, false}, first_pv[2] = {true, true};
+      uint32_t pend_vs[2] = {0, 0}, pend_vph[2] = {0, 0};
 
-        auto do_pv = [&](int t) {
-          UF_TR(0, (int)kcount, t * 2);
-          mbar_wait(bars + (P_FULL0 + t) * 8, pn[t] & 1); ++pn[t];
-          UF_TR(0, (int)kcount, t * 2 + 1);
-          const uint32_t vs = pend_vs[t];
-          mbar_wait(bars + (V_FULL0 + vs) * 8, pend_vpar[t]);
-          tc_fence_after();
-          const uint32_t vaddr = base + kOffV + vs * kTile;
-          const uint32_t d_tmem = tmem + 256 + t * 128;
-          const uint32_t p_tmem = tmem + t * 128;
-          const int left = (vs == 0) ? --vrem0 : --vrem1;
+      auto do_pv = [&](int t) {
+        uint32_t& pph = t ? pph1 : pph0;
+        UF_TR(0, trc, t * 2);
+        mbar_wait(bars + (P_FULL0 + t) * 8, pph);
+        UF_TR(0, trc, t * 2 + 1);
+        pph ^= 1;
+        const uint32_t pvs = pend_vs[t];
+        mbar_wait(bars + (V_FULL0 + pvs) * 8, pend_vph[t]);
+        tc_fence_after();
+        const int left = (pvs == 0) ? --vrem0 : --vrem1;
+        if (elect_one()) {
+          // B = V tile, MN-major: 8-key groups 1024 B apart (SBO), the two 64-column halves 16 KB apart (LBO)
+          const uint32_t v_lo = v_lo_base + pvs * (kTile >> 4);
+          const uint32_t d_tmem = tmem + 256 + t * 128, p_tmem = tmem + t * 128;
+#pragma unroll
+          for (int k = 0; k < 8; ++k)
+            mma_ts(d_tmem, p_tmem + k * 8, v_lo + k * (2048 >> 4), kIdescPV, (first_pv[t] && k == 0) ? 0u : 1u);
+          if (left == 0) tc_commit(bars + (V_EMPTY0 + pvs) * 8);
+        }
+        first_pv[t] = false;
+        pend[t] = false;
+      };
+
+      auto step = [&](int m) {
+        UF_TR(0, trc, 6);
+        mbar_wait(bars + (K_FULL0 + ks) * 8, kph);
+        tc_fence_after();
+        UF_TR(0, trc, 4);
+        const uint32_t k_lo = k_lo_base + ks * (kTile >> 4);
+        int users = 0;
+#pragma unroll
+        for (int t = 0; t < 2; ++t) {
+          if (!(m & (1 << t))) continue;
+          if (pend[t]) do_pv(t);
           if (elect_one()) {
+            const uint32_t q_lo = t ? q_lo1 : q_lo0;
 #pragma unroll
             for (int k = 0; k < 8; ++k) {
-              // B = V tile, MN-major: 8-key groups 1024 B apart (SBO), the two 64-column halves 16 KB apart (LBO)
-              const uint64_t bd = make_desc(vaddr + k * 2048, kHalf, 1024);
-#ifndef UF_DBG_NOPV
-              mma_ts(d_tmem, p_tmem + k * 8, bd, kIdescPV, (first_pv[t] && k == 0) ? 0u : 1u);
-#endif
+              // K-major operands: 8-row groups 1024 B apart (SBO); 16 elements = 32 B along K, second half +16 KB
+              const uint32_t koff = ((k & 3) * 32 + (k >> 2) * kHalf) >> 4;
+              mma_ss(tmem + t * 128, q_lo + koff, k_lo + koff, kIdescQK, k == 0 ? 0u : 1u);
             }
-            if (left == 0) tc_commit(bars + (V_EMPTY0 + vs) * 8);
+            tc_commit(bars + (S_FULL0 + t) * 8);
           }
-          __syncwarp();
-          first_pv[t] = false;
-          pend[t] = false;
-        };
-
-        int32_t e = get_entry<true>(a, x, 0);
-        for (int st = 0; st < x.n_steps; ++st) {
-          const int32_t en = (st + 1 < x.n_steps) ? get_entry<true>(a, x, st + 1) : 0;
-          const int m = uf_entry_mask(e);
-          const uint32_t ks = kcount % kNK, kpar = (kcount / kNK) & 1;
-          const uint32_t vs = vcount % kNV, vpar = (vcount / kNV) & 1;
-          UF_TR(0, (int)kcount, 6);
-          mbar_wait(bars + (K_FULL0 + ks) * 8, kpar);
-          UF_TR(0, (int)kcount, 7);
-          tc_fence_after();
-          UF_TR(0, (int)kcount, 4);
-          const uint32_t kaddr = base + kOffK + ks * kTile;
-          int users = 0;
-#pragma unroll
-          for (int t = 0; t < 2; ++t) {
-            if (!(m & (1 << t))) continue;
-            if (pend[t]) do_pv(t);
-            const uint32_t qaddr = base + kOffQ + t * kTile;
-            if (elect_one()) {
-#pragma unroll
-              for (int k = 0; k < 8; ++k) {
-                // K-major operands: 8-row groups 1024 B apart (SBO); 16 elements = 32 B along K, second half +16 KB
-                const uint32_t koff = (k & 3) * 32 + (k >> 2) * kHalf;
-#ifndef UF_DBG_NOQK
-                mma_ss(tmem + t * 128, make_desc(qaddr + koff, 16, 1024), make_desc(kaddr + koff, 16, 1024), kIdescQK,
-                       k == 0 ? 0u : 1u);
-#endif
-              }
-              tc_commit(bars + (S_FULL0 + t) * 8);
-            }
-            __syncwarp();
-            pend[t] = true; pend_vs[t] = vs; pend_vpar[t] = vpar;
-            ++users;
-          }
-          if (elect_one()) tc_commit(bars + (K_EMPTY0 + ks) * 8);
-          __syncwarp();
-          UF_TR(0, (int)kcount, 5);
-          if (vs == 0) vrem0 = users; else vrem1 = users;
-          ++kcount; ++vcount;
-#pragma unroll
-          for (int t = 0; t < 2; ++t)
-            if (!(m & (1 << t)) && pend[t]) do_pv(t);      // keep V stages flowing (no deadlock)
-          e = en;
+          pend[t] = true; pend_vs[t] = vs; pend_vph[t] = vph;
+          ++users;
         }
+        if (elect_one()) tc_commit(bars + (K_EMPTY0 + ks) * 8);
+        UF_TR(0, trc, 5);
+        ++trc;
+        if (vs == 0) vrem0 = users; else vrem1 = users;
+        if (++ks == kNK) { ks = 0; kph ^= 1; }
+        if (++vs == kNV) { vs = 0; vph ^= 1; }
+#pragma unroll
+        for (int t = 0; t < 2; ++t)
+          if (!(m & (1 << t)) && pend[t]) do_pv(t);      // keep V stages flowing (no deadlock)
+      };
+
+      UF_ITEM_LOOP_BEGIN
+        int32_t nxt = (lane < n_u) ? __ldg(ulist + lane) : 0;
+        first_pv[0] = first_pv[1] = true;
+        if (full_mask & 1) { mbar_wait(bars + Q_FULL0 * 8, qph0); qph0 ^= 1; }
+        if (full_mask & 2) { mbar_wait(bars + Q_FULL1 * 8, qph1); qph1 ^= 1; }
+        for (int st0 = 0; st0 < n_u; st0 += 32) {
+          const int32_t mine = nxt;
+          if (st0 + 32 + lane < n_u) nxt = __ldg(ulist + st0 + 32 + lane);
+          const int cnt = min(32, n_u - st0);
+          for (int j = 0; j < cnt; ++j) step(uf_entry_mask(__shfl_sync(0xffffffffu, mine, j)));
+        }
+        for (int j = 0; j < a.n_sink + a.nqb; ++j) step(full_mask);
 #pragma unroll
         for (int t = 0; t < 2; ++t) {
           if (pend[t]) do_pv(t);
-          if (x.full_mask & (1 << t)) {
-            if (elect_one()) tc_commit(bars + (O_FULL0 + t) * 8);
-            __syncwarp();
-          }
+          if ((full_mask & (1 << t)) && elect_one()) tc_commit(bars + (O_FULL0 + t) * 8);
         }
-      }
+      UF_ITEM_LOOP_END
     }
   } else {
     // ================================== softmax + epilogue ==================================
@@ -557,103 +555,142 @@ uf_attn_sm100_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_cons
     const uint32_t b_ofull = bars + (O_FULL0 + t) * 8;
     const uint32_t b_qempty = bars + (Q_EMPTY0 + t) * 8;
     unsigned char* stage = base_ptr + kOffQ + t * kTile;
-    uint32_t sn = 0, on = 0;
-    for (int it = blockIdx.x; it < n_items; it += gridDim.x) {
-      const Item x = get_item(a, it);
-      if (!(x.full_mask & (1 << t))) continue;
+    const float sl2 = a.sl2;
+    const uint64_t sl22 = pack2(sl2, sl2);
+    uint32_t sph = 0, oph = 0;
+    int trc = 0; (void)trc;                            // UF_DBG_TRACE step counter
+
+    UF_ITEM_LOOP_BEGIN
+      if (!(full_mask & (1 << t))) continue;
       float m = -INFINITY, l = 0.f;
-      bool first = true;
-      int32_t e = get_entry(a, x, 0);
-      for (int st = 0; st < x.n_steps; ++st) {
-        const int32_t en = (st + 1 < x.n_steps) ? get_entry(a, x, st + 1) : 0;
-        const int32_t ecur = e;
-        e = en;
-        if (!(uf_entry_mask(ecur) & (1 << t))) continue;
-        const int nvalid = uf_entry_nvalid(ecur);
-        if (wq == 0 && lane == 0) UF_TR(1 + t, (int)sn, 0);
-        mbar_wait(b_sfull, sn & 1); ++sn;
+      float f_pend = 1.0f, m_pend = 0.f;               // pending raise of m: a raise left pending at the end of
+      bool first = true;                               // the item is dropped (O_t / l does not depend on it)
+
+      // multiply the O_t row in TMEM by f (O_t is quiescent between S_FULL and our P_FULL arrive: the
+      // commit behind S_FULL also covers the earlier O_t += P_t V)
+      auto rescale_o = [&](float f) {
+#pragma unroll
+        for (int cc = 0; cc < 128; cc += 32) {
+          uint32_t ov[32];
+          UF_TMEM_LD32(o_tmem + cc, ov, 0);
+          UF_TMEM_WAIT_LD32(ov);
+#pragma unroll
+          for (int c = 0; c < 32; ++c) ov[c] = __float_as_uint(__uint_as_float(ov[c]) * f);
+          UF_TMEM_ST32(o_tmem + cc, ov, 0);
+        }
+      };
+
+      auto softmax_step = [&](int nvalid) {
+        if (wq == 0 && lane == 0) UF_TR(1 + t, trc, 0);
+        mbar_wait(b_sfull, sph);
+        sph ^= 1;
         tc_fence_after();
-        if (wq == 0 && lane == 0) UF_TR(1 + t, (int)sn - 1, 1);
-#ifdef UF_DBG_NOSOFTMAX
-        l = 1.f;
-        tc_fence_before();
-        __syncwarp();
-        if (lane == 0) mbar_arrive(b_pfull);
-        if (wq == 0 && lane == 0) UF_TR(1 + t, (int)sn - 1, 2);
-        continue;
-#endif
-        uint32_t s[128];
-        uint32_t pk[64];
-        auto load_s = [&]() {
-          UF_TMEM_LD32(s_tmem + 0, s, 0);
-          UF_TMEM_LD32(s_tmem + 32, s, 32);
-          UF_TMEM_LD32(s_tmem + 64, s, 64);
-          UF_TMEM_LD32(s_tmem + 96, s, 96);
-          tmem_wait_ld();
-          if (nvalid < 128) {
+        if (wq == 0 && lane == 0) UF_TR(1 + t, trc, 1);
+        uint32_t sa[32], sb[32], pk[16];
+        const bool exact = kSafe || first;
+        if (!kSafe && __any_sync(0xffffffffu, f_pend != 1.0f)) {     // deferred raise of m (see below)
+          rescale_o(f_pend);                                         // f_pend == 1 in rows with nothing pending
+          l *= f_pend;
+          if (f_pend != 1.0f) m = m_pend;
+          f_pend = 1.0f;
+        }
+        if (exact) {
+          // exact row max BEFORE the exponentials: first key block of an item / every block when kSafe
+          float mx0 = -INFINITY, mx1 = -INFINITY;
 #pragma unroll
-            for (int c = 0; c < 128; ++c)
-              if (c >= nvalid) s[c] = 0xff800000u;     // -inf: ragged key block (R-3)
-          }
-        };
-        load_s();
-        float lsum, rowmax = 0.f;
-#ifdef UF_DBG_NOEXP
-        lsum = 1.f;
+          for (int c = 0; c < 4; ++c) {
+            UF_TMEM_LD32(s_tmem + c * 32, sa, 0);
+            UF_TMEM_WAIT_LD32(sa);
+            const int left = nvalid - c * 32;
 #pragma unroll
-        for (int c = 0; c < 64; ++c) pk[c] = s[c] ^ s[c + 64];
-#else
-        if (first) {
-          m = max_pass(s) * a.sl2;
-          first = false;
-          lsum = exp_pass<false>(s, pk, m, a.sl2, rowmax);
-        } else {
-          // Exponentials against the running max of the EARLIER blocks, the row max of this block
-          // computed beside them: the max -> exp dependency leaves the critical path.  Valid while
-          // the new max exceeds m by at most 2^8 (the lazy-rescale invariant); otherwise redo.
-          lsum = exp_pass<true>(s, pk, m, a.sl2, rowmax);
-          const float m_new = fmaxf(m, rowmax * a.sl2);
-          const bool need = (m_new - m) > kRescaleThreshold;
-          if (__any_sync(0xffffffffu, need)) {
-            // O_t is quiescent here: S_t's commit covers the earlier O_t += P_t V
-            const float f = need ? ex2(m - m_new) : 1.0f;
-            if (need) { m = m_new; l *= f; }
-#pragma unroll
-            for (int cc = 0; cc < 128; cc += 32) {
-              uint32_t ov[32];
-              UF_TMEM_LD32(o_tmem + cc, ov, 0);
-              tmem_wait_ld();
-#pragma unroll
-              for (int c = 0; c < 32; ++c) ov[c] = __float_as_uint(__uint_as_float(ov[c]) * f);
-              UF_TMEM_ST32(o_tmem + cc, ov, 0);
+            for (int u = 0; u < 32; u += 2) {
+              const float v0 = (u < left) ? __uint_as_float(sa[u]) : -INFINITY;
+              const float v1 = (u + 1 < left) ? __uint_as_float(sa[u + 1]) : -INFINITY;
+              if (u & 2) mx1 = max3(mx1, v0, v1); else mx0 = max3(mx0, v0, v1);
             }
-            load_s();
-            lsum = exp_pass<false>(s, pk, m, a.sl2, rowmax);
+          }
+          const float m_new = fmaxf(m, fmaxf(mx0, mx1) * sl2);
+          if (first) {
+            m = m_new;
+            first = false;
+          } else {
+            const bool need = (m_new - m) > kRescaleThreshold;
+            if (__any_sync(0xffffffffu, need)) {
+              const float f = need ? ex2(m - m_new) : 1.0f;
+              if (need) { m = m_new; l *= f; }
+              rescale_o(f);
+            }
           }
         }
-#endif
+        // exponentials, chunk c + 1 in flight while chunk c is processed; P chunk c goes to columns
+        // [16c, 16c + 16) of S_t, all of which are in registers by then
+        const uint64_t nm2 = pack2(-m, -m);
+        uint64_t acc0 = pack2(0.f, 0.f), acc1 = acc0;
+        float mx0 = -INFINITY, mx1 = -INFINITY;
+        UF_TMEM_LD32(s_tmem + 0, sa, 0);
+        UF_TMEM_WAIT_LD32(sa);
+        UF_TMEM_LD32(s_tmem + 32, sb, 0);
+        exp_chunk(sa, pk, 0, nvalid, sl22, nm2, acc0, acc1, mx0, mx1);
+        UF_TMEM_ST16(s_tmem + 0, pk);
+        UF_TMEM_WAIT_LD32(sb);
+        UF_TMEM_LD32(s_tmem + 64, sa, 0);
+        exp_chunk(sb, pk, 1, nvalid - 32, sl22, nm2, acc0, acc1, mx0, mx1);
+        UF_TMEM_ST16(s_tmem + 16, pk);
+        UF_TMEM_WAIT_LD32(sa);
+        UF_TMEM_LD32(s_tmem + 96, sb, 0);
+        exp_chunk(sa, pk, 2, nvalid - 64, sl22, nm2, acc0, acc1, mx0, mx1);
+        UF_TMEM_ST16(s_tmem + 32, pk);
+        UF_TMEM_WAIT_LD32(sb);
+        exp_chunk(sb, pk, 3, nvalid - 96, sl22, nm2, acc0, acc1, mx0, mx1);
+        UF_TMEM_ST16(s_tmem + 48, pk);
+        float a0, a1, b0, b1;
+        unpack2(acc0, a0, a1);
+        unpack2(acc1, b0, b1);
+        float lsum = (a0 + a1) + (b0 + b1);
         l += lsum;
-        UF_TMEM_ST32(s_tmem + 0, pk, 0);
-        UF_TMEM_ST32(s_tmem + 32, pk, 32);
+        if (!exact) {
+          // The row max of this block, checked after the fact.  If it outgrew m by more than 2^8, m is
+          // raised BEFORE THE NEXT block (O_t and l are multiplied by f then: O_t is quiescent again only
+          // after this block's P V); this block's P and row sum stay relative to the old m, which is exact.
+          const float m_new = fmaxf(m, fmaxf(mx0, mx1) * sl2);
+          if ((m_new - m) > kRescaleThreshold) {
+            if ((m_new - m) > kPanicThreshold) {        // exponentials may have overflowed: redo the item
+              a.panic_item[it] = a.seq;
+              *a.panic_last = a.seq;
+            }
+            f_pend = ex2(m - m_new);
+            m_pend = m_new;
+          }
+        }
         tmem_wait_st();
         tc_fence_before();
-#ifdef UF_ARRIVE_ALL
-        mbar_arrive(b_pfull);
-#else
         __syncwarp();
         if (lane == 0) mbar_arrive(b_pfull);
-#endif
-        if (wq == 0 && lane == 0) UF_TR(1 + t, (int)sn - 1, 2);
+        if (wq == 0 && lane == 0) UF_TR(1 + t, trc, 2);
+        ++trc;
+      };
+
+      {
+        int32_t mine = 0;
+        for (int st = 0; st < n_u; ++st) {
+          if ((st & 31) == 0) mine = (st + lane < n_u) ? __ldg(ulist + st + lane) : 0;
+          const int32_t e = __shfl_sync(0xffffffffu, mine, st & 31);
+          if (uf_entry_mask(e) & (1 << t)) softmax_step(uf_entry_nvalid(e));
+        }
+        for (int j = 0; j < a.n_sink; ++j) softmax_step(min(128, a.sink_ntok - j * 128));
+        for (int j = 0; j < a.nqb; ++j) softmax_step(min(128, a.ntok - j * 128));
       }
+
       // ---- epilogue: O_t / l -> bf16 -> swizzled staging (Q_t buffer) -> TMA store ----
-      mbar_wait(b_ofull, on & 1); ++on;
+      mbar_wait(b_ofull, oph);
+      oph ^= 1;
       tc_fence_after();
       const float inv = 1.0f / l;
 #pragma unroll
       for (int cc = 0; cc < 128; cc += 32) {
         uint32_t ov[32];
         UF_TMEM_LD32(o_tmem + cc, ov, 0);
-        tmem_wait_ld();
+        UF_TMEM_WAIT_LD32(ov);
         unsigned char* half_base = stage + (cc >> 6) * kHalf + row * 128;
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
@@ -669,29 +706,24 @@ uf_attn_sm100_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_cons
       tc_fence_before();
       fence_proxy_async();
       asm volatile("bar.sync %0, 128;" ::"r"(1 + t) : "memory");
-      const int row0 = (2 * x.p + t) * 128;
+      const int row0 = (2 * p + t) * 128;
       if (wq == 0 && lane == 0) {
         const uint32_t src = base + kOffQ + t * kTile;
-        tma_store_3d(&tm_o, src, 0, row0, x.h);
-        tma_store_3d(&tm_o, src + kHalf, 64, row0, x.h);
+        tma_store_3d(&tm_o, src, 0, row0, h);
+        tma_store_3d(&tm_o, src + kHalf, 64, row0, h);
         tma_store_commit_and_wait_read();
         mbar_arrive(b_qempty);
       }
       if (a.lse != nullptr && row0 + row < a.ntok)
-        a.lse[(int64_t)x.h * a.ntok + row0 + row] = (m + log2f(l)) * 0.6931471805599453f;
-    }
+        a.lse[(int64_t)h * a.ntok + row0 + row] = (m + log2f(l)) * 0.6931471805599453f;
+    UF_ITEM_LOOP_END
     if (wq == 0 && lane == 0) tma_store_wait_all();
   }
+#undef UF_ITEM_LOOP_BEGIN
+#undef UF_ITEM_LOOP_END
 
   tc_fence_before();
   __syncthreads();
-#ifdef UF_DBG_CLOCK
-  if (blockIdx.x == 0 && threadIdx.x == 0) {
-    unsigned long long c1 = clock64(), t1;
-    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1));
-    printf("UFCLK cycles %llu ns %llu MHz %.1f\n", c1 - dbg_c0, t1 - dbg_t0, 1e3 * (double)(c1 - dbg_c0) / (double)(t1 - dbg_t0));
-  }
-#endif
   if (warp == 10) {
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem) : "memory");
   }
@@ -735,7 +767,9 @@ int uf_sm100_make_cache_maps(uf_ctx* c) {
     c->err = "cuTensorMapEncodeTiled failed for the K/V cache";
     return UF_ERR_CUDA;
   }
-  cudaError_t e = cudaFuncSetAttribute(uf_attn_sm100_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+  cudaError_t e = cudaFuncSetAttribute(uf_attn_sm100_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+  if (e == cudaSuccess)
+    e = cudaFuncSetAttribute(uf_attn_sm100_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
   if (e != cudaSuccess) {
     c->err = std::string("cudaFuncSetAttribute(smem): ") + cudaGetErrorString(e);
     return UF_ERR_CUDA;
@@ -761,8 +795,12 @@ int uf_launch_attn_sm100(uf_ctx* c, const UfView& v, const __nv_bfloat16* q, __n
   a.sl2 = scale * 1.4426950408889634f;
   const int n_items = a.H * a.np_cur;
   const int grid = n_items < c->sm_count ? n_items : c->sm_count;
-  uf_attn_sm100_kernel<<<grid, kThreads, kSmemBytes, s>>>(tm_q, tm_o, c->tm_k, c->tm_v, a);
-  c->launches += 1;
+  if (++c->attn_seq <= 0) c->attn_seq = 1;
+  a.panic_item = c->panic_item; a.panic_last = c->panic_last; a.seq = c->attn_seq;
+  // fast kernel, then the safe kernel for the items it flagged (returns at once when there are none)
+  uf_attn_sm100_kernel<false><<<grid, kThreads, kSmemBytes, s>>>(tm_q, tm_o, c->tm_k, c->tm_v, a);
+  uf_attn_sm100_kernel<true><<<grid, kThreads, kSmemBytes, s>>>(tm_q, tm_o, c->tm_k, c->tm_v, a);
+  c->launches += 2;
 #ifdef UF_DBG_TRACE
   if (const char* path = getenv("UF_TRACE_PATH")) {
     cudaDeviceSynchronize();

@@ -72,6 +72,9 @@ struct uf_ctx {
   int32_t* sel_rank = nullptr;    // candidate index of every sel_q entry (merge key); [H][BPC][kcap]
   int32_t* sel_pair = nullptr;    // per (h, q-block pair): merged union list with tile masks; [H][NP][2*kcap]
   int32_t* pair_cnt = nullptr;    // [H][NP]
+  int32_t* panic_item = nullptr;  // [H][NP]: == attn_seq when the safe attention kernel must redo the item
+  int32_t* panic_last = nullptr;  // [1]: == attn_seq when the last fast launch flagged anything
+  int32_t attn_seq = 0;           // sm100 attention launch sequence number
   int kcap = 0;                   // (C-1)*BPC
   int64_t dev_bytes = 0;
   // host state
