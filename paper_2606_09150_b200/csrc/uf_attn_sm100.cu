@@ -9,9 +9,9 @@
 //                           (128 x 128 bf16, two 64-column boxes, 128-byte swizzle) into smem rings
 //   warp 9   MMA issuer   : S_t = Q_t K^T  (tcgen05.mma, SS, M=N=K=128) into TMEM,
 //                           O_t += P_t V   (tcgen05.mma, A = P_t from TMEM, B = V tile MN-major)
-//   warps 0-3 / 4-7       : softmax of tile 0 / tile 1, one thread per query row, S read from TMEM
-//                           in 32-column chunks (next chunk in flight while this one is processed),
-//                           bf16 P written back over S_t's columns chunk by chunk
+//   warps 0-7             : softmax of tile 0 and tile 1 in turn, TWO threads per query row (64 keys
+//                           each), S read from TMEM in 32-column chunks (next chunk in flight while
+//                           this one is processed), bf16 P written back over the thread's own S columns
 //   epilogue (same warps) : O_t / l -> bf16 -> swizzled smem (the Q_t buffer) -> TMA store
 //
 // Warps 8 and 9 run their control flow warp-uniformly and issue TMA / tcgen05.mma / tcgen05.commit
@@ -22,19 +22,19 @@
 // a precomputed 32-bit base plus a constant, stage counters are incremental, entries are prefetched.
 //
 // Softmax (R-20): p = 2^(s*scale*log2e - m).  The reference max m of a row is the one of the EARLIER
-// key blocks; the row max of the current block is computed beside the exponentials and checked
-// afterwards, so the max -> exp dependency is off the critical path:
-//   growth <= 2^8   : nothing to do (lazy rescale; the final O/l uses the same m, so this is exact)
-//   growth <= 2^100 : this block's P and row sum stay relative to the old m (exact); before the next
-//                     block m is raised and O_t (TMEM) and l are multiplied by f = 2^(m_old - m_new)
-//   growth >  2^100 : (exponentials may have overflowed) the item is flagged and redone by the
+// key blocks, so no max -> exp dependency sits on the critical path; how far the current block
+// outgrew it is read off the block's row sum afterwards (max p <= sum p):
+//   sum <= 2^8      : nothing to do (lazy rescale; the final O/l uses the same m, so this is exact)
+//   sum <  2^100    : this block's P and row sum stay relative to the old m (exact); before the next
+//                     block m is raised by D = floor(log2 sum) + 1 and O_t (TMEM), l are multiplied by 2^-D
+//   otherwise       : (exponentials may have overflowed) the item is flagged and redone by the
 //                     kSafe instantiation of this kernel, which takes the exact row max before the
 //                     exponentials of every block; it is launched right after and returns at once
 //                     when nothing was flagged.
 // The first key block of an item always takes the exact-max path.
 //
-// TMEM (512 columns): S_0 [0,128)  S_1 [128,256)  O_0 [256,384)  O_1 [384,512); P_t aliases the
-// first 64 columns of S_t (tensor-pipe ops run in issue order, so S_t(next) is issued after
+// TMEM (512 columns): S_0 [0,128)  S_1 [128,256)  O_0 [256,384)  O_1 [384,512); P_t (bf16) aliases
+// columns [0,32) and [64,96) of S_t (tensor-pipe ops run in issue order, so S_t(next) is issued after
 // O_t += P_t V(prev) and may overwrite it).
 //
 // Key blocks of an item: first the merged TOPK union of the pair (per entry a 2-bit mask says which
@@ -52,8 +52,8 @@ constexpr int kTile = 128 * 128 * 2;   // bytes of one 128 x 128 bf16 tile
 constexpr int kHalf = kTile / 2;       // one 64-column box
 constexpr int kThreads = 384;
 constexpr float kRescaleThreshold = 8.0f;   // log2 units: below this growth of the row max, keep m
-constexpr float kPanicThreshold = 100.0f;   // log2 units: above this growth, redo the item in the safe kernel
-constexpr uint32_t kPArrivals = 4;          // one elected lane per softmax warp arrives on P_FULL
+constexpr float kPanicSum = 1.2676506e30f;   // 2^100: a block row sum at or above this -> redo the item in the safe kernel
+constexpr uint32_t kPArrivals = 8;          // one lane of each of the 8 softmax warps arrives on P_FULL
 
 // smem carve-up (offsets from a 1024-aligned base)
 constexpr int kOffQ = 0;                          // 2 tiles
@@ -62,7 +62,9 @@ constexpr int kOffV = kOffK + kNK * kTile;
 constexpr int kOffBar = kOffV + kNV * kTile;
 constexpr int kNumBars = 4 + 2 * kNK + 2 * kNV + 6;
 constexpr int kOffTmemPtr = kOffBar + kNumBars * 8;
-constexpr int kSmemBytes = kOffTmemPtr + 16 + 1024;   // + alignment slack
+constexpr int kOffXc = kOffTmemPtr + 16;              // softmax row-pair exchange: [tile][half][row][parity] bytes
+constexpr int kSmemBytes = kOffXc + 2 * 2 * 128 * 2 + 1024;   // + alignment slack
+static_assert(kSmemBytes <= 232448, "more than 227 KB of shared memory");
 
 enum Bar {
   Q_FULL0 = 0, Q_FULL1, Q_EMPTY0, Q_EMPTY1,
@@ -288,13 +290,11 @@ __device__ __forceinline__ uint64_t ex2_pair(uint64_t x, bool emulate) {
   return pack2(p0, p1);
 }
 
-// One 32-column chunk of a softmax pass: p = 2^(s*sl2 - m) as bf16 pairs into pk[], fp32 row sums into
-// the two packed accumulators, and the raw max of the chunk into mx0/mx1 (computed beside the
-// exponentials: the m used here is the running max of the EARLIER key blocks).  `chunk` selects which
-// column pairs take the polynomial; `nvalid_left` < 32 masks the tail of a ragged key block (R-3).
+// One 32-column chunk of a softmax pass: p = 2^(s*sl2 - m) as bf16 pairs into pk[] and fp32 row sums into
+// the two packed accumulators.  `chunk` (0..3, position in the 128-key block) selects which column pairs
+// take the polynomial (unused: the pattern has period 8 pairs); `nvalid_left` < 32 masks the tail of a ragged key block (R-3).
 __device__ __forceinline__ void exp_chunk(uint32_t (&s)[32], uint32_t (&pk)[16], int chunk, int nvalid_left,
-                                          uint64_t sl22, uint64_t nm2, uint64_t& acc0, uint64_t& acc1,
-                                          float& mx0, float& mx1) {
+                                          uint64_t sl22, uint64_t nm2, uint64_t& acc0, uint64_t& acc1) {
   if (nvalid_left < 32) {
 #pragma unroll
     for (int c = 0; c < 32; ++c)
@@ -302,7 +302,7 @@ __device__ __forceinline__ void exp_chunk(uint32_t (&s)[32], uint32_t (&pk)[16],
   }
 #pragma unroll
   for (int u = 0; u < 32; u += 2) {
-    const int j = chunk * 16 + (u >> 1);
+    const int j = (u >> 1);                               // pattern repeats every 8 pairs
     const uint64_t x = fma2(pack2(__uint_as_float(s[u]), __uint_as_float(s[u + 1])), sl22, nm2);
     const uint64_t p = ex2_pair(x, pair_emulated(j));
     if (j & 1) acc1 = add2(acc1, p); else acc0 = add2(acc0, p);
@@ -310,11 +310,12 @@ __device__ __forceinline__ void exp_chunk(uint32_t (&s)[32], uint32_t (&pk)[16],
     unpack2(p, p0, p1);
     pk[u >> 1] = pack_bf16x2(p0, p1);
   }
-#pragma unroll
-  for (int u = 0; u < 32; u += 4) {
-    mx0 = max3(mx0, __uint_as_float(s[u + 0]), __uint_as_float(s[u + 1]));
-    mx1 = max3(mx1, __uint_as_float(s[u + 2]), __uint_as_float(s[u + 3]));
-  }
+}
+
+// upper 16 bits of x rounded toward +infinity (a bf16 >= x); -inf stays -inf
+__device__ __forceinline__ uint32_t bf16_bits_up(float x) {
+  const uint32_t u = __float_as_uint(x);
+  return (u >> 16) + (((u & 0xffffu) != 0u && x > 0.f) ? 1u : 0u);
 }
 
 // instruction descriptor kind::f16: D fp32, A/B bf16, M = N = 128; B MN-major for P V
@@ -480,7 +481,9 @@ uf_attn_sm100_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_cons
           const uint32_t d_tmem = tmem + 256 + t * 128, p_tmem = tmem + t * 128;
 #pragma unroll
           for (int k = 0; k < 8; ++k)
-            mma_ts(d_tmem, p_tmem + k * 8, v_lo + k * (2048 >> 4), kIdescPV, (first_pv[t] && k == 0) ? 0u : 1u);
+            // keys [16k, 16k + 16) of P_t: the thread pair's halves sit at S_t columns [0, 32) and [64, 96)
+            mma_ts(d_tmem, p_tmem + (k >> 2) * 64 + (k & 3) * 8, v_lo + k * (2048 >> 4), kIdescPV,
+                   (first_pv[t] && k == 0) ? 0u : 1u);
           if (left == 0) tc_commit(bars + (V_EMPTY0 + pvs) * 8);
         }
         first_pv[t] = false;
@@ -543,73 +546,95 @@ uf_attn_sm100_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_cons
     }
   } else {
     // ================================== softmax + epilogue ==================================
+    // All 8 warps work on ONE tile at a time (tile 0 and tile 1 alternate, in the order the MMA warp
+    // produces S_0 / S_1): a query row is shared by two threads, lane `lane` of warps wq and wq + 4
+    // (both may touch TMEM lanes [32 wq, 32 wq + 32)); the thread with half = 0 owns S columns (keys)
+    // [0, 64) and O columns [0, 64), the other one [64, 128).  So every scheduler always has two warps
+    // on the same softmax step and the step takes half as long as with one thread per row.
+    // The two threads of a row must use the same reference max m: after a step each publishes in shared
+    // memory by how many binades D its partial row sum exceeds 2^8 (one byte, 0 = not at all; slots
+    // double-buffered by step parity because the partner may be one step ahead); both read the other's
+    // before their next step of that tile (the P_FULL -> S_FULL chain orders the accesses) and raise m by
+    // the larger D: the same number on both sides, and O_t, l are rescaled by an exact power of two.
     asm volatile("setmaxnreg.inc.sync.aligned.u32 208;");
-    const int t = warp >> 2;                           // tile
     const int wq = warp & 3;                           // TMEM lane quarter
+    const int half = warp >> 2;                        // which 64 keys of a block / 64 columns of O
     const int row = wq * 32 + lane;                    // row in the tile == TMEM lane
     const uint32_t lane_addr = (uint32_t)(wq * 32) << 16;
-    const uint32_t s_tmem = tmem + lane_addr + t * 128;
-    const uint32_t o_tmem = tmem + lane_addr + 256 + t * 128;
-    const uint32_t b_sfull = bars + (S_FULL0 + t) * 8;
-    const uint32_t b_pfull = bars + (P_FULL0 + t) * 8;
-    const uint32_t b_ofull = bars + (O_FULL0 + t) * 8;
-    const uint32_t b_qempty = bars + (Q_EMPTY0 + t) * 8;
-    unsigned char* stage = base_ptr + kOffQ + t * kTile;
+    const uint32_t col0 = (uint32_t)half * 64;
     const float sl2 = a.sl2;
     const uint64_t sl22 = pack2(sl2, sl2);
-    uint32_t sph = 0, oph = 0;
+    volatile uint8_t* xc = reinterpret_cast<volatile uint8_t*>(base_ptr + kOffXc);     // [tile][half][row][parity]
+    uint32_t sph0 = 0, sph1 = 0, oph0 = 0, oph1 = 0;
     int trc = 0; (void)trc;                            // UF_DBG_TRACE step counter
 
     UF_ITEM_LOOP_BEGIN
-      if (!(full_mask & (1 << t))) continue;
-      float m = -INFINITY, l = 0.f;
-      float f_pend = 1.0f, m_pend = 0.f;               // pending raise of m: a raise left pending at the end of
-      bool first = true;                               // the item is dropped (O_t / l does not depend on it)
+      // per tile: reference max, partial row sum (this thread's keys), own published D, step parity
+      float m0 = -INFINITY, m1 = -INFINITY, l0 = 0.f, l1 = 0.f;
+      int d0 = 0, d1 = 0, par0 = 0, par1 = 0;
+      bool first0 = true, first1 = true;
 
-      // multiply the O_t row in TMEM by f (O_t is quiescent between S_FULL and our P_FULL arrive: the
-      // commit behind S_FULL also covers the earlier O_t += P_t V)
-      auto rescale_o = [&](float f) {
+      auto softmax_step = [&](const int t, float& m, float& l, int& d_own, int& par, bool& first, uint32_t& sph,
+                              int nvalid) {
+        const uint32_t s_tmem = tmem + lane_addr + t * 128 + col0;          // this thread's 64 S columns
+        const uint32_t o_tmem = tmem + lane_addr + 256 + t * 128 + col0;    // and its 64 O columns
+        volatile uint8_t* x_own = xc + ((t * 2 + half) * 128 + row) * 2;
+        volatile uint8_t* x_oth = xc + ((t * 2 + (half ^ 1)) * 128 + row) * 2;
+        const int left = nvalid - (int)col0;                                // valid keys in this thread's half
+        // multiply this thread's half of the O_t row by f (O_t is quiescent between S_FULL and our
+        // P_FULL arrive: the commit behind S_FULL also covers the earlier O_t += P_t V)
+        auto rescale_o = [&](float f) {
 #pragma unroll
-        for (int cc = 0; cc < 128; cc += 32) {
-          uint32_t ov[32];
-          UF_TMEM_LD32(o_tmem + cc, ov, 0);
-          UF_TMEM_WAIT_LD32(ov);
+          for (int cc = 0; cc < 64; cc += 32) {
+            uint32_t ov[32];
+            UF_TMEM_LD32(o_tmem + cc, ov, 0);
+            UF_TMEM_WAIT_LD32(ov);
 #pragma unroll
-          for (int c = 0; c < 32; ++c) ov[c] = __float_as_uint(__uint_as_float(ov[c]) * f);
-          UF_TMEM_ST32(o_tmem + cc, ov, 0);
-        }
-      };
+            for (int c = 0; c < 32; ++c) ov[c] = __float_as_uint(__uint_as_float(ov[c]) * f);
+            UF_TMEM_ST32(o_tmem + cc, ov, 0);
+          }
+        };
 
-      auto softmax_step = [&](int nvalid) {
-        if (wq == 0 && lane == 0) UF_TR(1 + t, trc, 0);
-        mbar_wait(b_sfull, sph);
+        if (half == 0 && wq == 0 && lane == 0) UF_TR(1 + t, trc, 0);
+        mbar_wait(bars + (S_FULL0 + t) * 8, sph);
         sph ^= 1;
         tc_fence_after();
-        if (wq == 0 && lane == 0) UF_TR(1 + t, trc, 1);
+        if (half == 0 && wq == 0 && lane == 0) UF_TR(1 + t, trc, 1);
         uint32_t sa[32], sb[32], pk[16];
         const bool exact = kSafe || first;
-        if (!kSafe && __any_sync(0xffffffffu, f_pend != 1.0f)) {     // deferred raise of m (see below)
-          rescale_o(f_pend);                                         // f_pend == 1 in rows with nothing pending
-          l *= f_pend;
-          if (f_pend != 1.0f) m = m_pend;
-          f_pend = 1.0f;
+        if (!kSafe && !first) {
+          // deferred raise of m by D binades: the larger of what the two threads of the row published
+          // after the previous step of this tile
+          const int D = max(d_own, (int)x_oth[par ^ 1]);
+          if (__any_sync(0xffffffffu, D > 0)) {
+            const float f = __int_as_float((127 - D) << 23);                // 2^-D (D <= 101), 1 if D == 0
+            rescale_o(f);
+            l *= f;
+            m += (float)D;
+          }
         }
         if (exact) {
-          // exact row max BEFORE the exponentials: first key block of an item / every block when kSafe
+          // exact row max BEFORE the exponentials: first key block of an item / every block when kSafe.
+          // The halves are exchanged as bf16 (both threads then hold the same number).
           float mx0 = -INFINITY, mx1 = -INFINITY;
 #pragma unroll
-          for (int c = 0; c < 4; ++c) {
+          for (int c = 0; c < 2; ++c) {
             UF_TMEM_LD32(s_tmem + c * 32, sa, 0);
             UF_TMEM_WAIT_LD32(sa);
-            const int left = nvalid - c * 32;
 #pragma unroll
             for (int u = 0; u < 32; u += 2) {
-              const float v0 = (u < left) ? __uint_as_float(sa[u]) : -INFINITY;
-              const float v1 = (u + 1 < left) ? __uint_as_float(sa[u + 1]) : -INFINITY;
+              const float v0 = (c * 32 + u < left) ? __uint_as_float(sa[u]) : -INFINITY;
+              const float v1 = (c * 32 + u + 1 < left) ? __uint_as_float(sa[u + 1]) : -INFINITY;
               if (u & 2) mx1 = max3(mx1, v0, v1); else mx0 = max3(mx0, v0, v1);
             }
           }
-          const float m_new = fmaxf(m, fmaxf(mx0, mx1) * sl2);
+          const uint32_t mine = bf16_bits_up(fmaxf(mx0, mx1));
+          *reinterpret_cast<volatile uint16_t*>(x_own) = (uint16_t)mine;
+          asm volatile("bar.sync %0, 64;" ::"r"(2 + wq) : "memory");
+          const uint32_t theirs = *reinterpret_cast<volatile uint16_t*>(x_oth);
+          const float rowmax = fmaxf(__uint_as_float(mine << 16), __uint_as_float(theirs << 16));
+          asm volatile("bar.sync %0, 64;" ::"r"(2 + wq) : "memory");     // both have read: the slot may be reused
+          const float m_new = fmaxf(m, rowmax * sl2);
           if (first) {
             m = m_new;
             first = false;
@@ -622,102 +647,115 @@ uf_attn_sm100_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_cons
             }
           }
         }
-        // exponentials, chunk c + 1 in flight while chunk c is processed; P chunk c goes to columns
-        // [16c, 16c + 16) of S_t, all of which are in registers by then
+        // exponentials of this thread's 64 keys: chunk 1 in flight while chunk 0 is processed; the P chunks
+        // go to columns [col0, col0 + 32) of S_t, which are in registers by then
         const uint64_t nm2 = pack2(-m, -m);
         uint64_t acc0 = pack2(0.f, 0.f), acc1 = acc0;
-        float mx0 = -INFINITY, mx1 = -INFINITY;
         UF_TMEM_LD32(s_tmem + 0, sa, 0);
         UF_TMEM_WAIT_LD32(sa);
         UF_TMEM_LD32(s_tmem + 32, sb, 0);
-        exp_chunk(sa, pk, 0, nvalid, sl22, nm2, acc0, acc1, mx0, mx1);
+        exp_chunk(sa, pk, half * 2 + 0, left, sl22, nm2, acc0, acc1);
         UF_TMEM_ST16(s_tmem + 0, pk);
         UF_TMEM_WAIT_LD32(sb);
-        UF_TMEM_LD32(s_tmem + 64, sa, 0);
-        exp_chunk(sb, pk, 1, nvalid - 32, sl22, nm2, acc0, acc1, mx0, mx1);
+        exp_chunk(sb, pk, half * 2 + 1, left - 32, sl22, nm2, acc0, acc1);
         UF_TMEM_ST16(s_tmem + 16, pk);
-        UF_TMEM_WAIT_LD32(sa);
-        UF_TMEM_LD32(s_tmem + 96, sb, 0);
-        exp_chunk(sa, pk, 2, nvalid - 64, sl22, nm2, acc0, acc1, mx0, mx1);
-        UF_TMEM_ST16(s_tmem + 32, pk);
-        UF_TMEM_WAIT_LD32(sb);
-        exp_chunk(sb, pk, 3, nvalid - 96, sl22, nm2, acc0, acc1, mx0, mx1);
-        UF_TMEM_ST16(s_tmem + 48, pk);
         float a0, a1, b0, b1;
         unpack2(acc0, a0, a1);
         unpack2(acc1, b0, b1);
-        float lsum = (a0 + a1) + (b0 + b1);
+        const float lsum = (a0 + a1) + (b0 + b1);
         l += lsum;
-        if (!exact) {
-          // The row max of this block, checked after the fact.  If it outgrew m by more than 2^8, m is
-          // raised BEFORE THE NEXT block (O_t and l are multiplied by f then: O_t is quiescent again only
-          // after this block's P V); this block's P and row sum stay relative to the old m, which is exact.
-          const float m_new = fmaxf(m, fmaxf(mx0, mx1) * sl2);
-          if ((m_new - m) > kRescaleThreshold) {
-            if ((m_new - m) > kPanicThreshold) {        // exponentials may have overflowed: redo the item
+        if (!kSafe) {
+          // p <= lsum, so while the partial row sum stays below 2^8 no exponent exceeded 8 and m can stay;
+          // otherwise propose to raise m by D = floor(log2 lsum) + 1 binades (m + D > the true max of these keys).
+          int D = 0;
+          if (!(lsum <= 256.0f)) {
+            if (lsum < kPanicSum) {
+              D = (int)((__float_as_uint(lsum) >> 23) & 0xffu) - 126;      // floor(log2 lsum) + 1
+            } else {                                    // (also inf / NaN) exponentials may have overflowed
               a.panic_item[it] = a.seq;
               *a.panic_last = a.seq;
+              D = 101;
             }
-            f_pend = ex2(m - m_new);
-            m_pend = m_new;
           }
+          x_own[par] = (uint8_t)D;
+          d_own = D;
         }
+        par ^= 1;
         tmem_wait_st();
         tc_fence_before();
         __syncwarp();
-        if (lane == 0) mbar_arrive(b_pfull);
-        if (wq == 0 && lane == 0) UF_TR(1 + t, trc, 2);
-        ++trc;
+        if (lane == 0) mbar_arrive(bars + (P_FULL0 + t) * 8);
+        if (half == 0 && wq == 0 && lane == 0) UF_TR(1 + t, trc, 2);
+        if (t == 1) ++trc;
       };
 
+      // ---- the item's key blocks, in the MMA warp's order: per block tile 0 then tile 1 ----
       {
         int32_t mine = 0;
         for (int st = 0; st < n_u; ++st) {
           if ((st & 31) == 0) mine = (st + lane < n_u) ? __ldg(ulist + st + lane) : 0;
           const int32_t e = __shfl_sync(0xffffffffu, mine, st & 31);
-          if (uf_entry_mask(e) & (1 << t)) softmax_step(uf_entry_nvalid(e));
+          const int msk = uf_entry_mask(e), nvalid = uf_entry_nvalid(e);
+          if (msk & 1) softmax_step(0, m0, l0, d0, par0, first0, sph0, nvalid);
+          if (msk & 2) softmax_step(1, m1, l1, d1, par1, first1, sph1, nvalid);
         }
-        for (int j = 0; j < a.n_sink; ++j) softmax_step(min(128, a.sink_ntok - j * 128));
-        for (int j = 0; j < a.nqb; ++j) softmax_step(min(128, a.ntok - j * 128));
+        for (int j = 0; j < a.n_sink + a.nqb; ++j) {
+          const int nvalid = (j < a.n_sink) ? min(128, a.sink_ntok - j * 128) : min(128, a.ntok - (j - a.n_sink) * 128);
+          softmax_step(0, m0, l0, d0, par0, first0, sph0, nvalid);
+          if (full_mask & 2) softmax_step(1, m1, l1, d1, par1, first1, sph1, nvalid);
+        }
       }
 
-      // ---- epilogue: O_t / l -> bf16 -> swizzled staging (Q_t buffer) -> TMA store ----
-      mbar_wait(b_ofull, oph);
-      oph ^= 1;
-      tc_fence_after();
-      const float inv = 1.0f / l;
+      // ---- epilogue per tile: O_t / l -> bf16 -> swizzled staging (the Q_t buffer) -> TMA store ----
+      // (a raise of m still pending here is dropped: O_t / l does not depend on it, and m, l stay consistent)
+      auto epilogue = [&](const int t, float m, float l, uint32_t& oph) {
+        const uint32_t o_tmem = tmem + lane_addr + 256 + t * 128 + col0;
+        unsigned char* stage = base_ptr + kOffQ + t * kTile;
+        mbar_wait(bars + (O_FULL0 + t) * 8, oph);      // every MMA of the item is complete: Q_t is free too
+        oph ^= 1;
+        tc_fence_after();
+        // total row sum = the two threads' partial sums (exchanged through the staging buffer)
+        volatile float* xl = reinterpret_cast<volatile float*>(stage);
+        xl[half * 128 + row] = l;
+        asm volatile("bar.sync 1, 256;" ::: "memory");
+        const float l_tot = l + xl[(half ^ 1) * 128 + row];
+        asm volatile("bar.sync 1, 256;" ::: "memory");                     // all read before the staging writes
+        const float inv = 1.0f / l_tot;
 #pragma unroll
-      for (int cc = 0; cc < 128; cc += 32) {
-        uint32_t ov[32];
-        UF_TMEM_LD32(o_tmem + cc, ov, 0);
-        UF_TMEM_WAIT_LD32(ov);
-        unsigned char* half_base = stage + (cc >> 6) * kHalf + row * 128;
+        for (int cc = 0; cc < 64; cc += 32) {
+          uint32_t ov[32];
+          UF_TMEM_LD32(o_tmem + cc, ov, 0);
+          UF_TMEM_WAIT_LD32(ov);
+          unsigned char* half_base = stage + half * kHalf + row * 128;     // 64-column box `half` of the tile
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-          uint4 w;
-          w.x = pack_bf16x2(__uint_as_float(ov[8 * j + 0]) * inv, __uint_as_float(ov[8 * j + 1]) * inv);
-          w.y = pack_bf16x2(__uint_as_float(ov[8 * j + 2]) * inv, __uint_as_float(ov[8 * j + 3]) * inv);
-          w.z = pack_bf16x2(__uint_as_float(ov[8 * j + 4]) * inv, __uint_as_float(ov[8 * j + 5]) * inv);
-          w.w = pack_bf16x2(__uint_as_float(ov[8 * j + 6]) * inv, __uint_as_float(ov[8 * j + 7]) * inv);
-          const int chunk = ((cc & 63) >> 3) + j;                  // 16-byte chunk within the 128-byte row
-          *reinterpret_cast<uint4*>(half_base + ((chunk ^ (row & 7)) << 4)) = w;
+          for (int j = 0; j < 4; ++j) {
+            uint4 w;
+            w.x = pack_bf16x2(__uint_as_float(ov[8 * j + 0]) * inv, __uint_as_float(ov[8 * j + 1]) * inv);
+            w.y = pack_bf16x2(__uint_as_float(ov[8 * j + 2]) * inv, __uint_as_float(ov[8 * j + 3]) * inv);
+            w.z = pack_bf16x2(__uint_as_float(ov[8 * j + 4]) * inv, __uint_as_float(ov[8 * j + 5]) * inv);
+            w.w = pack_bf16x2(__uint_as_float(ov[8 * j + 6]) * inv, __uint_as_float(ov[8 * j + 7]) * inv);
+            const int chunk = (cc >> 3) + j;                               // 16-byte chunk within the 128-byte row
+            *reinterpret_cast<uint4*>(half_base + ((chunk ^ (row & 7)) << 4)) = w;
+          }
         }
-      }
-      tc_fence_before();
-      fence_proxy_async();
-      asm volatile("bar.sync %0, 128;" ::"r"(1 + t) : "memory");
-      const int row0 = (2 * p + t) * 128;
-      if (wq == 0 && lane == 0) {
-        const uint32_t src = base + kOffQ + t * kTile;
-        tma_store_3d(&tm_o, src, 0, row0, h);
-        tma_store_3d(&tm_o, src + kHalf, 64, row0, h);
-        tma_store_commit_and_wait_read();
-        mbar_arrive(b_qempty);
-      }
-      if (a.lse != nullptr && row0 + row < a.ntok)
-        a.lse[(int64_t)h * a.ntok + row0 + row] = (m + log2f(l)) * 0.6931471805599453f;
+        tc_fence_before();
+        fence_proxy_async();
+        asm volatile("bar.sync 1, 256;" ::: "memory");
+        const int row0 = (2 * p + t) * 128;
+        if (warp == 0 && lane == 0) {
+          const uint32_t src = base + kOffQ + t * kTile;
+          tma_store_3d(&tm_o, src, 0, row0, h);
+          tma_store_3d(&tm_o, src + kHalf, 64, row0, h);
+          tma_store_commit_and_wait_read();
+          mbar_arrive(bars + (Q_EMPTY0 + t) * 8);
+        }
+        if (half == 0 && a.lse != nullptr && row0 + row < a.ntok)
+          a.lse[(int64_t)h * a.ntok + row0 + row] = (m + log2f(l_tot)) * 0.6931471805599453f;
+      };
+      epilogue(0, m0, l0, oph0);
+      if (full_mask & 2) epilogue(1, m1, l1, oph1);
     UF_ITEM_LOOP_END
-    if (wq == 0 && lane == 0) tma_store_wait_all();
+    if (warp == 0 && lane == 0) tma_store_wait_all();
   }
 #undef UF_ITEM_LOOP_BEGIN
 #undef UF_ITEM_LOOP_END
