@@ -143,6 +143,12 @@ int32_t uf_get_cache_block(uf_ctx* ctx, int32_t global_block, int32_t head,
  * host memory (same addressing as uf_get_cache_block).  Synchronises `stream`. */
 int32_t uf_get_pooled_k(uf_ctx* ctx, int32_t global_block, int32_t head, double* out, void* stream);
 
+/* uf_attn_redone_items: how many work items (head, query-block pair) of the LAST uf_sparse_attn_fwd call
+ * were redone by the exact-max ("safe") instantiation of the tcgen05 attention kernel because a row
+ * max outgrew the running reference by 2^100 or more within one key block.  Writes the
+ * count to host memory `*n_items` (0 for the generic kernel).  Synchronises `stream`. */
+int32_t uf_attn_redone_items(uf_ctx* ctx, int32_t* n_items, void* stream);
+
 /* Bytes of device memory the ctx owns. */
 int64_t uf_ctx_device_bytes(const uf_ctx* ctx);
 

@@ -7,14 +7,14 @@ loudly (UFError) without one.
 """
 from .binding import (  # noqa: F401
     LIB_PATH, SYMBOLS, UFError, load_library, uf_ctx_create, uf_ctx_destroy, uf_ctx_device_bytes,
-    uf_ctx_launch_count, uf_ctx_reset, uf_get_cache_block, uf_get_pooled_k, uf_get_slot_map, uf_kv_append,
+    uf_attn_redone_items, uf_ctx_launch_count, uf_ctx_reset, uf_get_cache_block, uf_get_pooled_k, uf_get_slot_map, uf_kv_append,
     uf_last_error, uf_query_topk, uf_select_blocks, uf_set_attn_impl, uf_sparse_attn_fwd, uf_version,
 )
 from .build import build  # noqa: F401
 
 __all__ = [
     "LIB_PATH", "SYMBOLS", "UFError", "build", "load_library", "uf_ctx_create", "uf_ctx_destroy",
-    "uf_ctx_device_bytes", "uf_ctx_launch_count", "uf_ctx_reset", "uf_get_cache_block", "uf_get_pooled_k",
+    "uf_attn_redone_items", "uf_ctx_device_bytes", "uf_ctx_launch_count", "uf_ctx_reset", "uf_get_cache_block", "uf_get_pooled_k",
     "uf_get_slot_map", "uf_kv_append", "uf_last_error", "uf_query_topk", "uf_select_blocks", "uf_set_attn_impl",
     "uf_sparse_attn_fwd", "uf_version",
 ]

@@ -23,7 +23,7 @@ _ERR_NAMES = {1: "UF_ERR_INVALID_ARG", 2: "UF_ERR_STATE", 3: "UF_ERR_CAPACITY", 
 SYMBOLS = [
     "uf_ctx_create", "uf_ctx_destroy", "uf_ctx_reset", "uf_kv_append", "uf_query_topk", "uf_select_blocks",
     "uf_sparse_attn_fwd", "uf_set_attn_impl", "uf_get_slot_map", "uf_get_cache_block", "uf_get_pooled_k",
-    "uf_ctx_device_bytes", "uf_ctx_launch_count", "uf_last_error", "uf_version",
+    "uf_attn_redone_items", "uf_ctx_device_bytes", "uf_ctx_launch_count", "uf_last_error", "uf_version",
 ]
 
 
@@ -64,6 +64,7 @@ def load_library() -> ctypes.CDLL:
     lib.uf_get_pooled_k.argtypes = [P, c_int32, c_int32, POINTER(c_double), P]
     lib.uf_ctx_device_bytes.argtypes = [P]
     lib.uf_ctx_device_bytes.restype = c_int64
+    lib.uf_attn_redone_items.argtypes = [P, POINTER(c_int32), P]
     lib.uf_ctx_launch_count.argtypes = [P]
     lib.uf_ctx_launch_count.restype = c_int64
     lib.uf_last_error.argtypes = [P]
@@ -173,6 +174,12 @@ def uf_get_pooled_k(ctx, global_block: int, head: int, out, stream=None) -> None
 
 def uf_ctx_device_bytes(ctx) -> int:
     return load_library().uf_ctx_device_bytes(ctx)
+
+
+def uf_attn_redone_items(ctx, stream=None) -> int:
+    n = c_int32(0)
+    _check(ctx, load_library().uf_attn_redone_items(ctx, byref(n), _stream(stream)))
+    return int(n.value)
 
 
 def uf_ctx_launch_count(ctx) -> int:

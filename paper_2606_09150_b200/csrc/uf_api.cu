@@ -294,6 +294,7 @@ int32_t uf_sparse_attn_fwd(uf_ctx* c, const void* q, void* o, float* lse, int32_
   float scale = softmax_scale == 0.0f ? (float)(1.0 / std::sqrt((double)c->cfg.head_dim)) : softmax_scale;
   UF_CUDA(c, cudaSetDevice(c->cfg.device));
   const bool fast = (c->cfg.block == 128 && c->cfg.head_dim == 128 && c->attn_impl == 0 && c->tm_ok);
+  c->last_attn_sm100 = fast;
   if (fast)
     return uf_launch_attn_sm100(c, v, (const __nv_bfloat16*)q, (__nv_bfloat16*)o, lse, tok_stride, head_stride,
                                 scale, (cudaStream_t)stream);
@@ -370,5 +371,24 @@ int32_t uf_get_pooled_k(uf_ctx* c, int32_t g, int32_t head, double* out, void* s
 
 int64_t uf_ctx_device_bytes(const uf_ctx* c) { return c ? c->dev_bytes : 0; }
 int64_t uf_ctx_launch_count(const uf_ctx* c) { return c ? c->launches : 0; }
+
+int32_t uf_attn_redone_items(uf_ctx* c, int32_t* n_items, void* stream) {
+  if (!c || !n_items) return UF_ERR_INVALID_ARG;
+  if (c->host_only) return fail(c, UF_ERR_STATE, "uf_attn_redone_items: host-only ctx");
+  *n_items = 0;
+  if (c->attn_seq == 0 || !c->last_attn_sm100) return UF_OK;
+  UF_CUDA(c, cudaSetDevice(c->cfg.device));
+  UF_CUDA(c, cudaStreamSynchronize((cudaStream_t)stream));
+  const size_t n = (size_t)c->cfg.n_heads * ((c->BPC + 1) / 2);
+  int32_t* host = new (std::nothrow) int32_t[n];
+  if (!host) return fail(c, UF_ERR_CAPACITY, "uf_attn_redone_items: out of host memory");
+  cudaError_t e = cudaMemcpy(host, c->panic_item, n * sizeof(int32_t), cudaMemcpyDeviceToHost);
+  if (e != cudaSuccess) { delete[] host; return fail_cuda(c, e, "cudaMemcpy(panic_item)"); }
+  int cnt = 0;
+  for (size_t i = 0; i < n; ++i) cnt += (host[i] == c->attn_seq);
+  delete[] host;
+  *n_items = cnt;
+  return UF_OK;
+}
 
 }  // extern "C"

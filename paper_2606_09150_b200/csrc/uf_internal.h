@@ -75,6 +75,7 @@ struct uf_ctx {
   int32_t* panic_item = nullptr;  // [H][NP]: == attn_seq when the safe attention kernel must redo the item
   int32_t* panic_last = nullptr;  // [1]: == attn_seq when the last fast launch flagged anything
   int32_t attn_seq = 0;           // sm100 attention launch sequence number
+  bool last_attn_sm100 = false;   // the last uf_sparse_attn_fwd ran the sm100 kernels
   int kcap = 0;                   // (C-1)*BPC
   int64_t dev_bytes = 0;
   // host state

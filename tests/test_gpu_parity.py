@@ -138,6 +138,41 @@ def test_custom_scale_and_no_lse():
         cu.close()
 
 
+@pytest.mark.parametrize("scale", [0.3, 8.0])
+def test_sharp_softmax_deferred_raise_and_safe_kernel(scale):
+    """Logits far sharper than 1/sqrt(d) gives.  scale 0.3: the row max outgrows the running reference by
+    many binades inside single key blocks, so the deferred raise of m (O_t, l rescaled by 2^-D before the
+    next block) runs all the time.  scale 8: it outgrows it by more than 2^100, the exponentials overflow,
+    the items are flagged and the exact-max ("safe") instantiation of the kernel must redo them; the result
+    is then practically a one-hot selection of V rows.  The generic kernel is the second opinion."""
+    import torch
+    w = wl.scaled(wl.CONFIGS["1k"], "sharp128", n_heads=2, frames_per_chunk=1, grid_h=20, grid_w=29,
+                  capacity_chunks=3, topk_percent=50)
+    assert w.chunk_tokens == 580                                    # 5 query blocks, ragged tail of 68
+    cu, orc = hz.CudaStream(w), hz.make_oracle(w)
+    try:
+        redone = 0
+        for c in range(3):
+            Qb, Kb, Vb = wl.make_chunk(w, c)
+            got = cu.step(Qb, Kb, Vb, topk_percent=50, scale=scale)
+            redone += cu.uf.uf_attn_redone_items(cu.ctx, cu.stream)
+            ref = hz.oracle_step(orc, Qb, Kb, Vb, topk_percent=50, scale=scale)
+            hz.compare_step(got, ref, f"[sharp scale {scale} chunk {c}]")
+            q = cu.to_dev(Qb)
+            o2 = torch.empty_like(q)
+            n, H, d = Qb.shape
+            cu.uf.uf_set_attn_impl(cu.ctx, 1)
+            cu.uf.uf_sparse_attn_fwd(cu.ctx, q, o2, None, n, H * d, d, scale, cu.stream)
+            torch.cuda.synchronize()
+            assert cu.uf.uf_attn_redone_items(cu.ctx, cu.stream) == 0        # generic kernel: nothing to redo
+            diff = np.abs(got["O"] - o2.float().cpu().numpy())
+            assert diff.max() <= 2e-2 and diff.mean() <= 2e-3, (diff.max(), diff.mean())
+        if scale >= 8.0:
+            assert redone > 0, "scale 8 must overflow the stale-max exponentials and take the safe kernel"
+    finally:
+        cu.close()
+
+
 def test_error_codes_and_call_order():
     import torch
     import paper_2606_09150_b200 as uf
