@@ -30,6 +30,10 @@ if ROOT not in sys.path:
 
 import uf_workloads as wl  # noqa: E402
 
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE uf_attn_sm100_kernel<false> launch, from the committed
+# `ncu --set full` capture of this command (profiles/README.md names it); null for workloads not captured.
+NCU_ATTN_DRAM_BYTES = {"1k": 471.0e6 + 66.0e6}
+
 METRIC = "effective TFLOP/s on kept blocks, sparse causal chunk attention step (ms/chunk in ms_per_step)"
 UNIT = "TFLOP/s"
 
@@ -73,7 +77,7 @@ class ClockSampler:
     def __enter__(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.device}", f"--query-gpu={self.Q}",
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "20"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.th = threading.Thread(target=self._read, daemon=True)
             self.th.start()
@@ -181,9 +185,15 @@ class HotPath:
     def close(self):
         self.uf.uf_ctx_destroy(self.ctx)
 
-    def step(self, q, k, v, ev=None):
+    def step(self, q, k, v, ev=None, ev_pre=None):
+        """ev = (before attention, after attention); ev_pre = (before append, before select) for the
+        per-call breakdown pass (not used inside the timed region)."""
         uf, w = self.uf, self.w
+        if ev_pre is not None:
+            ev_pre[0].record(self.stream)
         uf.uf_kv_append(self.ctx, k, v, self.n, self.ts, self.hs, 0, self.stream)
+        if ev_pre is not None:
+            ev_pre[1].record(self.stream)
         uf.uf_select_blocks(self.ctx, q, self.n, self.ts, self.hs, w.topk_count, w.topk_percent,
                             self.idx, self.cnt, self.stream)
         if ev is not None:
@@ -193,9 +203,9 @@ class HotPath:
             ev[1].record(self.stream)
         self.step_no += 1
 
-    def step_resident(self, ev=None):
+    def step_resident(self, ev=None, ev_pre=None):
         q, k, v = self.devc[self.step_no % len(self.devc)]
-        self.step(q, k, v, ev)
+        self.step(q, k, v, ev, ev_pre)
 
     def step_e2e(self):
         hq, hk, hv = self.host[self.step_no % len(self.host)]
@@ -240,6 +250,34 @@ def time_steps(hp: HotPath, steps: int, warmup: int, e2e: bool):
     attn_ms = None if e2e else float(np.mean([a.elapsed_time(b) for a, b in attn_ev]))
     launches = hp.uf.uf_ctx_launch_count(hp.ctx) - launches0
     return total_ms, attn_ms, launches
+
+
+def call_breakdown(hp: HotPath, steps: int, hbm_gbs: float):
+    """Separate pass after the timed region: CUDA events around each of the three C-ABI calls, and the
+    HBM-roofline view of the two data-movement calls (algorithmic bytes of DESIGN.md 5.2 / 5.3)."""
+    torch, w = hp.torch, hp.w
+    E = lambda: torch.cuda.Event(enable_timing=True)  # noqa: E731
+    evs = [(E(), E(), E(), E()) for _ in range(steps)]
+    for e in evs:
+        hp.step_resident(ev=(e[2], e[3]), ev_pre=(e[0], e[1]))
+    torch.cuda.synchronize(hp.dev)
+    app = float(np.mean([e[0].elapsed_time(e[1]) for e in evs]))
+    sel = float(np.mean([e[1].elapsed_time(e[2]) for e in evs]))
+    att = float(np.mean([e[2].elapsed_time(e[3]) for e in evs]))
+    nhd2 = hp.n * hp.H * hp.d * 2
+    nb = -(-hp.n // w.block)
+    app_bytes = 4 * nhd2 + 8 * hp.H * hp.d * nb                       # read K,V + write both caches + pooled K
+    n_cand, k_eff = hp.uf.uf_query_topk(hp.ctx, w.topk_count, w.topk_percent)
+    sel_bytes = nhd2 + 8 * hp.H * hp.d * (nb + n_cand) + 4 * hp.H * nb * (k_eff + 1)   # read Q, pooled Q/K, write ids
+    return {
+        "append": {"ms": app, "algorithmic_bytes": app_bytes, "achieved_gbs": app_bytes / app / 1e6,
+                   "frac_of_hbm_peak": app_bytes / app / 1e6 / hbm_gbs},
+        "select": {"ms": sel, "algorithmic_bytes": sel_bytes, "achieved_gbs": sel_bytes / sel / 1e6,
+                   "frac_of_hbm_peak": sel_bytes / sel / 1e6 / hbm_gbs,
+                   "note": "3 kernels: pool Q (HBM-bound), fp64 score + exact rank top-k (ALU-bound), pair merge"},
+        "attention": {"ms": att},
+        "hbm_peak_gbs": hbm_gbs,
+    }
 
 
 def stream_percentiles(hp: HotPath, repeats: int):
@@ -339,6 +377,7 @@ def measure_workload(w, device, steps, warmup, with_e2e=True):
         flop, n_cand, k_eff = hp.current_kept_flop()
         out = {"total_ms": total_ms, "attn_ms": attn_ms, "launches": launches, "flop": flop, "n_cand": n_cand,
                "k_eff": k_eff, "clocks": cs.summary(), "device_bytes": hp.uf.uf_ctx_device_bytes(hp.ctx)}
+        out["calls"] = call_breakdown(hp, min(steps, 10), load_peaks()["hbm_gbs"])
         if with_e2e:
             e2e_ms, _, _ = time_steps(hp, steps, min(warmup, 3), e2e=True)
             out["e2e_ms"] = e2e_ms
@@ -405,11 +444,12 @@ def main():
         "clocks": m["clocks"],
         "roofline": {
             "kernel": "uf_attn_sm100_kernel", "bound": "tensor", "achieved": attn_tflops, "peak": peaks["bf16_burst"],
-            "unit": "TFLOP/s", "frac": attn_tflops / peaks["bf16_burst"], "traffic": None,
+            "unit": "TFLOP/s", "frac": attn_tflops / peaks["bf16_burst"], "traffic": NCU_ATTN_DRAM_BYTES.get(w.name),
             "peak_source": peaks["source"] + ", bf16 burst; sustained %.1f -> frac %.3f" % (
                 peaks["bf16_sustained"], attn_tflops / peaks["bf16_sustained"]),
             "algorithmic_flop_per_launch": m["flop"],
         },
+        "calls": m["calls"],
     }
     if rank == 0 and not args.no_also and args.workload == "1k":
         m2 = measure_workload(wl.CONFIGS["2k"], device, max(3, args.steps // 2), 3, with_e2e=False)

@@ -94,7 +94,7 @@ uf_score_topk_kernel(UfView v, const double* __restrict__ qbar, const double* __
     double acc[kQG];
 #pragma unroll
     for (int g = 0; g < kQG; ++g) acc[g] = 0.0;
-#pragma unroll 4
+#pragma unroll 16
     for (int t = 0; t < D; ++t) {
       const double kv = kp[(int64_t)t * v.P];
 #pragma unroll
@@ -147,34 +147,64 @@ uf_score_topk_kernel(UfView v, const double* __restrict__ qbar, const double* __
 }
 
 // ---- merge the lists of query blocks (2p, 2p+1) into one ascending union with tile masks ----------
-// One thread per (h, pair).  Both lists are subsequences of CAND in candidate order (sel_rank holds the
-// candidate index of every kept entry), so a two-pointer merge yields the union in that order; bit 0 of
-// the mask = tile 0 (block 2p) attends the entry, bit 1 = tile 1 (block 2p+1).
-__global__ void uf_pair_merge_kernel(const int32_t* __restrict__ sel_q, const int32_t* __restrict__ sel_rank,
-                                     int32_t* __restrict__ sel_pair, int32_t* __restrict__ pair_cnt,
-                                     int H, int BPC, int nqb, int k_eff, int kcap) {
-  const int NP = (BPC + 1) / 2;
+// One warp per (h, pair).  Both lists are subsets of CAND; sel_rank holds the candidate index of every kept
+// entry, so each list becomes a bitmap over the candidates in shared memory, the union is the OR of the two,
+// an entry's position is the number of union bits below it (word popcounts + a warp scan), and its payload
+// (physical block, valid rows) is recomputed from the candidate index.  Bit 0 of the mask = tile 0 (block 2p)
+// attends the entry, bit 1 = tile 1 (block 2p+1).  dynamic smem: uint32 [warps][2][ceil(n_cand / 32)]
+constexpr int kMergeWarps = 4;
+__global__ void __launch_bounds__(kMergeWarps * 32)
+uf_pair_merge_kernel(UfView v, const int32_t* __restrict__ sel_rank, int32_t* __restrict__ sel_pair,
+                     int32_t* __restrict__ pair_cnt, int nqb, int k_eff, int kcap) {
+  extern __shared__ uint32_t bm_raw[];
+  const int NP = (v.BPC + 1) / 2;
   const int np_cur = (nqb + 1) / 2;
-  const int x = blockIdx.x * blockDim.x + threadIdx.x;
-  if (x >= H * np_cur) return;
+  const int nw = (v.n_cand + 31) / 32;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int x = blockIdx.x * kMergeWarps + warp;
+  if (x >= v.H * np_cur) return;
   const int h = x / np_cur, p = x % np_cur;
-  const int i0 = 2 * p, i1 = 2 * p + 1;
-  const int32_t* a = sel_q + ((int64_t)h * BPC + i0) * kcap;
-  const int32_t* ra = sel_rank + ((int64_t)h * BPC + i0) * kcap;
-  const bool has1 = i1 < nqb;
-  const int32_t* b = sel_q + ((int64_t)h * BPC + i1) * kcap;
-  const int32_t* rb = sel_rank + ((int64_t)h * BPC + i1) * kcap;
-  int32_t* out = sel_pair + ((int64_t)h * NP + p) * 2 * kcap;
-  int ia = 0, ib = 0, n = 0;
-  const int na = k_eff, nb = has1 ? k_eff : 0;
-  while (ia < na || ib < nb) {
-    const int ka = ia < na ? ra[ia] : 0x7fffffff;
-    const int kb = ib < nb ? rb[ib] : 0x7fffffff;
-    if (ka == kb)      { out[n++] = a[ia] | (3 << 28); ++ia; ++ib; }
-    else if (ka < kb)  { out[n++] = a[ia] | (1 << 28); ++ia; }
-    else               { out[n++] = b[ib] | (2 << 28); ++ib; }
+  uint32_t* bma = bm_raw + (size_t)warp * 2 * nw;
+  uint32_t* bmb = bma + nw;
+  for (int w = lane; w < 2 * nw; w += 32) bma[w] = 0u;
+  __syncwarp();
+  const int32_t* ra = sel_rank + ((int64_t)h * v.BPC + 2 * p) * kcap;
+  const int32_t* rb = ra + kcap;
+  const bool has1 = 2 * p + 1 < nqb;
+  for (int e = lane; e < k_eff; e += 32) {
+    const int ja = ra[e];
+    atomicOr(&bma[ja >> 5], 1u << (ja & 31));
+    if (has1) {
+      const int jb = rb[e];
+      atomicOr(&bmb[jb >> 5], 1u << (jb & 31));
+    }
   }
-  pair_cnt[(int64_t)h * NP + p] = n;
+  __syncwarp();
+  int32_t* out = sel_pair + ((int64_t)h * NP + p) * 2 * kcap;
+  int base = 0;
+  for (int w0 = 0; w0 < nw; w0 += 32) {
+    const int w = w0 + lane;
+    const uint32_t wa = w < nw ? bma[w] : 0u, wb = w < nw ? bmb[w] : 0u;
+    uint32_t u = wa | wb;
+    const int cnt = __popc(u);
+    int incl = cnt;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int y = __shfl_up_sync(0xffffffffu, incl, o);
+      if (lane >= o) incl += y;
+    }
+    int pos = base + incl - cnt;
+    while (u) {
+      const int b = __ffs(u) - 1;
+      u &= u - 1;
+      int gid, phys, nval;
+      uf_cand_lookup(v, w * 32 + b, &gid, &phys, &nval);
+      const int mask = ((wa >> b) & 1u) | (((wb >> b) & 1u) << 1);
+      out[pos++] = uf_entry_pack(phys, nval, mask);
+    }
+    base += __shfl_sync(0xffffffffu, incl, 31);
+  }
+  if (lane == 0) pair_cnt[(int64_t)h * NP + p] = base;
 }
 
 }  // namespace
@@ -231,9 +261,9 @@ cudaError_t uf_launch_select(uf_ctx* c, const UfView& v, const __nv_bfloat16* q,
   if (e != cudaSuccess) return e;
   if (v.B == 128 && v.d == 128) {
     const int np_cur = (nqb + 1) / 2;
-    uf_pair_merge_kernel<<<uf_ceil_div(v.H * np_cur, 128), 128, 0, s>>>(c->sel_q, c->sel_rank, c->sel_pair,
-                                                                        c->pair_cnt, v.H, v.BPC, nqb, k_eff,
-                                                                        c->kcap);
+    const size_t msmem = (size_t)kMergeWarps * 2 * uf_ceil_div(v.n_cand, 32) * sizeof(uint32_t);
+    uf_pair_merge_kernel<<<uf_ceil_div(v.H * np_cur, kMergeWarps), kMergeWarps * 32, msmem, s>>>(
+        v, c->sel_rank, c->sel_pair, c->pair_cnt, nqb, k_eff, c->kcap);
     c->launches += 1;
     e = cudaGetLastError();
   }
