@@ -73,7 +73,6 @@ uf_score_topk_kernel(UfView v, const double* __restrict__ qbar, const double* __
   extern __shared__ __align__(16) unsigned char smem_raw[];
   double* qs = reinterpret_cast<double*>(smem_raw);                                  // [kQG][D]
   unsigned long long* key = reinterpret_cast<unsigned long long*>(qs + kQG * D);     // [kQG][n_cand]
-  __shared__ int warp_cnt[kScoreThreads / 32];
   const int h = blockIdx.y;
   const int i0 = blockIdx.x * kQG;
   const int ng = min(kQG, nqb - i0);
@@ -105,44 +104,47 @@ uf_score_topk_kernel(UfView v, const double* __restrict__ qbar, const double* __
   }
   __syncthreads();
 
-  // rank of candidate j = #{j' : s[j'] > s[j]} + #{j' < j : s[j'] == s[j]}; kept iff rank < k'.
-  // Candidates are in ascending global id, so an ordered compaction emits ascending ids.
-  for (int g = 0; g < ng; ++g) {
+  // Exact top-k', one warp per query block.  T = the k'-th largest key, found bit by bit from the top
+  // (T is the largest value with #{key >= T} >= k').  Kept: every key > T, and of the keys == T the first
+  // (k' - #{key > T}) in candidate order, i.e. ties go to the lower global id (R-12).  Candidates are in
+  // ascending global id, so the ordered ballot compaction below emits ascending ids.
+  const int lane = tid & 31, wid = tid >> 5;
+  for (int g = wid; g < ng; g += kScoreThreads / 32) {
     const unsigned long long* kg = key + (int64_t)g * nc;
     const int i = i0 + g;
-    int base = 0;
-    for (int j0 = 0; j0 < nc; j0 += kScoreThreads) {
-      const int j = j0 + tid;
-      bool keep = false;
-      if (j < nc) {
-        const unsigned long long mine = kg[j];
-        int rank = 0;
-        for (int jj = 0; jj < nc; ++jj) {
-          const unsigned long long o = kg[jj];
-          rank += (o > mine) || (o == mine && jj < j);
-        }
-        keep = rank < k_eff;
-      }
+    unsigned long long T = 0ull;
+    for (int b = 63; b >= 0; --b) {
+      const unsigned long long cand = T | (1ull << b);
+      int cnt = 0;
+      for (int j = lane; j < nc; j += 32) cnt += (kg[j] >= cand);
+      cnt = __reduce_add_sync(0xffffffffu, cnt);
+      if (cnt >= k_eff) T = cand;
+    }
+    int n_gt = 0;
+    for (int j = lane; j < nc; j += 32) n_gt += (kg[j] > T);
+    n_gt = __reduce_add_sync(0xffffffffu, n_gt);
+    const int need_eq = k_eff - n_gt;                  // >= 1 by the definition of T
+    int pos0 = 0, eq_seen = 0;
+    const int64_t rowq = ((int64_t)h * v.BPC + i) * kcap;
+    for (int j0 = 0; j0 < nc; j0 += 32) {
+      const int j = j0 + lane;
+      const unsigned long long mine = j < nc ? kg[j] : 0ull;
+      const bool gt = j < nc && mine > T, eq = j < nc && mine == T;
+      const unsigned beq = __ballot_sync(0xffffffffu, eq);
+      const bool keep = gt || (eq && eq_seen + __popc(beq & ((1u << lane) - 1u)) < need_eq);
       const unsigned ball = __ballot_sync(0xffffffffu, keep);
-      const int lane = tid & 31, w = tid >> 5;
-      if (lane == 0) warp_cnt[w] = __popc(ball);
-      __syncthreads();
-      int off = base;
-      for (int ww = 0; ww < w; ++ww) off += warp_cnt[ww];
-      int total = 0;
-      for (int ww = 0; ww < kScoreThreads / 32; ++ww) total += warp_cnt[ww];
       if (keep) {
-        const int pos = off + __popc(ball & ((1u << lane) - 1u));
+        const int pos = pos0 + __popc(ball & ((1u << lane) - 1u));
         int gid, phys, nval;
         uf_cand_lookup(v, j, &gid, &phys, &nval);
-        sel_q[((int64_t)h * v.BPC + i) * kcap + pos] = uf_entry_pack(phys, nval, 0);
-        sel_rank[((int64_t)h * v.BPC + i) * kcap + pos] = j;       // candidate index: the merge key
+        sel_q[rowq + pos] = uf_entry_pack(phys, nval, 0);
+        sel_rank[rowq + pos] = j;                      // candidate index: the merge key
         if (idx_out) idx_out[((int64_t)h * nqb + i) * k_eff + pos] = gid;
       }
-      base += total;
-      __syncthreads();
+      pos0 += __popc(ball);
+      eq_seen += __popc(beq);
     }
-    if (tid == 0 && cnt_out) cnt_out[(int64_t)h * nqb + i] = k_eff;
+    if (lane == 0 && cnt_out) cnt_out[(int64_t)h * nqb + i] = k_eff;
   }
 }
 
