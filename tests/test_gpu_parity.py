@@ -211,9 +211,9 @@ def _sampled_pairs(w, n_random, seed):
     return heads, qblocks
 
 
-@pytest.mark.parametrize("name", ["1k", "2k"])
+@pytest.mark.parametrize("name", ["1k", "2k", "wide"])
 def test_full_size_step(name):
-    """BASELINE.json configs[1] / configs[2] at full size, in the launch configuration bench.py times:
+    """BASELINE.json configs[1] / configs[2] / configs[4] at full size, in the launch configuration bench.py times:
     slot maps and ALL selected block ids bit-exact; attention compared on sampled (head, query block)
     pairs the oracle computes one by one (first, second, last two blocks incl. the ragged one, + random)."""
     w = wl.CONFIGS[name]
@@ -231,6 +231,33 @@ def test_full_size_step(name):
                 assert not np.isnan(got["O"]).any(), "every output row must be written"
                 assert np.isfinite(got["lse"]).all()
                 print(f"{name}: sampled O max-abs {r[0]:.3e} mean-abs {r[1]:.3e}, oracle min top-k gap {ref['min_gap']:.3e}")
+    finally:
+        cu.close()
+
+
+def test_full_size_rolling_stream():
+    """BASELINE.json configs[3]: 20 consecutive 1K chunks (per-chunk seeds 0..19), capacity 3 chunks + sink, oldest
+    non-sink chunk evicted after each append.  Slot maps and ALL selected block ids bit-exact on every chunk;
+    attention compared on sampled (head, query block) pairs on ramp-up, mid-stream and final chunks; after the
+    stream the cache holds chunks 17, 18, 19 + the sink, byte-exact."""
+    w = wl.CONFIGS["1k_stream"]
+    heads, qblocks = [0, w.n_heads - 1], [0, 95, w.bpc - 1]
+    check_attn = {0, 1, 2, 3, 10, w.n_stream_chunks - 1}
+    cu, orc = hz.CudaStream(w), hz.make_oracle(w)
+    try:
+        worst = 0.0
+        for c in range(w.n_stream_chunks):
+            Qb, Kb, Vb = wl.make_chunk(w, c)
+            got = cu.step(Qb, Kb, Vb, topk_percent=w.topk_percent)
+            ref = hz.oracle_step(orc, Qb, Kb, Vb, topk_percent=w.topk_percent, heads=heads, qblocks=qblocks,
+                                 attn=c in check_attn)
+            r = hz.compare_step(got, ref, f"[1k_stream chunk {c}]")
+            if r:
+                worst = max(worst, r[0])
+            assert cu.uf.uf_attn_redone_items(cu.ctx, cu.stream) == 0
+        assert sorted(x for x in got["slot_map"][0] if x >= 0) == [17, 18, 19]
+        _check_cache(cu, orc, w)
+        print(f"1k_stream: worst sampled O max-abs {worst:.3e}")
     finally:
         cu.close()
 
