@@ -42,13 +42,21 @@ class CudaStream:
         t = self.torch.from_numpy(bits.view(np.int16)).to(self.dev)
         return t.view(self.torch.bfloat16)
 
-    def step(self, Qb, Kb, Vb, topk_count=-1, topk_percent=-1, window=0, want_lse=True, impl=0, scale=0.0):
+    def step(self, Qb, Kb, Vb, topk_count=-1, topk_percent=-1, window=0, want_lse=True, impl=0, scale=0.0,
+             fused_qkv=False):
         """append -> select -> attention for one chunk of bf16 bit arrays [n, H, d].
+        fused_qkv: Q, K, V are the three slices of ONE [n, 3, H, d] tensor (token stride 3*H*d), the layout a
+        fused QKV projection leaves them in, and O is written into a slice of a [n, 2, H, d] tensor.
         Returns dict(slot_map, idx, cnt, O (float32 [n,H,d]), lse (float32 [H,n]))."""
         torch, uf, w = self.torch, self.uf, self.w
         n, H, d = Qb.shape
-        q, k, v = self.to_dev(Qb), self.to_dev(Kb), self.to_dev(Vb)
-        ts, hs = H * d, d
+        if fused_qkv:
+            qkv = self.to_dev(np.ascontiguousarray(np.stack([Qb, Kb, Vb], axis=1)))      # [n, 3, H, d]
+            q, k, v = qkv[:, 0], qkv[:, 1], qkv[:, 2]
+            ts, hs = 3 * H * d, d
+        else:
+            q, k, v = self.to_dev(Qb), self.to_dev(Kb), self.to_dev(Vb)
+            ts, hs = H * d, d
         uf.uf_kv_append(self.ctx, k, v, n, ts, hs, window, self.stream)
         slot_map = uf.uf_get_slot_map(self.ctx, w.capacity_chunks)
         n_cand, k_eff = uf.uf_query_topk(self.ctx, topk_count, topk_percent)
@@ -56,10 +64,23 @@ class CudaStream:
         idx = torch.full((H, nqb, max(k_eff, 1)), -1, dtype=torch.int32, device=self.dev)
         cnt = torch.full((H, nqb), -1, dtype=torch.int32, device=self.dev)
         uf.uf_select_blocks(self.ctx, q, n, ts, hs, topk_count, topk_percent, idx, cnt, self.stream)
-        o = torch.full((n, H, d), float("nan"), dtype=torch.bfloat16, device=self.dev)
+        if fused_qkv:
+            o2 = torch.full((n, 2, H, d), float("nan"), dtype=torch.bfloat16, device=self.dev)
+            o = o2[:, 1]
+        else:
+            o = torch.full((n, H, d), float("nan"), dtype=torch.bfloat16, device=self.dev)
         lse = torch.full((H, n), float("nan"), dtype=torch.float32, device=self.dev) if want_lse else None
         uf.uf_set_attn_impl(self.ctx, impl)
-        uf.uf_sparse_attn_fwd(self.ctx, q, o, lse, n, ts, hs, scale, self.stream)
+        if fused_qkv:
+            # attention takes one token stride for Q and O: O's [n, 2, H, d] slice has stride 2*H*d, so Q is
+            # re-packed to that stride too (Q of the select call above kept the fused layout)
+            q2 = torch.empty((n, 2, H, d), dtype=torch.bfloat16, device=self.dev)
+            q2[:, 0] = q
+            uf.uf_sparse_attn_fwd(self.ctx, q2[:, 0], o, lse, n, 2 * H * d, hs, scale, self.stream)
+            torch.cuda.synchronize(self.dev)
+            assert torch.isnan(o2[:, 0].float()).all(), "attention wrote outside its O slice"
+        else:
+            uf.uf_sparse_attn_fwd(self.ctx, q, o, lse, n, ts, hs, scale, self.stream)
         torch.cuda.synchronize(self.dev)
         return {
             "slot_map": slot_map, "n_cand": n_cand, "k_eff": k_eff,
@@ -96,7 +117,15 @@ def oracle_step(orc: UFOracle, Qb, Kb, Vb, topk_count=-1, topk_percent=-1, windo
     return out
 
 
-def compare_step(got: dict, ref: dict, where: str = ""):
+def sharp_o_max_abs(v_abs_max: float) -> float:
+    """Max-abs bound on O for tests that sharpen the softmax beyond the 1/sqrt(d) of the BASELINE.json workloads
+    (DESIGN.md section 6): the row sum adds the unrounded fp32 probabilities while the P V MMA multiplies their bf16
+    roundings, so a (nearly) one-hot row carries the relative rounding error of its one probability, <= 2^-8, times
+    |v|, on top of the bf16 rounding of the output, <= 2^-8 |O| <= 2^-8 max|V|."""
+    return max(O_MAX_ABS, 2.0 ** -7 * v_abs_max)
+
+
+def compare_step(got: dict, ref: dict, where: str = "", o_max_abs: float = O_MAX_ABS):
     """Bit-exact slot map / indices / counts; O and LSE within tolerance on the rows the oracle computed."""
     assert got["slot_map"] == ref["slot_map"], f"{where} slot map {got['slot_map']} != {ref['slot_map']}"
     assert got["cnt"].shape == ref["cnt"].shape and np.array_equal(got["cnt"], ref["cnt"]), f"{where} counts differ"
@@ -110,7 +139,7 @@ def compare_step(got: dict, ref: dict, where: str = ""):
         assert mask.any()
         assert not np.isnan(got["O"][mask]).any(), f"{where} CUDA output has NaN / unwritten rows"
         err = np.abs(got["O"].astype(np.float64)[mask] - ref["O"][mask])
-        assert err.max() <= O_MAX_ABS, f"{where} O max-abs {err.max():.3e} > {O_MAX_ABS}"
+        assert err.max() <= o_max_abs, f"{where} O max-abs {err.max():.3e} > {o_max_abs:.3e}"
         assert err.mean() <= O_MEAN_ABS, f"{where} O mean-abs {err.mean():.3e} > {O_MEAN_ABS}"
         if got.get("lse") is not None:
             lm = ~np.isnan(ref["lse"])
