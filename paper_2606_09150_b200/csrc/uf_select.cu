@@ -148,12 +148,14 @@ uf_score_topk_kernel(UfView v, const double* __restrict__ qbar, const double* __
   }
 }
 
-// ---- merge the lists of query blocks (2p, 2p+1) into one ascending union with tile masks ----------
+// ---- merge the lists of query blocks (2p, 2p+1) into one union list with tile masks -----------------
 // One warp per (h, pair).  Both lists are subsets of CAND; sel_rank holds the candidate index of every kept
-// entry, so each list becomes a bitmap over the candidates in shared memory, the union is the OR of the two,
-// an entry's position is the number of union bits below it (word popcounts + a warp scan), and its payload
-// (physical block, valid rows) is recomputed from the candidate index.  Bit 0 of the mask = tile 0 (block 2p)
-// attends the entry, bit 1 = tile 1 (block 2p+1).  dynamic smem: uint32 [warps][2][ceil(n_cand / 32)]
+// entry, so each list becomes a bitmap over the candidates in shared memory.  Output order (the attention
+// kernel's softmax does not depend on it): first the entries BOTH tiles attend (mask 3), then the entries only
+// one tile attends, alternating tile 0 / tile 1 (mask 1, 2, 1, 2, ...), so that while one tile's softmax runs the
+// tensor pipe has the other tile's MMAs (two single-tile steps of the same tile in a row would serialise).
+// An entry's position is its rank within its class (word popcounts + a warp scan); its payload (physical
+// block, valid rows) is recomputed from the candidate index.  dynamic smem: uint32 [warps][2][ceil(n_cand / 32)]
 constexpr int kMergeWarps = 4;
 __global__ void __launch_bounds__(kMergeWarps * 32)
 uf_pair_merge_kernel(UfView v, const int32_t* __restrict__ sel_rank, int32_t* __restrict__ sel_pair,
@@ -182,31 +184,47 @@ uf_pair_merge_kernel(UfView v, const int32_t* __restrict__ sel_rank, int32_t* __
     }
   }
   __syncwarp();
+  // class sizes: both, only tile 0, only tile 1
+  int n3 = 0, n1 = 0, n2 = 0;
+  for (int w = lane; w < nw; w += 32) {
+    const uint32_t wa = bma[w], wb = bmb[w];
+    n3 += __popc(wa & wb); n1 += __popc(wa & ~wb); n2 += __popc(wb & ~wa);
+  }
+  n3 = __reduce_add_sync(0xffffffffu, n3);
+  n1 = __reduce_add_sync(0xffffffffu, n1);
+  n2 = __reduce_add_sync(0xffffffffu, n2);
   int32_t* out = sel_pair + ((int64_t)h * NP + p) * 2 * kcap;
-  int base = 0;
+  int base3 = 0, base1 = 0, base2 = 0;                 // entries of each class in the words before this round
   for (int w0 = 0; w0 < nw; w0 += 32) {
     const int w = w0 + lane;
     const uint32_t wa = w < nw ? bma[w] : 0u, wb = w < nw ? bmb[w] : 0u;
-    uint32_t u = wa | wb;
-    const int cnt = __popc(u);
-    int incl = cnt;
+    const int c3 = __popc(wa & wb), c1 = __popc(wa & ~wb), c2 = __popc(wb & ~wa);
+    int i3 = c3, i1 = c1, i2 = c2;                      // inclusive warp scans
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
-      const int y = __shfl_up_sync(0xffffffffu, incl, o);
-      if (lane >= o) incl += y;
+      const int y3 = __shfl_up_sync(0xffffffffu, i3, o), y1 = __shfl_up_sync(0xffffffffu, i1, o),
+                y2 = __shfl_up_sync(0xffffffffu, i2, o);
+      if (lane >= o) { i3 += y3; i1 += y1; i2 += y2; }
     }
-    int pos = base + incl - cnt;
+    int r3 = base3 + i3 - c3, r1 = base1 + i1 - c1, r2 = base2 + i2 - c2;   // rank within the class
+    uint32_t u = wa | wb;
     while (u) {
       const int b = __ffs(u) - 1;
       u &= u - 1;
       int gid, phys, nval;
       uf_cand_lookup(v, w * 32 + b, &gid, &phys, &nval);
       const int mask = ((wa >> b) & 1u) | (((wb >> b) & 1u) << 1);
-      out[pos++] = uf_entry_pack(phys, nval, mask);
+      int pos;
+      if (mask == 3)      { pos = r3; ++r3; }
+      else if (mask == 1) { pos = n3 + r1 + min(r1, n2); ++r1; }            // a_i at 2i while b_i exists
+      else                { pos = n3 + r2 + min(r2 + 1, n1); ++r2; }        // b_i at 2i + 1 while a_i exists
+      out[pos] = uf_entry_pack(phys, nval, mask);
     }
-    base += __shfl_sync(0xffffffffu, incl, 31);
+    base3 += __shfl_sync(0xffffffffu, i3, 31);
+    base1 += __shfl_sync(0xffffffffu, i1, 31);
+    base2 += __shfl_sync(0xffffffffu, i2, 31);
   }
-  if (lane == 0) pair_cnt[(int64_t)h * NP + p] = base;
+  if (lane == 0) pair_cnt[(int64_t)h * NP + p] = n3 + n1 + n2;
 }
 
 }  // namespace
