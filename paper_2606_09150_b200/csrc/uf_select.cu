@@ -104,26 +104,45 @@ uf_score_topk_kernel(UfView v, const double* __restrict__ qbar, const double* __
   }
   __syncthreads();
 
-  // Exact top-k', one warp per query block.  T = the k'-th largest key, found bit by bit from the top
-  // (T is the largest value with #{key >= T} >= k').  Kept: every key > T, and of the keys == T the first
+  // Exact top-k', one warp per query block.  T = a threshold with #{key > T} < k' <= #{key >= T}, found bit by
+  // bit from the top (the largest value with #{key >= T} >= k').  Kept: every key > T, and of the keys == T the first
   // (k' - #{key > T}) in candidate order, i.e. ties go to the lower global id (R-12).  Candidates are in
   // ascending global id, so the ordered ballot compaction below emits ascending ids.
   const int lane = tid & 31, wid = tid >> 5;
   for (int g = wid; g < ng; g += kScoreThreads / 32) {
     const unsigned long long* kg = key + (int64_t)g * nc;
     const int i = i0 + g;
-    unsigned long long T = 0ull;
-    for (int b = 63; b >= 0; --b) {
-      const unsigned long long cand = T | (1ull << b);
+    // high words first (32 rounds on 32-bit values); the low words only matter if more keys share the high word
+    // of the k'-th than may be kept (scores that agree to ~2^-20 relative: rare)
+    const uint32_t* kw = reinterpret_cast<const uint32_t*>(kg);      // little endian: [2j] low, [2j + 1] high
+    uint32_t Th = 0u;
+    for (int b = 31; b >= 0; --b) {
+      const uint32_t cand = Th | (1u << b);
       int cnt = 0;
-      for (int j = lane; j < nc; j += 32) cnt += (kg[j] >= cand);
+      for (int j = lane; j < nc; j += 32) cnt += (kw[2 * j + 1] >= cand);
       cnt = __reduce_add_sync(0xffffffffu, cnt);
-      if (cnt >= k_eff) T = cand;
+      if (cnt >= k_eff) Th = cand;
     }
+    int c_gt = 0, c_eq = 0;
+    for (int j = lane; j < nc; j += 32) { const uint32_t hw = kw[2 * j + 1]; c_gt += (hw > Th); c_eq += (hw == Th); }
+    c_gt = __reduce_add_sync(0xffffffffu, c_gt);
+    c_eq = __reduce_add_sync(0xffffffffu, c_eq);
+    uint32_t Tl = 0u;                                 // c_gt + c_eq == k': every key with that high word is kept
+    if (c_gt + c_eq > k_eff) {
+      const int need = k_eff - c_gt;                  // of the keys with high word Th keep the `need` largest
+      for (int b = 31; b >= 0; --b) {
+        const uint32_t cand = Tl | (1u << b);
+        int cnt = 0;
+        for (int j = lane; j < nc; j += 32) cnt += (kw[2 * j + 1] == Th && kw[2 * j] >= cand);
+        cnt = __reduce_add_sync(0xffffffffu, cnt);
+        if (cnt >= need) Tl = cand;
+      }
+    }
+    const unsigned long long T = ((unsigned long long)Th << 32) | Tl;
     int n_gt = 0;
     for (int j = lane; j < nc; j += 32) n_gt += (kg[j] > T);
     n_gt = __reduce_add_sync(0xffffffffu, n_gt);
-    const int need_eq = k_eff - n_gt;                  // >= 1 by the definition of T
+    const int need_eq = k_eff - n_gt;                  // keys == T still to keep (lowest candidate index first)
     int pos0 = 0, eq_seen = 0;
     const int64_t rowq = ((int64_t)h * v.BPC + i) * kcap;
     for (int j0 = 0; j0 < nc; j0 += 32) {
