@@ -313,7 +313,7 @@ def call_breakdown(hp: HotPath, steps: int, hbm_gbs: float):
                    "frac_of_hbm_peak": app_bytes / app / 1e6 / hbm_gbs},
         "select": {"ms": sel, "algorithmic_bytes": sel_bytes, "achieved_gbs": sel_bytes / sel / 1e6,
                    "frac_of_hbm_peak": sel_bytes / sel / 1e6 / hbm_gbs,
-                   "note": "3 kernels: pool Q (HBM-bound), fp64 score + exact rank top-k (ALU-bound), pair merge"},
+                   "note": "3 kernels: pool Q (HBM-bound), fp64 score + exact threshold-search top-k (latency/ALU-bound), pair merge"},
         "attention": {"ms": att},
         "hbm_peak_gbs": hbm_gbs,
     }
