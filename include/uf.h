@@ -118,7 +118,13 @@ int32_t uf_select_blocks(uf_ctx* ctx, const void* q, int32_t n_tokens,
  *   lse         device pointer or NULL: fp32 [H, n_tokens], natural-log sum-exp of the scaled logits
  *   softmax_scale  0 -> 1/sqrt(d)
  * Kernels: B == 128 && d == 128 -> TMA + tcgen05/TMEM kernel; other shapes -> the generic CUDA-core
- * kernel.  uf_set_attn_impl can force the generic kernel (cross-checks). */
+ * kernel.  uf_set_attn_impl can force the generic kernel (cross-checks).  The tcgen05 path enqueues two
+ * launches: the fast kernel (exponentials against the running max of the earlier key blocks) and an
+ * exact-max instantiation that redoes the work items in which a row max outgrew that reference by 2^100
+ * or more inside one key block (normally none: it returns at once; uf_attn_redone_items reports them).
+ * Asynchronous on `stream`; needs softmax_scale >= 0 and finite (else UF_ERR_INVALID_ARG), a preceding
+ * uf_select_blocks for the same chunk (else UF_ERR_STATE) and, on the tcgen05 path, 16-byte-aligned q / o
+ * with strides that are multiples of 8 elements (TMA; else UF_ERR_INVALID_ARG). */
 int32_t uf_sparse_attn_fwd(uf_ctx* ctx, const void* q, void* o, float* lse, int32_t n_tokens,
                            int64_t tok_stride, int64_t head_stride, float softmax_scale,
                            void* stream);
