@@ -93,11 +93,16 @@ uf_score_topk_kernel(UfView v, const double* __restrict__ qbar, const double* __
     double acc[kQG];
 #pragma unroll
     for (int g = 0; g < kQG; ++g) acc[g] = 0.0;
-#pragma unroll 16
-    for (int t = 0; t < D; ++t) {
-      const double kv = kp[(int64_t)t * v.P];
+    // 16 pooled-K loads in flight at a time; the additions stay in index order (R-4)
+    for (int t0 = 0; t0 < D; t0 += 16) {
+      double kv[16];
 #pragma unroll
-      for (int g = 0; g < kQG; ++g) acc[g] = __dadd_rn(acc[g], __dmul_rn(qs[g * D + t], kv));
+      for (int u = 0; u < 16; ++u) kv[u] = __ldg(kp + (int64_t)(t0 + u) * v.P);
+#pragma unroll
+      for (int u = 0; u < 16; ++u) {
+#pragma unroll
+        for (int g = 0; g < kQG; ++g) acc[g] = __dadd_rn(acc[g], __dmul_rn(qs[g * D + t0 + u], kv[u]));
+      }
     }
 #pragma unroll
     for (int g = 0; g < kQG; ++g) key[(int64_t)g * nc + j] = sortable(__ddiv_rn(acc[g], inv) + 0.0);
