@@ -33,7 +33,7 @@ import uf_workloads as wl  # noqa: E402
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE uf_attn_sm100_kernel<false> launch, from the committed
 # `ncu --set full` capture of this command (profiles/r1e_ncu_full_all_kernels.txt, command in profiles/README.md);
 # null for workloads not captured.
-NCU_ATTN_DRAM_BYTES = {"1k": 464.973312e6 + 66.604800e6}
+NCU_ATTN_DRAM_BYTES = {"1k": 476.457984e6 + 66.498048e6}
 
 METRIC = "effective TFLOP/s on kept blocks, sparse causal chunk attention step (ms/chunk in ms_per_step)"
 UNIT = "TFLOP/s"
