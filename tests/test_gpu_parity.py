@@ -229,6 +229,45 @@ def test_randomised_streams(seed):
         cu.close()
 
 
+def test_reset_starts_a_new_stream_and_two_ctx_interleave():
+    """uf_ctx_reset empties the cache (a new video starts at chunk 0: sink rewritten, no candidates), and two
+    contexts (two layers / two streams) driven in turn on their own CUDA streams do not disturb each other."""
+    import torch
+    w = wl.scaled(wl.CONFIGS["1k"], "reset128", n_heads=2, frames_per_chunk=1, grid_h=18, grid_w=25,
+                  capacity_chunks=2, topk_percent=50)
+    cu_a, cu_b = hz.CudaStream(w), hz.CudaStream(w)
+    cu_b.stream = torch.cuda.Stream(cu_b.dev)
+    orc_a, orc_b = hz.make_oracle(w), hz.make_oracle(w)
+    try:
+        # stream A sees chunks 0, 1, 2; stream B sees the same recipe with other seeds, interleaved with A
+        for c in range(3):
+            Qa, Ka, Va = wl.make_chunk(w, c)
+            Qb, Kb, Vb = wl.make_chunk(w, c, seed=100 + c)
+            with torch.cuda.stream(cu_b.stream):
+                got_b = cu_b.step(Qb, Kb, Vb, topk_percent=50)
+            got_a = cu_a.step(Qa, Ka, Va, topk_percent=50)
+            hz.compare_step(got_a, hz.oracle_step(orc_a, Qa, Ka, Va, topk_percent=50), f"[ctx A chunk {c}]")
+            hz.compare_step(got_b, hz.oracle_step(orc_b, Qb, Kb, Vb, topk_percent=50), f"[ctx B chunk {c}]")
+        # reset A: the next chunk is chunk 0 of a new video (fresh oracle), B carries on untouched
+        cu_a.uf.uf_ctx_reset(cu_a.ctx, cu_a.stream)
+        orc_a = hz.make_oracle(w)
+        for c in range(2):
+            Qa, Ka, Va = wl.make_chunk(w, c, seed=200 + c)
+            got_a = cu_a.step(Qa, Ka, Va, topk_percent=50)
+            ref_a = hz.oracle_step(orc_a, Qa, Ka, Va, topk_percent=50)
+            hz.compare_step(got_a, ref_a, f"[ctx A after reset chunk {c}]")
+            assert got_a["n_cand"] == (0 if c == 0 else w.bpc - w.sink_blocks)
+        Qb, Kb, Vb = wl.make_chunk(w, 3, seed=103)
+        with torch.cuda.stream(cu_b.stream):
+            got_b = cu_b.step(Qb, Kb, Vb, topk_percent=50)
+        hz.compare_step(got_b, hz.oracle_step(orc_b, Qb, Kb, Vb, topk_percent=50), "[ctx B chunk 3]")
+        _check_cache(cu_a, orc_a, w)
+        _check_cache(cu_b, orc_b, w)
+    finally:
+        cu_a.close()
+        cu_b.close()
+
+
 def test_error_codes_and_call_order():
     import torch
     import paper_2606_09150_b200 as uf
