@@ -33,7 +33,8 @@ import uf_workloads as wl  # noqa: E402
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE uf_attn_sm100_kernel<false> launch, from the committed
 # `ncu --set full` capture of this command (profiles/r1e_ncu_full_all_kernels.txt, command in profiles/README.md);
 # null for workloads not captured.
-NCU_ATTN_DRAM_BYTES = {"1k": 476.457984e6 + 66.498048e6}
+NCU_ATTN_DRAM_BYTES = {"1k": 476.457984e6 + 66.498048e6,      # profiles/r1e_ncu_full_all_kernels.txt
+                       "2k": 1.735499e9 + 131.152896e6}        # profiles/r1e_2k_attn_sm100_ncu_full.txt
 
 METRIC = "effective TFLOP/s on kept blocks, sparse causal chunk attention step (ms/chunk in ms_per_step)"
 UNIT = "TFLOP/s"
@@ -497,6 +498,10 @@ def main():
                                "kept_tflop_per_step": m2["flop"] / 1e12,
                                "value": m2["flop"] / (m2["total_ms"] / max(3, args.steps // 2) * 1e-3) / 1e12,
                                "attn_tflops": t2, "attn_frac_of_burst_peak": t2 / peaks["bf16_burst"],
+                               "roofline": {"kernel": "uf_attn_sm100_kernel", "bound": "tensor", "achieved": t2,
+                                            "peak": peaks["bf16_burst"], "unit": "TFLOP/s", "frac": t2 / peaks["bf16_burst"],
+                                            "traffic": NCU_ATTN_DRAM_BYTES.get("2k"),
+                                            "algorithmic_flop_per_launch": m2["flop"]},
                                "k_eff": m2["k_eff"], "n_cand": m2["n_cand"], "clocks": m2["clocks"]}}
     if "stream" in m:
         line["stream"] = m["stream"]
