@@ -73,8 +73,9 @@ int32_t uf_ctx_create(const uf_config* cfg, uf_ctx** out);
 /* Free everything the ctx owns.  NULL is accepted. */
 int32_t uf_ctx_destroy(uf_ctx* ctx);
 
-/* Start a new video stream: empty cache, no sink, chunk counter back to 0 (R-27).  Re-zeroes the
- * caches on `stream`. */
+/* Start a new video stream: empty cache, no sink, chunk counter back to 0 (R-27).  Host state only:
+ * nothing on the device is cleared (every block an append makes addressable is rewritten in full, pad
+ * rows as zeros; blocks that are not addressable are never read); `stream` is unused. */
 int32_t uf_ctx_reset(uf_ctx* ctx, void* stream);
 
 /* Step a1 — KV append + evict (P:136 (iii) "dynamically selecting a compact cache window",
@@ -86,6 +87,7 @@ int32_t uf_ctx_reset(uf_ctx* ctx, void* stream);
  * block-mean pooled K of the chunk's blocks, used by uf_select_blocks.
  *   k, v        device pointers, bf16 [n_tokens, H, d] with the given element strides
  *   n_tokens    1..chunk_tokens_max
+ * If the device work cannot be enqueued (UF_ERR_CUDA) the ctx is left exactly as before the call.
  * With a host-only ctx (device == -1) k, v, stream are ignored and only the slot map advances. */
 int32_t uf_kv_append(uf_ctx* ctx, const void* k, const void* v, int32_t n_tokens,
                      int64_t tok_stride, int64_t head_stride, int32_t window_chunks, void* stream);
@@ -101,7 +103,10 @@ int32_t uf_query_topk(const uf_ctx* ctx, int32_t topk_count, int32_t topk_percen
 /* Steps a2-a4 — block pooling, scoring (Eq. 4: s_ij^h = qbar_i^h . kbar_j^h / sqrt(d_h), fp64,
  * terms added in index order, no fused multiply-add, R-4) and top-k per (head, query block); equal
  * scores -> the smaller global id wins (BJ); lists ascending by global id.  The selection is kept
- * in the ctx for the following uf_sparse_attn_fwd.
+ * in the ctx for the following uf_sparse_attn_fwd.  The score is a fixed function of the input bits as long
+ * as the block sums are exact in fp64, i.e. the bf16 values of one (block, head, channel) column span fewer
+ * than 2^38 between the largest magnitude and the smallest non-zero ulp (8 + 7 + 38 = 53 bits); beyond that
+ * the summation order may change the last bit of a pooled mean.
  *   q           device pointer, bf16 [n_tokens, H, d]; n_tokens must equal the last append's
  *   idx_out     device pointer or NULL: int32 [H, ceil(n_tokens/B), k'] global block ids
  *   cnt_out     device pointer or NULL: int32 [H, ceil(n_tokens/B)] (= k' for every row)     */
@@ -117,8 +122,11 @@ int32_t uf_select_blocks(uf_ctx* ctx, const void* q, int32_t n_tokens,
  *   q, o        device pointers, bf16 [n_tokens, H, d] (same strides for both)
  *   lse         device pointer or NULL: fp32 [H, n_tokens], natural-log sum-exp of the scaled logits
  *   softmax_scale  0 -> 1/sqrt(d)
- * Kernels: B == 128 && d == 128 -> TMA + tcgen05/TMEM kernel; other shapes -> the generic CUDA-core
- * kernel.  uf_set_attn_impl can force the generic kernel (cross-checks).  The tcgen05 path enqueues two
+ *               o must not overlap q (UF_ERR_INVALID_ARG); disjoint slices of one fused tensor are fine
+ * Kernels: B == 128 && d == 128 -> TMA + tcgen05/TMEM kernel.  Other shapes have only the CUDA-core kernel
+ * (one warp per query row, orders of magnitude slower): the call returns UF_ERR_UNSUPPORTED unless the caller
+ * opted in with uf_set_attn_impl(ctx, 1), which also forces that kernel for B == d == 128 (cross-checks).
+ * The tcgen05 path enqueues two
  * launches: the fast kernel (exponentials against the running max of the earlier key blocks) and an
  * exact-max instantiation that redoes the work items in which a row max outgrew that reference by 2^100
  * or more inside one key block (normally none: it returns at once; uf_attn_redone_items reports them).
@@ -129,7 +137,8 @@ int32_t uf_sparse_attn_fwd(uf_ctx* ctx, const void* q, void* o, float* lse, int3
                            int64_t tok_stride, int64_t head_stride, float softmax_scale,
                            void* stream);
 
-/* impl: 0 = automatic (default), 1 = force the generic CUDA-core attention kernel. */
+/* impl: 0 = tcgen05 kernel only (default; shapes it does not cover -> UF_ERR_UNSUPPORTED),
+ *       1 = the generic CUDA-core attention kernel (any supported shape; slow). */
 int32_t uf_set_attn_impl(uf_ctx* ctx, int32_t impl);
 
 /* Observability (host outputs).

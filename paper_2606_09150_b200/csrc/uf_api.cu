@@ -189,14 +189,11 @@ int32_t uf_ctx_destroy(uf_ctx* c) {
 
 int32_t uf_ctx_reset(uf_ctx* c, void* stream) {
   if (!c) return UF_ERR_INVALID_ARG;
+  (void)stream;
+  // Host state only.  Nothing on the device has to be cleared: the append kernel rewrites every row (pad rows as
+  // zeros) of every block it makes addressable, the sink region and the pooled-K entries included, and a block
+  // that is not addressable through the slot map / sink count is never read.
   clear_host_state(c);
-  if (c->host_only) return UF_OK;
-  UF_CUDA(c, cudaSetDevice(c->cfg.device));
-  cudaStream_t s = (cudaStream_t)stream;
-  const int64_t H = c->cfg.n_heads, d = c->cfg.head_dim, B = c->cfg.block, P = c->P;
-  UF_CUDA(c, cudaMemsetAsync(c->kc, 0, (size_t)(H * P * B * d * 2), s));
-  UF_CUDA(c, cudaMemsetAsync(c->vc, 0, (size_t)(H * P * B * d * 2), s));
-  UF_CUDA(c, cudaMemsetAsync(c->kpool, 0, (size_t)(H * d * P * 8), s));
   return UF_OK;
 }
 
@@ -213,34 +210,52 @@ int32_t uf_kv_append(uf_ctx* c, const void* k, const void* v, int32_t n_tokens,
     r = check_tensor_args(c, v, tok_stride, head_stride, "uf_kv_append v");
     if (r) return r;
   }
-  // --- cache policy (host, integers only) ---
+  // --- cache policy (host, integers only), computed on a copy of the slot state: it is committed only after
+  // the device work was enqueued, so a failing launch leaves the ctx as it was ---
   const int cid = c->next_chunk;
   const int W = window_chunks == 0 ? C : window_chunks;
+  int slot_chunk[UF_MAXC], slot_ntok[UF_MAXC];
+  for (int s = 0; s < UF_MAXC; ++s) { slot_chunk[s] = c->slot_chunk[s]; slot_ntok[s] = c->slot_ntok[s]; }
   for (;;) {   // evict ids <= cid - W, oldest first
     int oldest = -1;
     for (int s = 0; s < C; ++s)
-      if (c->slot_chunk[s] >= 0 && (oldest < 0 || c->slot_chunk[s] < c->slot_chunk[oldest])) oldest = s;
-    if (oldest < 0 || c->slot_chunk[oldest] > cid - W) break;
-    c->slot_chunk[oldest] = -1; c->slot_ntok[oldest] = 0;
+      if (slot_chunk[s] >= 0 && (oldest < 0 || slot_chunk[s] < slot_chunk[oldest])) oldest = s;
+    if (oldest < 0 || slot_chunk[oldest] > cid - W) break;
+    slot_chunk[oldest] = -1; slot_ntok[oldest] = 0;
   }
   int slot = -1;
-  for (int s = 0; s < C; ++s) if (c->slot_chunk[s] < 0) { slot = s; break; }   // lowest free slot
+  for (int s = 0; s < C; ++s) if (slot_chunk[s] < 0) { slot = s; break; }   // lowest free slot
   if (slot < 0) return fail(c, UF_ERR_STATE, "uf_kv_append: no free slot (internal)");
-  c->slot_chunk[slot] = cid; c->slot_ntok[slot] = n_tokens;
+  slot_chunk[slot] = cid; slot_ntok[slot] = n_tokens;
+  int sink_ntok = c->sink_ntok;
   if (cid == 0) {
     int ns = c->cfg.sink_blocks * c->cfg.block;
-    c->sink_ntok = ns < n_tokens ? ns : n_tokens;
+    sink_ntok = ns < n_tokens ? ns : n_tokens;
   }
-  c->next_chunk = cid + 1;
-  c->sel_valid = false;
+  struct Saved { int slot_chunk[UF_MAXC], slot_ntok[UF_MAXC], next_chunk, sink_ntok; bool sel_valid; } old;
+  for (int s = 0; s < UF_MAXC; ++s) { old.slot_chunk[s] = c->slot_chunk[s]; old.slot_ntok[s] = c->slot_ntok[s]; }
+  old.next_chunk = c->next_chunk; old.sink_ntok = c->sink_ntok; old.sel_valid = c->sel_valid;
+  auto commit = [&]() {
+    for (int s = 0; s < UF_MAXC; ++s) { c->slot_chunk[s] = slot_chunk[s]; c->slot_ntok[s] = slot_ntok[s]; }
+    c->sink_ntok = sink_ntok; c->next_chunk = cid + 1; c->sel_valid = false;
+  };
+  auto rollback = [&]() {
+    for (int s = 0; s < UF_MAXC; ++s) { c->slot_chunk[s] = old.slot_chunk[s]; c->slot_ntok[s] = old.slot_ntok[s]; }
+    c->sink_ntok = old.sink_ntok; c->next_chunk = old.next_chunk; c->sel_valid = old.sel_valid;
+  };
+  commit();
   if (c->host_only) return UF_OK;
   // --- device: copy + pooled K ---
-  UF_CUDA(c, cudaSetDevice(c->cfg.device));
+  cudaError_t e = cudaSetDevice(c->cfg.device);
   UfView view;
-  make_view(c, &view);
-  cudaError_t e = uf_launch_append(c, view, (const __nv_bfloat16*)k, (const __nv_bfloat16*)v,
-                                   tok_stride, head_stride, (cudaStream_t)stream);
-  if (e != cudaSuccess) return fail_cuda(c, e, "uf_kv_append kernel launch");
+  if (e == cudaSuccess && !make_view(c, &view)) { rollback(); return fail(c, UF_ERR_STATE, "uf_kv_append: inconsistent slot state (internal)"); }
+  if (e == cudaSuccess)
+    e = uf_launch_append(c, view, (const __nv_bfloat16*)k, (const __nv_bfloat16*)v, tok_stride, head_stride,
+                         (cudaStream_t)stream);
+  if (e != cudaSuccess) {
+    rollback();                       // the chunk was not written: the ctx still describes the previous state
+    return fail_cuda(c, e, "uf_kv_append kernel launch");
+  }
   return UF_OK;
 }
 
@@ -294,6 +309,32 @@ int32_t uf_sparse_attn_fwd(uf_ctx* c, const void* q, void* o, float* lse, int32_
   float scale = softmax_scale == 0.0f ? (float)(1.0 / std::sqrt((double)c->cfg.head_dim)) : softmax_scale;
   UF_CUDA(c, cudaSetDevice(c->cfg.device));
   const bool fast = (c->cfg.block == 128 && c->cfg.head_dim == 128 && c->attn_impl == 0 && c->tm_ok);
+  if (!fast && c->attn_impl == 0)
+    return fail(c, UF_ERR_UNSUPPORTED,
+                "uf_sparse_attn_fwd: the tcgen05 kernel needs block == 128 and head_dim == 128; other shapes only run "
+                "on the (slow) CUDA-core kernel after uf_set_attn_impl(ctx, 1)");
+  if (fast) {
+    // the exact-max kernel re-reads Q of the items it redoes after the fast kernel stored their O rows
+    const int64_t span = ((int64_t)(n_tokens - 1) * tok_stride + (int64_t)(c->cfg.n_heads - 1) * head_stride +
+                          c->cfg.head_dim) * 2;
+    const uintptr_t qa = (uintptr_t)q, oa = (uintptr_t)o;
+    if (qa < oa + (uintptr_t)span && oa < qa + (uintptr_t)span) {
+      // the address ranges interleave: fine when q and o are different slices of one fused tensor, i.e. when
+      // no (token, head) row of o can touch a row of q.  Offsets in elements, d = row length:
+      //   token level: a token's rows span E = (H-1)*head_stride + d elements; disjoint if the offset between
+      //                the bases, modulo tok_stride, leaves E free on both sides;
+      //   head level:  if tok_stride is a multiple of head_stride, every row of q starts at 0 mod head_stride
+      //                and every row of o at delta mod head_stride.
+      const int64_t d = c->cfg.head_dim;
+      const int64_t delta = (int64_t)(oa > qa ? oa - qa : qa - oa) / 2;
+      const int64_t E = (int64_t)(c->cfg.n_heads - 1) * head_stride + d;
+      const int64_t rt = delta % tok_stride, rh = delta % head_stride;
+      const bool tok_disjoint = rt >= E && tok_stride - rt >= E;
+      const bool head_disjoint = (tok_stride % head_stride == 0) && rh >= d && head_stride - rh >= d;
+      if (!tok_disjoint && !head_disjoint)
+        return fail(c, UF_ERR_INVALID_ARG, "uf_sparse_attn_fwd: o must not overlap q");
+    }
+  }
   c->last_attn_sm100 = fast;
   if (fast)
     return uf_launch_attn_sm100(c, v, (const __nv_bfloat16*)q, (__nv_bfloat16*)o, lse, tok_stride, head_stride,

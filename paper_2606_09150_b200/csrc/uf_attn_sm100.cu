@@ -41,9 +41,6 @@
 // tile attends it), then SINK, then CUR (both tiles).  All K/V come from the ctx cache.
 #include "uf_internal.h"
 
-#include <cstdio>
-#include <cstdlib>
-
 namespace {
 
 constexpr int kNK = 3;                 // K ring stages
@@ -263,20 +260,24 @@ __device__ __forceinline__ float max3(float a, float b, float c) {
 // 8 column pairs.  2^x = 2^floor(x) * 2^frac(x): floor via the round-down magic-number add (the integer
 // lands in the low mantissa bits), 2^frac by a degree-3 minimax polynomial on [0,1) (max relative error
 // 7.5e-5, far below the bf16 rounding of P), the exponent added into the float's bits by one LEA.
-// Valid for x >= -126 (clamped: the polynomial can return 1 - 7.5e-5, i.e. exponent field 126) and x < 128
-// (larger x means the row max grew by more than 2^100: the panic path).
-#ifndef UF_EMU_PAIRS
-#define UF_EMU_PAIRS 3
-#endif
-constexpr int kEmuPairs = UF_EMU_PAIRS;
+// x is clamped to [-126, 126] by ONE instruction (min.xorsign.abs -> FMNMX.XORSIGN): below, because the
+// polynomial can return 1 - 7.5e-5 (exponent field 126, so floor(x) = -127 would wrap); above, because for
+// x >= 129 the exponent add would wrap into the sign bit and silently return a small or negative number.
+// A clamped 2^126 makes the row sum >= 2^100, so the item takes the panic path (redo with the exact max).
+constexpr int kEmuPairs = 3;
 __device__ __forceinline__ constexpr bool pair_emulated(int j) { return ((j & 7) * kEmuPairs) % 8 < kEmuPairs; }
 
+__device__ __forceinline__ float clamp126(float x) {       // sign(x) * min(|x|, 126)
+  float y;
+  asm("min.xorsign.abs.f32 %0, %1, %2;" : "=f"(y) : "f"(x), "f"(126.0f));
+  return y;
+}
 __device__ __forceinline__ uint64_t ex2_pair(uint64_t x, bool emulate) {
   float x0, x1;
   unpack2(x, x0, x1);
   if (!emulate) return pack2(ex2(x0), ex2(x1));
   const uint64_t magic = pack2(12582912.0f, 12582912.0f);            // 2^23 + 2^22
-  x = pack2(fmaxf(x0, -126.0f), fmaxf(x1, -126.0f));
+  x = pack2(clamp126(x0), clamp126(x1));
   const uint64_t r = add2_rm(x, magic);
   const uint64_t fr = sub2(x, sub2(r, magic));
   uint64_t p = fma2(fr, pack2(0.07802452147006989f, 0.07802452147006989f), pack2(0.22606715559959412f, 0.22606715559959412f));
@@ -291,7 +292,10 @@ __device__ __forceinline__ uint64_t ex2_pair(uint64_t x, bool emulate) {
 }
 
 // One 32-column chunk of a softmax pass: p = 2^(s*sl2 - m) as bf16 pairs into pk[] and fp32 row sums into
-// the two packed accumulators.  `chunk` (0..3, position in the 128-key block) selects which column pairs
+// the two packed accumulators.  The row sum adds the bf16-ROUNDED probabilities, the very numbers the P V MMA
+// multiplies, so O = sum(P~ v) / sum(P~) is a consistent weighted mean whatever the rounding of P~ (a one-hot
+// row returns its V row exactly; with the unrounded sum it carried the 2^-8 relative rounding error of its
+// single probability, which is not 1 under a stale reference max).  `chunk` (0..3, position in the 128-key block) selects which column pairs
 // take the polynomial (unused: the pattern has period 8 pairs); `nvalid_left` < 32 masks the tail of a ragged key block (R-3).
 __device__ __forceinline__ void exp_chunk(uint32_t (&s)[32], uint32_t (&pk)[16], int chunk, int nvalid_left,
                                           uint64_t sl22, uint64_t nm2, uint64_t& acc0, uint64_t& acc1) {
@@ -305,10 +309,22 @@ __device__ __forceinline__ void exp_chunk(uint32_t (&s)[32], uint32_t (&pk)[16],
     const int j = (u >> 1);                               // pattern repeats every 8 pairs
     const uint64_t x = fma2(pack2(__uint_as_float(s[u]), __uint_as_float(s[u + 1])), sl22, nm2);
     const uint64_t p = ex2_pair(x, pair_emulated(j));
-    if (j & 1) acc1 = add2(acc1, p); else acc0 = add2(acc0, p);
     float p0, p1;
     unpack2(p, p0, p1);
-    pk[u >> 1] = pack_bf16x2(p0, p1);
+    const uint32_t w = pack_bf16x2(p0, p1);
+    pk[u >> 1] = w;
+    // add.rn.f32.bf16 (FHADD.BF16 with a half-register select): fp32 accumulator += one bf16 half of w, one
+    // instruction per element and no unpacking (measured against widening with shift / mask + packed add)
+    {
+      float a0, a1;
+      uint64_t& acc = (j & 1) ? acc1 : acc0;
+      unpack2(acc, a0, a1);
+      unsigned short lo, hi;
+      asm("mov.b32 {%0, %1}, %2;" : "=h"(lo), "=h"(hi) : "r"(w));
+      asm("add.rn.f32.bf16 %0, %1, %0;" : "+f"(a0) : "h"(lo));
+      asm("add.rn.f32.bf16 %0, %1, %0;" : "+f"(a1) : "h"(hi));
+      acc = pack2(a0, a1);
+    }
   }
 }
 
@@ -321,15 +337,6 @@ __device__ __forceinline__ uint32_t bf16_bits_up(float x) {
 // instruction descriptor kind::f16: D fp32, A/B bf16, M = N = 128; B MN-major for P V
 constexpr uint32_t kIdescQK = (1u << 4) | (1u << 7) | (1u << 10) | ((128u >> 3) << 17) | ((128u >> 4) << 24);
 constexpr uint32_t kIdescPV = kIdescQK | (1u << 16);
-
-#ifdef UF_DBG_TRACE
-// debug only: clock64 timestamps of CTA 0's first kTraceSteps steps; roles: 0 = MMA warp, 1 / 2 = softmax tile 0 / 1
-constexpr int kTraceSteps = 600;
-__device__ long long uf_trace[3][kTraceSteps][8];
-#define UF_TR(role, step, slot) do { if (blockIdx.x == 0 && (int)(step) < kTraceSteps) uf_trace[role][step][slot] = clock64(); } while (0)
-#else
-#define UF_TR(role, step, slot) do { } while (0)
-#endif
 
 struct AttnParams {
   const int32_t* sel_pair;   // [H][NP][2*kcap]
@@ -461,15 +468,12 @@ uf_attn_sm100_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_cons
       static_assert(kNV == 2, "vrem0/vrem1 below assume a 2-stage V ring");
       uint32_t ks = 0, kph = 0, vs = 0, vph = 0, qph0 = 0, qph1 = 0, pph0 = 0, pph1 = 0;
       int vrem0 = 0, vrem1 = 0;                      // tiles that still have to consume V stage 0 / 1
-      int trc = 0; (void)trc;                        // UF_DBG_TRACE step counter
       bool pend[2] = {false, false}, first_pv[2] = {true, true};
       uint32_t pend_vs[2] = {0, 0}, pend_vph[2] = {0, 0};
 
       auto do_pv = [&](int t) {
         uint32_t& pph = t ? pph1 : pph0;
-        UF_TR(0, trc, t * 2);
         mbar_wait(bars + (P_FULL0 + t) * 8, pph);
-        UF_TR(0, trc, t * 2 + 1);
         pph ^= 1;
         const uint32_t pvs = pend_vs[t];
         mbar_wait(bars + (V_FULL0 + pvs) * 8, pend_vph[t]);
@@ -491,10 +495,8 @@ uf_attn_sm100_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_cons
       };
 
       auto step = [&](int m) {
-        UF_TR(0, trc, 6);
         mbar_wait(bars + (K_FULL0 + ks) * 8, kph);
         tc_fence_after();
-        UF_TR(0, trc, 4);
         const uint32_t k_lo = k_lo_base + ks * (kTile >> 4);
         int users = 0;
 #pragma unroll
@@ -515,8 +517,6 @@ uf_attn_sm100_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_cons
           ++users;
         }
         if (elect_one()) tc_commit(bars + (K_EMPTY0 + ks) * 8);
-        UF_TR(0, trc, 5);
-        ++trc;
         if (vs == 0) vrem0 = users; else vrem1 = users;
         if (++ks == kNK) { ks = 0; kph ^= 1; }
         if (++vs == kNV) { vs = 0; vph ^= 1; }
@@ -566,7 +566,6 @@ uf_attn_sm100_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_cons
     const uint64_t sl22 = pack2(sl2, sl2);
     volatile uint8_t* xc = reinterpret_cast<volatile uint8_t*>(base_ptr + kOffXc);     // [tile][half][row][parity]
     uint32_t sph0 = 0, sph1 = 0, oph0 = 0, oph1 = 0;
-    int trc = 0; (void)trc;                            // UF_DBG_TRACE step counter
 
     UF_ITEM_LOOP_BEGIN
       // per tile: reference max, partial row sum (this thread's keys), own published D, step parity
@@ -594,12 +593,9 @@ uf_attn_sm100_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_cons
             UF_TMEM_ST32(o_tmem + cc, ov, 0);
           }
         };
-
-        if (half == 0 && wq == 0 && lane == 0) UF_TR(1 + t, trc, 0);
         mbar_wait(bars + (S_FULL0 + t) * 8, sph);
         sph ^= 1;
         tc_fence_after();
-        if (half == 0 && wq == 0 && lane == 0) UF_TR(1 + t, trc, 1);
         uint32_t sa[32], sb[32], pk[16];
         const bool exact = kSafe || first;
         if (!kSafe && !first) {
@@ -685,8 +681,6 @@ uf_attn_sm100_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_cons
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(bars + (P_FULL0 + t) * 8);
-        if (half == 0 && wq == 0 && lane == 0) UF_TR(1 + t, trc, 2);
-        if (t == 1) ++trc;
       };
 
       // ---- the item's key blocks, in the MMA warp's order: per block tile 0 then tile 1 ----
@@ -796,6 +790,20 @@ bool encode_map(CUtensorMap* m, const void* ptr, uint64_t rows, uint64_t H, uint
             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+// Q / O maps are looked up in the ctx's small cache first (a tensor map is a pure function of the key)
+const CUtensorMap* cached_map(uf_ctx* c, const void* ptr, int rows, int H, int64_t tok_stride, int64_t head_stride) {
+  for (int i = 0; i < c->tm_cache_n; ++i) {
+    const uf_ctx::TmEntry& e = c->tm_cache[i];
+    if (e.ptr == ptr && e.rows == rows && e.tok_stride == tok_stride && e.head_stride == head_stride) return &e.map;
+  }
+  uf_ctx::TmEntry& e = c->tm_cache[c->tm_cache_next];
+  if (!encode_map(&e.map, ptr, rows, H, tok_stride, head_stride)) { e.ptr = nullptr; return nullptr; }
+  e.ptr = ptr; e.rows = rows; e.tok_stride = tok_stride; e.head_stride = head_stride;
+  c->tm_cache_next = (c->tm_cache_next + 1) % uf_ctx::kTmCache;
+  if (c->tm_cache_n < uf_ctx::kTmCache) ++c->tm_cache_n;
+  return &e.map;
+}
+
 }  // namespace
 
 int uf_sm100_make_cache_maps(uf_ctx* c) {
@@ -818,12 +826,13 @@ int uf_sm100_make_cache_maps(uf_ctx* c) {
 
 int uf_launch_attn_sm100(uf_ctx* c, const UfView& v, const __nv_bfloat16* q, __nv_bfloat16* o, float* lse,
                          int64_t tok_stride, int64_t head_stride, float scale, cudaStream_t s) {
-  CUtensorMap tm_q, tm_o;
-  if (!encode_map(&tm_q, q, v.cur_ntok, v.H, tok_stride, head_stride) ||
-      !encode_map(&tm_o, o, v.cur_ntok, v.H, tok_stride, head_stride)) {
+  const CUtensorMap* pq = cached_map(c, q, v.cur_ntok, v.H, tok_stride, head_stride);
+  const CUtensorMap* po = cached_map(c, o, v.cur_ntok, v.H, tok_stride, head_stride);
+  if (!pq || !po) {
     c->err = "cuTensorMapEncodeTiled failed for Q/O (check strides and alignment)";
     return UF_ERR_INVALID_ARG;
   }
+  const CUtensorMap tm_q = *pq, tm_o = *po;
   AttnParams a;
   a.sel_pair = c->sel_pair; a.pair_cnt = c->pair_cnt; a.lse = lse;
   a.H = v.H; a.NP = (v.BPC + 1) / 2; a.kcap = c->kcap;
@@ -839,14 +848,6 @@ int uf_launch_attn_sm100(uf_ctx* c, const UfView& v, const __nv_bfloat16* q, __n
   uf_attn_sm100_kernel<false><<<grid, kThreads, kSmemBytes, s>>>(tm_q, tm_o, c->tm_k, c->tm_v, a);
   uf_attn_sm100_kernel<true><<<grid, kThreads, kSmemBytes, s>>>(tm_q, tm_o, c->tm_k, c->tm_v, a);
   c->launches += 2;
-#ifdef UF_DBG_TRACE
-  if (const char* path = getenv("UF_TRACE_PATH")) {
-    cudaDeviceSynchronize();
-    static long long host[3][kTraceSteps][8];
-    cudaMemcpyFromSymbol(host, uf_trace, sizeof(host));
-    if (FILE* f = fopen(path, "wb")) { fwrite(host, 1, sizeof(host), f); fclose(f); }
-  }
-#endif
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) {
     c->err = std::string("uf_attn_sm100_kernel launch: ") + cudaGetErrorString(e);

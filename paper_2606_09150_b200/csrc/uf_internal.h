@@ -90,6 +90,13 @@ struct uf_ctx {
   int sm_count = 0;
   CUtensorMap tm_k, tm_v;         // K / V cache maps for the sm100 kernel (valid when B == d == 128)
   bool tm_ok = false;
+  // Q / O tensor maps of recent callers, keyed by (pointer, rows, strides): a model calls with the same few
+  // buffers for every layer and chunk, so cuTensorMapEncodeTiled runs once per buffer, not twice per call
+  struct TmEntry { const void* ptr; int64_t tok_stride, head_stride; int rows; CUtensorMap map; };
+  static constexpr int kTmCache = 8;
+  TmEntry tm_cache[kTmCache];
+  int tm_cache_n = 0, tm_cache_next = 0;
+  size_t score_smem_attr[3][4] = {};   // dynamic-smem limit already set on uf_score_topk_kernel<d, QG>
   std::string err;
 };
 

@@ -276,10 +276,13 @@ cudaError_t uf_launch_select(uf_ctx* c, const UfView& v, const __nv_bfloat16* q,
   dim3 gs(uf_ceil_div(nqb, qg), v.H);
 #define UF_SCORE_LAUNCH(DD, QG)                                                                              \
   {                                                                                                          \
-    if (smem > 48 * 1024)                                                                                    \
+    size_t& attr = c->score_smem_attr[DD == 32 ? 0 : DD == 64 ? 1 : 2][QG == 8 ? 0 : QG == 4 ? 1 : QG == 2 ? 2 : 3]; \
+    if (smem > 48 * 1024 && smem > attr) {          /* raise the limit once, not on every call */             \
       e = cudaFuncSetAttribute(uf_score_topk_kernel<DD, QG>, cudaFuncAttributeMaxDynamicSharedMemorySize,    \
                                (int)smem);                                                                   \
-    if (e != cudaSuccess) return e;                                                                          \
+      if (e != cudaSuccess) return e;                                                                        \
+      attr = smem;                                                                                           \
+    }                                                                                                        \
     uf_score_topk_kernel<DD, QG><<<gs, kScoreThreads, smem, s>>>(v, c->qbar, c->kpool, nqb, k_eff, c->sel_q, \
                                                                  c->sel_rank, c->kcap, idx_out, cnt_out);    \
   }

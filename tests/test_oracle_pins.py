@@ -472,6 +472,121 @@ def test_attention_vs_pure_python_bruteforce():
                 assert abs(res[c][3][0, r] - (mx + math.log(z))) < 1e-13
 
 
+@pytest.mark.parametrize("S,n0,C", [(0, 5, 2), (0, 5, 3), (2, 5, 2), (2, 5, 3), (2, 3, 2), (3, 3, 3), (1, 1, 2)])
+def test_sink_variants_vs_pure_python_bruteforce(S, n0, C):
+    """S = 0 (no sink), S >= 2, and a chunk 0 shorter than S*B (the sink is then all of chunk 0, its last
+    block ragged): SINK / CAND / KEPT sets, the selection and the attention re-done from the definitions with
+    Python loops (readings R-14/R-15: sink = blocks 0..S-1 of chunk 0 that exist, always attended for c > 0,
+    never a candidate, never counted twice; served from the sink copy after chunk 0 is evicted).  Catches: a sink
+    id left in CAND, a sink block attended twice while chunk 0 is resident, pad rows of a short sink block
+    counted as keys, sink dropped after eviction, S = 0 still reserving block 0."""
+    rng = np.random.default_rng(100 + 10 * S + n0 + C)
+    H, d, B, n, k = 1, 4, 2, 5, 2                                        # BPC = 3, ragged (2, 2, 1)
+    bpc = 3
+    lens = [n0, n, n, 4, n]
+    chunks = [rand_chunk(rng, m, H, d) for m in lens]
+    orc = UFOracle(H, d, B, n, C, sink_blocks=S)
+    res = run_stream(orc, chunks, topk_count=k)
+    sink_tok = min(S * B, n0)
+    sink_ids = list(range(-(-sink_tok // B)))                            # blocks of chunk 0 inside the sink
+
+    def rows_of(g):
+        cg, b = divmod(g, bpc)
+        return cg, range(b * B, min((b + 1) * B, lens[cg]))
+
+    for c in range(len(lens)):
+        Q = chunks[c][0]
+        resident_prior = [x for x in range(max(0, c - C + 1), c)]
+        sink = sink_ids if c > 0 else []
+        cand = [cc * bpc + b for cc in resident_prior for b in range(-(-lens[cc] // B))
+                if cc * bpc + b not in sink_ids]
+        assert orc_sets_equal(res[c], cand, k)
+        nqb = -(-lens[c] // B)
+        for i in range(nqb):
+            qrows = range(i * B, min((i + 1) * B, lens[c]))
+            qm = [sum(Q[r, 0, t] for r in qrows) / len(qrows) for t in range(d)]
+            sc = []
+            for g in cand:
+                cg, rr = rows_of(g)
+                km = [sum(chunks[cg][1][r, 0, t] for r in rr) / len(rr) for t in range(d)]
+                sc.append(sum(qm[t] * km[t] for t in range(d)) / math.sqrt(d))
+            top = brute_topk(sc, cand, min(k, len(cand)))
+            assert list(res[c][0][0, i, :len(top)]) == top
+            # keys: sink rows (from chunk 0's first sink_tok rows), top-k blocks, the whole current chunk
+            keys = []
+            for g in sink:
+                keys += [(0, m) for m in range(g * B, min((g + 1) * B, sink_tok))]
+            for g in top:
+                cg, rr = rows_of(g)
+                keys += [(cg, m) for m in rr]
+            keys += [(c, m) for m in range(lens[c])]
+            assert len(keys) == len(set(keys)), "a key row is attended twice"
+            for r in qrows:
+                logit = [sum(Q[r, 0, t] * chunks[cg][1][m, 0, t] for t in range(d)) / math.sqrt(d) for cg, m in keys]
+                mx = max(logit)
+                e = [math.exp(x - mx) for x in logit]
+                z = sum(e)
+                want = sum(ei * chunks[cg][2][m, 0] for ei, (cg, m) in zip(e, keys)) / z
+                assert np.allclose(res[c][2][r, 0], want, atol=1e-13)
+                assert abs(res[c][3][0, r] - (mx + math.log(z))) < 1e-13
+
+
+def orc_sets_equal(step_result, cand, k):
+    """count column of a step == min(k, |CAND|) for every (head, query block)"""
+    return bool(np.all(step_result[1] == min(k, len(cand))))
+
+
+def test_sink_candidate_and_kept_sets_explicit():
+    """The sets themselves, spelled out for S = 0 / 2 and a short chunk 0 (B = 4, BPC = 3, C = 2)."""
+    rng = np.random.default_rng(77)
+    H, d, B, n = 1, 4, 4, 12
+    # S = 0: nothing reserved, block 0 of chunk 0 is an ordinary candidate while chunk 0 is resident
+    o = UFOracle(H, d, B, n, 2, sink_blocks=0)
+    for c in range(3):
+        Q, K, V = rand_chunk(rng, n, H, d)
+        o.kv_append(K, V)
+        o.select_blocks(Q, topk_count=1)
+        assert o.sink_ids() == []
+        assert o.candidate_ids() == ([] if c == 0 else list(range((c - 1) * 3, c * 3)))
+        assert [g for g, fs in o.kept_blocks(0, 0) if fs] == []
+        assert len(o.kept_blocks(0, 0)) == (3 if c == 0 else 4)
+    # S = 2: ids 0, 1 are sink; chunk 1 sees CAND = {2} only; after eviction of chunk 0 the sink stays
+    o = UFOracle(H, d, B, n, 2, sink_blocks=2)
+    for c in range(3):
+        Q, K, V = rand_chunk(rng, n, H, d)
+        o.kv_append(K, V)
+        o.select_blocks(Q, topk_count=5)
+        assert o.sink_ids() == [0, 1]
+        assert o.candidate_ids() == [[], [2], [3, 4, 5]][c]
+        kept = o.kept_blocks(0, 1)
+        assert [g for g, fs in kept if fs] == ([] if c == 0 else [0, 1])
+        assert [g for g, fs in kept if not fs] == [[0, 1, 2], [2, 3, 4, 5], [3, 4, 5, 6, 7, 8]][c]
+    # chunk 0 of 6 tokens with S = 2: the sink is rows 0..5 (block 1 ragged, 2 rows); no candidate from chunk 0
+    o = UFOracle(H, d, B, n, 2, sink_blocks=2)
+    Q, K, V = rand_chunk(rng, 6, H, d)
+    o.kv_append(K, V)
+    assert o.sink_K.shape[0] == 6 and o.sink_ids() == [0, 1]
+    Q, K, V = rand_chunk(rng, n, H, d)
+    o.kv_append(K, V)
+    o.select_blocks(Q, topk_count=3)
+    assert o.candidate_ids() == [] and o.sel["cnt"].max() == 0
+    kr, vr = o.block_kv(1, from_sink=True)
+    assert kr.shape[0] == 2
+    assert sum(o.block_kv(g, fs)[0].shape[0] for g, fs in o.kept_blocks(0, 0)) == 6 + n
+
+
+def test_kept_flop_closed_form():
+    """kept_flop = 4 d sum(rows x keys): all blocks full -> 4 d H n (S B + k B + n)."""
+    rng = np.random.default_rng(78)
+    H, d, B, n = 2, 4, 4, 12
+    o = UFOracle(H, d, B, n, 3, sink_blocks=1)
+    for c in range(3):
+        Q, K, V = rand_chunk(rng, n, H, d)
+        o.kv_append(K, V)
+    o.select_blocks(Q, topk_count=2)
+    assert o.kept_flop() == 4 * d * H * n * (1 * B + 2 * B + n)
+
+
 def test_sparse_differs_from_dense_when_blocks_dropped():
     """Sanity: with k small the result is NOT the dense one (the mask really restricts)."""
     rng = np.random.default_rng(18)

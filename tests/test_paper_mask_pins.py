@@ -1,0 +1,234 @@
+"""Pins for the paper-faithful mask oracle (oracle/uf_paper_mask.py) against things
+other than itself: closed forms of the tiling, brute force over coordinates, an independently written dense
+chunk-causal attention, pure-Python loops from the definitions, and the values the paper prints (Table 21,
+tests/golden/table21_sparsity.txt).  CPU only.  Each test names the mistake it is meant to catch."""
+import math
+import os
+
+import numpy as np
+import pytest
+from scipy.special import logsumexp, softmax
+
+import uf_workloads as wl
+from oracle.uf_paper_mask import UFPaperOracle
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def bf16(x):
+    return wl.bf16_bits_to_f32(wl.f32_to_bf16_bits(np.asarray(x, dtype=np.float32))).astype(np.float64)
+
+
+def rand_chunk(rng, n, H, d, scale=1.0):
+    return tuple(bf16(scale * rng.standard_normal((n, H, d))) for _ in range(3))
+
+
+# --------------------------------------------------------------------------- tiling (R-29)
+@pytest.mark.parametrize("F,Hg,Wg", [(2, 16, 24), (3, 68, 120), (3, 90, 160), (2, 60, 104), (1, 5, 3)])
+def test_tiling_is_a_partition_with_closed_form_sizes(F, Hg, Wg):
+    """Every token of the chunk lies in exactly one tile; tile (it, ih, iw) holds min(b_t, F - it*b_t) * ... tokens;
+    a grid the block shape divides gives 128-token tiles only (2*8*8).  Catches: x/y swapped, a ragged edge
+    dropped or wrapped, tiles overlapping."""
+    o = UFPaperOracle(1, 4, F, Hg, Wg, 2)
+    assert o.NB == -(-F // 2) * -(-Hg // 8) * -(-Wg // 8)
+    seen = np.zeros(F * Hg * Wg, dtype=np.int32)
+    for b in range(o.NB):
+        it, ih, iw = o.coords(b)
+        assert b == (it * o.nbh + ih) * o.nbw + iw
+        want = min(2, F - 2 * it) * min(8, Hg - 8 * ih) * min(8, Wg - 8 * iw)
+        toks = o.tokens_of[b]
+        assert len(toks) == want >= 1
+        seen[toks] += 1
+        t, y, x = toks // (Hg * Wg), (toks // Wg) % Hg, toks % Wg
+        assert (t // 2 == it).all() and (y // 8 == ih).all() and (x // 8 == iw).all()
+    assert (seen == 1).all()
+    if F % 2 == 0 and Hg % 8 == 0 and Wg % 8 == 0:
+        assert all(len(t) == 128 for t in o.tokens_of)
+
+
+def test_block_counts_of_the_baseline_grids():
+    """BASELINE.json grids under (2,8,8): 1K 3x68x120 -> 2*9*15 = 270 tiles, 2K 3x90x160 -> 2*12*20 = 480;
+    the paper's own 1K chunk (2 latent frames of 960x1664 -> 60x104) -> 1*8*13 = 104 tiles,
+    i.e. two chunks in the causal mask give the "N_blocks ~ 200 at 1K" of P:820."""
+    assert UFPaperOracle(1, 4, 3, 68, 120, 2).NB == 270
+    assert UFPaperOracle(1, 4, 3, 90, 160, 2).NB == 480
+    assert UFPaperOracle(1, 4, 2, 60, 104, 2).NB == 104 and abs(2 * 104 - 200) <= 10
+
+
+def test_local_window_bruteforce_and_symmetry():
+    """M_local (r = 9): |dh| <= 4 and |dw| <= 4 in block coordinates, any temporal tile; symmetric; an interior
+    block has 81 neighbours per temporal tile.  Catches: window in token (not block) units, r vs (r-1)/2, a window
+    that also cuts the temporal axis."""
+    o = UFPaperOracle(1, 4, 4, 96, 120, 2)                 # 2 x 12 x 15 tiles
+    M = np.array([[o.is_local(i, j) for j in range(o.NB)] for i in range(o.NB)])
+    assert (M == M.T).all() and M.diagonal().all()
+    for i in range(o.NB):
+        _, hi, wi = o.coords(i)
+        want = sum(1 for j in range(o.NB) if max(abs(o.coords(j)[1] - hi), abs(o.coords(j)[2] - wi)) <= 4)
+        assert M[i].sum() == want
+    centre = (0 * o.nbh + 6) * o.nbw + 7
+    assert M[centre].sum() == 81 * o.nbt
+    o3 = UFPaperOracle(1, 4, 2, 96, 120, 2, window=3)
+    assert sum(o3.is_local(centre, j) for j in range(o3.NB)) == 9
+
+
+# --------------------------------------------------------------------------- Eq. 10 repaired (R-34)
+def test_adaptive_budget_floor_clamp_linearity_and_table21():
+    """tau_k = max(k_min, floor(rho * 0.42 * N_blocks)): k_min floor, clamp to N_blocks, linear in N_blocks
+    ("scales linearly with sequence length"), and the kept fraction against the sparsity column of Table 21
+    (P:826-832): exact at the default rho = 1.0, within 4 points elsewhere."""
+    o = UFPaperOracle(1, 4, 2, 16, 16, 2)
+    assert o.adaptive_budget(5, 1000) == 4 and o.adaptive_budget(3, 1000) == 3 and o.adaptive_budget(0, 1000) == 0
+    assert o.adaptive_budget(1000, 1000) == 420 and o.adaptive_budget(2000, 1000) == 840
+    assert o.adaptive_budget(540, 1000) == 226 and o.adaptive_budget(1440, 1000) == 604
+    assert o.adaptive_budget(100, 3000) == 100                                   # clamp
+    for n in (200, 312, 540, 1440, 10_000):
+        assert abs(o.adaptive_budget(2 * n, 1000) - 2 * o.adaptive_budget(n, 1000)) <= 1
+    rows = [l.split() for l in open(os.path.join(GOLDEN, "table21_sparsity.txt")) if l[0] != "#"]
+    assert len(rows) == 5
+    for rho, sparse in rows:
+        n = 10_000
+        kept = o.adaptive_budget(n, int(round(float(rho) * 1000))) / n
+        tol_permille = 5 if float(rho) == 1.0 else 40                             # "within 4 points"
+        assert abs(round((1.0 - kept) * 1000) - 10 * int(sparse)) <= tol_permille, (rho, kept)
+
+
+# --------------------------------------------------------------------------- selection (Eq. 4, R-32/R-33)
+def brute_select(o, chunks, c, Q, k, resident):
+    """KEPT from the definitions with Python loops: exact-k by score over every block of the resident chunks
+    (ties -> lower id), then the 9x9 window, then the own block."""
+    F, Hg, Wg, H, d = o.F, o.Hg, o.Wg, o.H, o.d
+    nbh, nbw = -(-Hg // 8), -(-Wg // 8)
+    NB = -(-F // 2) * nbh * nbw
+
+    def toks(b):
+        it, ih, iw = b // (nbh * nbw), (b // nbw) % nbh, b % nbw
+        return [(t * Hg + y) * Wg + x for t in range(2 * it, min(2 * it + 2, F))
+                for y in range(8 * ih, min(8 * ih + 8, Hg)) for x in range(8 * iw, min(8 * iw + 8, Wg))]
+
+    out = {}
+    for h in range(H):
+        for i in range(NB):
+            qm = [sum(Q[n, h, t] for n in toks(i)) / len(toks(i)) for t in range(d)]
+            sc = {}
+            for cc in resident:
+                for b in range(NB):
+                    km = [sum(chunks[cc][1][n, h, t] for n in toks(b)) / len(toks(b)) for t in range(d)]
+                    acc = 0.0
+                    for t in range(d):
+                        acc = acc + qm[t] * km[t]
+                    sc[cc * NB + b] = acc / math.sqrt(d)
+            order = sorted(sc, key=lambda g: (-sc[g], g))[:k]
+            ih, iw = (i // nbw) % nbh, i % nbw
+            half = (o.r - 1) // 2
+            keep = {g for g in order if abs(((g % NB) // nbw) % nbh - ih) <= half and abs((g % NB) % nbw - iw) <= half}
+            out[h, i] = sorted(keep | {c * NB + i})
+    return out, toks
+
+
+@pytest.mark.parametrize("window,k", [(3, 5), (9, 4), (1, 3)])
+def test_selection_and_attention_vs_pure_python_bruteforce(window, k):
+    """Whole paper-mode path on a tiny ragged grid (3 x 20 x 27 tokens -> 2 x 3 x 4 tiles) re-done with Python loops.
+    Catches: top-k taken inside the window instead of before it, missing own block, current chunk left out of the
+    candidates, wrong tile membership of edge tokens, pad tokens counted."""
+    rng = np.random.default_rng(20 + window)
+    H, d, F, Hg, Wg, C = 2, 4, 3, 20, 27, 2
+    o = UFPaperOracle(H, d, F, Hg, Wg, C, window=window, k_min=1)
+    n = F * Hg * Wg
+    chunks = [rand_chunk(rng, n, H, d) for _ in range(3)]
+    for c, (Q, K, V) in enumerate(chunks):
+        o.kv_append(K, V)
+        idx, cnt = o.select_blocks(Q, topk_count=k)
+        resident = [x for x in range(max(0, c - C + 1), c + 1)]
+        want, toks = brute_select(o, chunks, c, Q, k, resident)
+        for h in range(H):
+            for i in range(o.NB):
+                assert list(idx[h, i, :cnt[h, i]]) == want[h, i]
+                assert 1 <= cnt[h, i] <= k + 1 and (idx[h, i, cnt[h, i]:] == -1).all()
+        O, lse = o.sparse_attn(Q, heads=[1], qblocks=[0, o.NB - 1])
+        for i in (0, o.NB - 1):
+            keys = [(g // o.NB, m) for g in want[1, i] for m in toks(g % o.NB)]
+            for r in toks(i):
+                logit = [sum(Q[r, 1, t] * chunks[cc][1][m, 1, t] for t in range(d)) / math.sqrt(d) for cc, m in keys]
+                mx = max(logit)
+                e = [math.exp(x - mx) for x in logit]
+                z = sum(e)
+                wantv = sum(ei * chunks[cc][2][m, 1] for ei, (cc, m) in zip(e, keys)) / z
+                assert np.allclose(O[r, 1], wantv, atol=1e-13)
+                assert abs(lse[1, r] - (mx + math.log(z))) < 1e-12
+        assert np.isnan(O[toks(1), 1]).all()
+
+
+def test_all_kept_equals_dense_chunk_causal():
+    """Window covering the whole grid and k = N_blocks: the mask keeps every block of every resident chunk, so the
+    result is dense chunk-causal attention computed by an independent routine (scipy softmax over concatenated
+    raster-order tensors, no tiles).  Catches: a tile's tokens scattered back to the wrong raster rows."""
+    rng = np.random.default_rng(31)
+    H, d, F, Hg, Wg, C = 2, 8, 3, 12, 20, 3
+    n = F * Hg * Wg
+    o = UFPaperOracle(H, d, F, Hg, Wg, C, window=99)
+    chunks = [rand_chunk(rng, n, H, d) for _ in range(3)]
+    for c, (Q, K, V) in enumerate(chunks):
+        o.kv_append(K, V)
+        idx, cnt = o.select_blocks(Q, topk_count=10 ** 6)
+        assert (cnt == (c + 1) * o.NB).all()
+        O, lse = o.sparse_attn(Q)
+        Kc = np.concatenate([ch[1] for ch in chunks[:c + 1]], axis=0)
+        Vc = np.concatenate([ch[2] for ch in chunks[:c + 1]], axis=0)
+        logits = np.einsum("nhd,mhd->hnm", Q, Kc) / math.sqrt(d)
+        want = np.einsum("hnm,mhd->nhd", softmax(logits, axis=-1), Vc)
+        assert np.allclose(O, want, atol=1e-12) and np.allclose(lse, logsumexp(logits, axis=-1), atol=1e-12)
+
+
+def test_indicator_v_mass_only_on_kept_blocks_never_future_and_budget_mode():
+    """V channel = global block id indicator: attention mass is exactly 0 outside KEPT, sums to 1, no kept id belongs
+    to a later chunk or to an evicted one (M_causal), at most tau_k + 1 blocks per row with tau_k from the
+    repaired Eq. 10, every kept block but the own one inside the window."""
+    rng = np.random.default_rng(32)
+    H, F, Hg, Wg, C = 2, 2, 24, 40, 2                       # 1 x 3 x 5 = 15 tiles, all full
+    n = F * Hg * Wg
+    n_chunks = 3
+    o = UFPaperOracle(H, 15 * n_chunks, F, Hg, Wg, C, window=3)
+    for c in range(n_chunks):
+        Q, K, _ = rand_chunk(rng, n, H, o.d, scale=0.7)
+        V = np.zeros((n, H, o.d))
+        for b in range(o.NB):
+            V[o.tokens_of[b], :, c * o.NB + b] = 1.0
+        o.kv_append(K, V)
+        idx, cnt = o.select_blocks(Q, rho_permille=1500)
+        n_mask = min(c + 1, C) * o.NB
+        tau = max(4, (1500 * 420 * n_mask) // 1_000_000)
+        assert o.sel["k"] == tau and cnt.max() <= tau + 1
+        O, _ = o.sparse_attn(Q)
+        for h in range(H):
+            for i in range(o.NB):
+                kept = set(int(g) for g in idx[h, i, :cnt[h, i]])
+                assert c * o.NB + i in kept
+                assert all((c - C + 1) * o.NB <= g < (c + 1) * o.NB and g >= 0 for g in kept)
+                assert all(o.is_local(i, g % o.NB) for g in kept)
+                rows = O[o.tokens_of[i], h]
+                assert np.allclose(rows.sum(axis=1), 1.0, atol=1e-13)
+                for g in range(o.d):
+                    assert (rows[:, g] > 0).all() if g in kept else (rows[:, g] == 0).all()
+
+
+def test_ties_go_to_the_lower_id_before_the_window():
+    """Two bitwise-equal key tiles (one inside, one outside the window) tie; with room for one, the LOWER id takes
+    the slot even when it lies outside the window and is then cut by M_local (Eq. 4's order: top-k, then the
+    intersection)."""
+    rng = np.random.default_rng(33)
+    H, d, F, Hg, Wg = 1, 8, 2, 8, 48                       # 1 x 1 x 6 tiles
+    n = F * Hg * Wg
+    o = UFPaperOracle(H, d, F, Hg, Wg, 2, window=3, k_min=1)
+    Q0, K0, V0 = rand_chunk(rng, n, H, d, scale=0.1)
+    o.kv_append(K0, V0)
+    Q1, K1, V1 = rand_chunk(rng, n, H, d, scale=0.1)
+    strong = bf16(3.0 + 0.1 * rng.standard_normal((128, H, d)))
+    K1[o.tokens_of[0]] = strong                            # current chunk, tile 0 (outside tile 5's window)
+    K1[o.tokens_of[4]] = strong                            # current chunk, tile 4 (inside tile 5's window)
+    Q1[:] = bf16(np.abs(Q1) + 1.0)
+    o.kv_append(K1, V1)
+    idx, cnt = o.select_blocks(Q1, topk_count=1)
+    assert cnt[0, 5] == 1 and list(idx[0, 5, :1]) == [6 + 5]           # top-1 = tile 0 (lower id), cut; own block stays
+    idx, cnt = o.select_blocks(Q1, topk_count=2)
+    assert list(idx[0, 5, :cnt[0, 5]]) == [6 + 4, 6 + 5]

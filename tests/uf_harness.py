@@ -12,8 +12,12 @@ from oracle.uf_oracle import UFOracle
 # BASELINE.json north_star: attention outputs within max-abs 2e-2 and mean-abs 2e-3 of the fp64 oracle
 O_MAX_ABS = 2e-2
 O_MEAN_ABS = 2e-3
-# LSE is fp32 of a log-sum over <= ~60k keys: DESIGN.md "Tolerances"
-LSE_MAX_ABS = 2e-3
+# LSE has no tolerance in BASELINE.json; the bound is derived in DESIGN.md section 6 from the kernel's design: the
+# row sum l adds the bf16-rounded probabilities (the numbers the P V MMA multiplies, which is what keeps O inside
+# the BJ bound at every softmax scale), each within 2^-8 relative of its exact value (round-to-nearest, 8
+# significant bits), so |l~/l - 1| <= 2^-8 and |dLSE| <= -ln(1 - 2^-8) = 3.92e-3; the degree-3 exp2 polynomial
+# (7.5e-5), ex2.approx, the fp32 sum over <= 6e4 keys and log2f add < 1e-4.  Reached only by one-hot rows.
+LSE_MAX_ABS = 4.1e-3
 
 
 def bits_to_f64(bits: np.ndarray) -> np.ndarray:
@@ -70,7 +74,8 @@ class CudaStream:
         else:
             o = torch.full((n, H, d), float("nan"), dtype=torch.bfloat16, device=self.dev)
         lse = torch.full((H, n), float("nan"), dtype=torch.float32, device=self.dev) if want_lse else None
-        uf.uf_set_attn_impl(self.ctx, impl)
+        # shapes other than B = d = 128 have no tcgen05 kernel: the caller has to opt in to the CUDA-core kernel
+        uf.uf_set_attn_impl(self.ctx, impl if (w.block == 128 and w.head_dim == 128) else 1)
         if fused_qkv:
             # attention takes one token stride for Q and O: O's [n, 2, H, d] slice has stride 2*H*d, so Q is
             # re-packed to that stride too (Q of the select call above kept the fused layout)
@@ -115,14 +120,6 @@ def oracle_step(orc: UFOracle, Qb, Kb, Vb, topk_count=-1, topk_percent=-1, windo
     if attn:
         out["O"], out["lse"] = orc.sparse_attn(Q, heads=heads, qblocks=qblocks, softmax_scale=scale)
     return out
-
-
-def sharp_o_max_abs(v_abs_max: float) -> float:
-    """Max-abs bound on O for tests that sharpen the softmax beyond the 1/sqrt(d) of the BASELINE.json workloads
-    (DESIGN.md section 6): the row sum adds the unrounded fp32 probabilities while the P V MMA multiplies their bf16
-    roundings, so a (nearly) one-hot row carries the relative rounding error of its one probability, <= 2^-8, times
-    |v|, on top of the bf16 rounding of the output, <= 2^-8 |O| <= 2^-8 max|V|."""
-    return max(O_MAX_ABS, 2.0 ** -7 * v_abs_max)
 
 
 def compare_step(got: dict, ref: dict, where: str = "", o_max_abs: float = O_MAX_ABS):
