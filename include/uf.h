@@ -137,6 +137,61 @@ int32_t uf_sparse_attn_fwd(uf_ctx* ctx, const void* q, void* o, float* lse, int3
                            int64_t tok_stride, int64_t head_stride, float softmax_scale,
                            void* stream);
 
+/* ---- Paper-mask mode: the mask exactly as section 2.3.1 / appendix L.1 define it -----
+ * P:86  "The 3D token grid (t,h,w) is divided into non-overlapping blocks of (b_t,b_h,b_w) ... a spatial locality
+ *        mask M_local confines each block's receptive field to a sliding window of size r x r, and a temporal
+ *        causal mask M_causal ensures each temporal chunk attends only to current and preceding chunks"
+ * P:88  Eq. 4: M_sparse[i,j] = 1[softmax(s_i,:)_j >= tau_k]  n  M_local  n  M_causal
+ * P:815 Eq. 10 (repaired, reading R-34): tau_k = max(k_min, floor(rho * 0.42 * N_blocks))
+ * P:343 block (2,8,8), local window 9 x 9, rho = 1.0, k_min = 4.
+ * Differences from the default (BASELINE.json) mode: blocks are 3-D tiles of the chunk's token grid (edge tiles
+ * ragged, R-29); the candidates of the top-k are ALL blocks in the causal mask, the current chunk's included;
+ * the top-k is intersected with the window (R-30/R-32); the query block's own key block is always kept (R-33);
+ * there is no sink and no implicitly kept current chunk.
+ *
+ * Layout: in this mode Q, K, V, O are in TILED order: n_tokens = N_b * block rows, block b = (it*nbh + ih)*nbw + iw
+ * (nbt = ceil(F/bt), ...) owns rows [b*block, (b+1)*block), of which the first nvalid(b) hold the tokens of tile
+ * (it, ih, iw) that exist, in raster (t, y, x) order inside the tile, and the rest are pad rows (zeros; their O rows
+ * are meaningless).  A model keeps its activations in this order for all layers (attention is the only
+ * token-mixing op); uf_tile_tokens / uf_untile_tokens convert from / to raster order.  Global id g = chunk*N_b + b. */
+typedef struct uf_tiling {
+  int32_t frames, grid_h, grid_w;   /* F, Hg, Wg: token grid of one chunk (every chunk the same)               */
+  int32_t bt, bh, bw;               /* tile shape; bt*bh*bw must equal uf_config.block (paper: 2, 8, 8)        */
+  int32_t window;                   /* r, odd: |dih|, |diw| <= (r-1)/2 in tile coordinates (paper: 9)          */
+} uf_tiling;
+
+/* Switch an EMPTY ctx (before the first append, or after uf_ctx_reset) to paper-mask mode.  Needs
+ * sink_blocks == 0 and chunk_tokens_max == N_b * block.  Errors: UF_ERR_STATE (cache not empty),
+ * UF_ERR_INVALID_ARG (sizes).  From then on uf_kv_append takes tiled chunks of exactly N_b * block rows and
+ * uf_select_blocks is replaced by uf_select_blocks_paper. */
+int32_t uf_ctx_set_tiling(uf_ctx* ctx, const uf_tiling* tiling);
+
+/* Host query: N_blocks = blocks in the causal mask for the current state (all resident chunks incl. the newest)
+ * and the budget k' = min(k, N_blocks), k = topk_count if >= 0 else tau_k(rho_permille / 1000) above. */
+int32_t uf_query_budget_paper(const uf_ctx* ctx, int32_t topk_count, int32_t rho_permille,
+                              int32_t* n_blocks, int32_t* k_eff);
+
+/* Eq. 4 selection for the newest chunk (q in tiled order, as passed to the append): per (head, query tile) the k'
+ * best-scoring blocks of the causal mask (fp64 scores as in uf_select_blocks; ties -> lower global id), then only
+ * those inside the window, plus the tile's own block.
+ *   idx_out   device pointer or NULL: int32 [H, N_b, idx_stride] ascending global ids, padded with -1;
+ *             idx_stride >= min(k' + 1, N_blocks) (else UF_ERR_CAPACITY)
+ *   cnt_out   device pointer or NULL: int32 [H, N_b] kept blocks per row (1 .. k' + 1)
+ * The selection is kept in the ctx for the following uf_sparse_attn_fwd, which then attends exactly these blocks. */
+int32_t uf_select_blocks_paper(uf_ctx* ctx, const void* q, int32_t n_tokens,
+                               int64_t tok_stride, int64_t head_stride,
+                               int32_t topk_count, int32_t rho_permille,
+                               int32_t* idx_out, int32_t idx_stride, int32_t* cnt_out, void* stream);
+
+/* Raster [F*Hg*Wg, H, d] -> tiled [N_b*block, H, d] (pad rows written as zeros) and back (pad rows skipped).
+ * Device pointers, bf16, element strides as everywhere; src and dst must not overlap.  Asynchronous on `stream`. */
+int32_t uf_tile_tokens(uf_ctx* ctx, const void* raster, void* tiled,
+                       int64_t raster_tok_stride, int64_t raster_head_stride,
+                       int64_t tiled_tok_stride, int64_t tiled_head_stride, void* stream);
+int32_t uf_untile_tokens(uf_ctx* ctx, const void* tiled, void* raster,
+                         int64_t tiled_tok_stride, int64_t tiled_head_stride,
+                         int64_t raster_tok_stride, int64_t raster_head_stride, void* stream);
+
 /* impl: 0 = tcgen05 kernel only (default; shapes it does not cover -> UF_ERR_UNSUPPORTED),
  *       1 = the generic CUDA-core attention kernel (any supported shape; slow). */
 int32_t uf_set_attn_impl(uf_ctx* ctx, int32_t impl);

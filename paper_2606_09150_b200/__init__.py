@@ -5,16 +5,9 @@ by `build.py` for sm_100a).  This package is its thin ctypes binding: same call 
 marshalling only.  No CPU fallback exists; importing works without a GPU, every device call fails
 loudly (UFError) without one.
 """
-from .binding import (  # noqa: F401
-    LIB_PATH, SYMBOLS, UFError, load_library, uf_ctx_create, uf_ctx_destroy, uf_ctx_device_bytes,
-    uf_attn_redone_items, uf_ctx_launch_count, uf_ctx_reset, uf_get_cache_block, uf_get_pooled_k, uf_get_slot_map, uf_kv_append,
-    uf_last_error, uf_query_topk, uf_select_blocks, uf_set_attn_impl, uf_sparse_attn_fwd, uf_version,
-)
+from . import binding  # noqa: F401
+from .binding import *  # noqa: F401,F403
+from .binding import __all__ as _binding_all
 from .build import build  # noqa: F401
 
-__all__ = [
-    "LIB_PATH", "SYMBOLS", "UFError", "build", "load_library", "uf_ctx_create", "uf_ctx_destroy",
-    "uf_attn_redone_items", "uf_ctx_device_bytes", "uf_ctx_launch_count", "uf_ctx_reset", "uf_get_cache_block", "uf_get_pooled_k",
-    "uf_get_slot_map", "uf_kv_append", "uf_last_error", "uf_query_topk", "uf_select_blocks", "uf_set_attn_impl",
-    "uf_sparse_attn_fwd", "uf_version",
-]
+__all__ = list(_binding_all) + ["build", "binding"]

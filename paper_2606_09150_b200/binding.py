@@ -24,6 +24,7 @@ SYMBOLS = [
     "uf_ctx_create", "uf_ctx_destroy", "uf_ctx_reset", "uf_kv_append", "uf_query_topk", "uf_select_blocks",
     "uf_sparse_attn_fwd", "uf_set_attn_impl", "uf_get_slot_map", "uf_get_cache_block", "uf_get_pooled_k",
     "uf_attn_redone_items", "uf_ctx_device_bytes", "uf_ctx_launch_count", "uf_last_error", "uf_version",
+    "uf_ctx_set_tiling", "uf_query_budget_paper", "uf_select_blocks_paper", "uf_tile_tokens", "uf_untile_tokens",
 ]
 
 
@@ -36,6 +37,10 @@ class UFError(RuntimeError):
 class uf_config(Structure):
     _fields_ = [(n, c_int32) for n in ("n_heads", "head_dim", "block", "chunk_tokens_max", "capacity_chunks",
                                        "sink_blocks", "k_min", "device")]
+
+
+class uf_tiling(Structure):
+    _fields_ = [(n, c_int32) for n in ("frames", "grid_h", "grid_w", "bt", "bh", "bw", "window")]
 
 
 _lib = None
@@ -69,6 +74,11 @@ def load_library() -> ctypes.CDLL:
     lib.uf_ctx_launch_count.restype = c_int64
     lib.uf_last_error.argtypes = [P]
     lib.uf_last_error.restype = c_char_p
+    lib.uf_ctx_set_tiling.argtypes = [P, POINTER(uf_tiling)]
+    lib.uf_query_budget_paper.argtypes = [P, c_int32, c_int32, POINTER(c_int32), POINTER(c_int32)]
+    lib.uf_select_blocks_paper.argtypes = [P, P, c_int32, c_int64, c_int64, c_int32, c_int32, P, c_int32, P, P]
+    lib.uf_tile_tokens.argtypes = [P, P, P, c_int64, c_int64, c_int64, c_int64, P]
+    lib.uf_untile_tokens.argtypes = [P, P, P, c_int64, c_int64, c_int64, c_int64, P]
     lib.uf_version.argtypes = []
     lib.uf_version.restype = c_char_p
     for name in SYMBOLS:
@@ -142,6 +152,39 @@ def uf_select_blocks(ctx, q, n_tokens: int, tok_stride: int, head_stride: int, t
                                                 topk_percent, _ptr(idx_out), _ptr(cnt_out), _stream(stream)))
 
 
+def uf_ctx_set_tiling(ctx, frames: int, grid_h: int, grid_w: int, bt: int = 2, bh: int = 8, bw: int = 8,
+                      window: int = 9) -> None:
+    t = uf_tiling(frames, grid_h, grid_w, bt, bh, bw, window)
+    _check(ctx, load_library().uf_ctx_set_tiling(ctx, byref(t)))
+
+
+def uf_query_budget_paper(ctx, topk_count: int = -1, rho_permille: int = 1000) -> tuple[int, int]:
+    """-> (N_blocks in the causal mask, k')"""
+    n_blocks, k_eff = c_int32(0), c_int32(0)
+    _check(ctx, load_library().uf_query_budget_paper(ctx, topk_count, rho_permille, byref(n_blocks), byref(k_eff)))
+    return n_blocks.value, k_eff.value
+
+
+def uf_select_blocks_paper(ctx, q, n_tokens: int, tok_stride: int, head_stride: int, topk_count: int = -1,
+                           rho_permille: int = 1000, idx_out=None, idx_stride: int = 0, cnt_out=None,
+                           stream=None) -> None:
+    _check(ctx, load_library().uf_select_blocks_paper(ctx, _ptr(q), n_tokens, tok_stride, head_stride, topk_count,
+                                                      rho_permille, _ptr(idx_out), idx_stride, _ptr(cnt_out),
+                                                      _stream(stream)))
+
+
+def uf_tile_tokens(ctx, raster, tiled, raster_tok_stride: int, raster_head_stride: int, tiled_tok_stride: int,
+                   tiled_head_stride: int, stream=None) -> None:
+    _check(ctx, load_library().uf_tile_tokens(ctx, _ptr(raster), _ptr(tiled), raster_tok_stride, raster_head_stride,
+                                              tiled_tok_stride, tiled_head_stride, _stream(stream)))
+
+
+def uf_untile_tokens(ctx, tiled, raster, tiled_tok_stride: int, tiled_head_stride: int, raster_tok_stride: int,
+                     raster_head_stride: int, stream=None) -> None:
+    _check(ctx, load_library().uf_untile_tokens(ctx, _ptr(tiled), _ptr(raster), tiled_tok_stride, tiled_head_stride,
+                                                raster_tok_stride, raster_head_stride, _stream(stream)))
+
+
 def uf_sparse_attn_fwd(ctx, q, o, lse, n_tokens: int, tok_stride: int, head_stride: int,
                        softmax_scale: float = 0.0, stream=None) -> None:
     _check(ctx, load_library().uf_sparse_attn_fwd(ctx, _ptr(q), _ptr(o), _ptr(lse), n_tokens, tok_stride,
@@ -189,3 +232,6 @@ def uf_ctx_launch_count(ctx) -> int:
 def uf_last_error(ctx=None) -> str:
     msg = load_library().uf_last_error(ctx)
     return msg.decode() if msg else ""
+
+
+__all__ = ["LIB_PATH", "SYMBOLS", "UFError", "load_library", "uf_config", "uf_tiling"] + SYMBOLS

@@ -35,11 +35,14 @@ int n_resident(const uf_ctx* c) {
 }
 
 // Snapshot of the state for the newest chunk (the "current" one).
-bool make_view(const uf_ctx* c, UfView* v) {
+// paper = true (Eq. 4 mode, R-31/R-32): the candidate list is every block in the causal mask, i.e. the current
+// chunk is listed too, as the last "prior".
+bool make_view(const uf_ctx* c, UfView* v, bool paper = false) {
   const int C = c->cfg.capacity_chunks;
   int cur = c->next_chunk - 1;
   if (cur < 0) return false;
   memset(v, 0, sizeof(*v));
+  v->til = c->til;
   v->H = c->cfg.n_heads; v->d = c->cfg.head_dim; v->B = c->cfg.block;
   v->BPC = c->BPC; v->S = c->cfg.sink_blocks; v->P = c->P;
   v->cur_chunk = cur; v->cur_slot = -1;
@@ -57,7 +60,10 @@ bool make_view(const uf_ctx* c, UfView* v) {
     }
   int np = 0, pref = 0;
   for (int i = 0; i < n; ++i) {
-    if (ids[i] == cur) { v->cur_slot = slots[i]; v->cur_ntok = c->slot_ntok[slots[i]]; continue; }
+    if (ids[i] == cur) {
+      v->cur_slot = slots[i]; v->cur_ntok = c->slot_ntok[slots[i]];
+      if (!paper) continue;
+    }
     int nb = n_blocks(c, c->slot_ntok[slots[i]]);
     int first = (ids[i] == 0) ? (n_sink_ids < nb ? n_sink_ids : nb) : 0;   // CAND excludes SINK ids
     v->prior_chunk[np] = ids[i]; v->prior_slot[np] = slots[i];
@@ -119,8 +125,7 @@ int32_t uf_ctx_create(const uf_config* cfg, uf_ctx** out) {
   c->cfg = *cfg;
   c->BPC = uf_ceil_div(cfg->chunk_tokens_max, cfg->block);
   c->P = cfg->sink_blocks + cfg->capacity_chunks * c->BPC;
-  c->kcap = (cfg->capacity_chunks - 1) * c->BPC;
-  if (c->kcap < 1) c->kcap = 1;
+  c->kcap = cfg->capacity_chunks * c->BPC;     // a row keeps at most every block in the causal mask (paper-mask mode)
   if (c->P >= (1 << 20)) { delete c; return fail(nullptr, UF_ERR_CAPACITY, "uf_ctx_create: too many physical blocks"); }
   clear_host_state(c);
   c->host_only = cfg->device < 0;
@@ -148,6 +153,7 @@ int32_t uf_ctx_create(const uf_config* cfg, uf_ctx** out) {
       {(void**)&c->sel_rank, H * BPC * (int64_t)c->kcap * 4},
       {(void**)&c->sel_pair, H * NP * 2 * (int64_t)c->kcap * 4},
       {(void**)&c->pair_cnt, H * NP * 4},
+      {(void**)&c->sel_cnt, H * BPC * 4},
       {(void**)&c->panic_item, H * NP * 4},
       {(void**)&c->panic_last, 4},
   };
@@ -181,7 +187,7 @@ int32_t uf_ctx_destroy(uf_ctx* c) {
     cudaSetDevice(c->cfg.device);
     cudaFree(c->kc); cudaFree(c->vc); cudaFree(c->kpool); cudaFree(c->qbar);
     cudaFree(c->sel_q); cudaFree(c->sel_rank); cudaFree(c->sel_pair); cudaFree(c->pair_cnt);
-    cudaFree(c->panic_item); cudaFree(c->panic_last);
+    cudaFree(c->panic_item); cudaFree(c->panic_last); cudaFree(c->sel_cnt);
   }
   delete c;
   return UF_OK;
@@ -204,6 +210,8 @@ int32_t uf_kv_append(uf_ctx* c, const void* k, const void* v, int32_t n_tokens,
   if (n_tokens < 1) return fail(c, UF_ERR_INVALID_ARG, "uf_kv_append: n_tokens < 1");
   if (n_tokens > c->cfg.chunk_tokens_max) return fail(c, UF_ERR_CAPACITY, "uf_kv_append: n_tokens > chunk_tokens_max");
   if (window_chunks < 0 || window_chunks > C) return fail(c, UF_ERR_CAPACITY, "uf_kv_append: window_chunks outside 0..capacity_chunks");
+  if (c->til.enabled && n_tokens != c->BPC * c->cfg.block)
+    return fail(c, UF_ERR_INVALID_ARG, "uf_kv_append: a tiled ctx takes whole chunks in the tiled layout (n_tokens = N_b * block)");
   if (!c->host_only) {
     int r = check_tensor_args(c, k, tok_stride, head_stride, "uf_kv_append k");
     if (r) return r;
@@ -278,6 +286,7 @@ int32_t uf_select_blocks(uf_ctx* c, const void* q, int32_t n_tokens, int64_t tok
   if (c->host_only) return fail(c, UF_ERR_STATE, "uf_select_blocks: host-only ctx has no device path");
   UfView v;
   if (!make_view(c, &v)) return fail(c, UF_ERR_STATE, "uf_select_blocks: no chunk appended yet");
+  if (c->til.enabled) return fail(c, UF_ERR_STATE, "uf_select_blocks: this ctx is tiled (uf_ctx_set_tiling): use uf_select_blocks_paper");
   if (n_tokens != v.cur_ntok) return fail(c, UF_ERR_INVALID_ARG, "uf_select_blocks: n_tokens differs from the last append");
   int r = check_tensor_args(c, q, tok_stride, head_stride, "uf_select_blocks q");
   if (r) return r;
@@ -287,10 +296,115 @@ int32_t uf_select_blocks(uf_ctx* c, const void* q, int32_t n_tokens, int64_t tok
   if (k > c->kcap) return fail(c, UF_ERR_CAPACITY, "uf_select_blocks: k exceeds workspace (internal)");
   UF_CUDA(c, cudaSetDevice(c->cfg.device));
   cudaError_t e = uf_launch_select(c, v, (const __nv_bfloat16*)q, tok_stride, head_stride, k, idx_out, cnt_out,
-                                   (cudaStream_t)stream);
+                                   false, k, (cudaStream_t)stream);
   if (e != cudaSuccess) return fail_cuda(c, e, "uf_select_blocks kernel launch");
-  c->sel_valid = true; c->sel_k = k; c->sel_ntok = n_tokens;
+  c->sel_valid = true; c->sel_k = k; c->sel_ntok = n_tokens; c->sel_paper = false;
   return UF_OK;
+}
+
+// ---- paper-mask mode (readings R-29..R-35) ----------------
+
+int32_t uf_ctx_set_tiling(uf_ctx* c, const uf_tiling* t) {
+  if (!c || !t) return UF_ERR_INVALID_ARG;
+  if (c->next_chunk != 0) return fail(c, UF_ERR_STATE, "uf_ctx_set_tiling: the cache is not empty (call before the first append or after uf_ctx_reset)");
+  if (t->frames < 1 || t->grid_h < 1 || t->grid_w < 1 || t->bt < 1 || t->bh < 1 || t->bw < 1 ||
+      t->window < 1 || (t->window % 2) == 0)
+    return fail(c, UF_ERR_INVALID_ARG, "uf_ctx_set_tiling: sizes must be >= 1 and the window odd");
+  if ((int64_t)t->bt * t->bh * t->bw != c->cfg.block)
+    return fail(c, UF_ERR_INVALID_ARG, "uf_ctx_set_tiling: bt * bh * bw must equal the ctx's block size");
+  if (c->cfg.sink_blocks != 0)
+    return fail(c, UF_ERR_INVALID_ARG, "uf_ctx_set_tiling: the paper's mask has no sink (create the ctx with sink_blocks = 0)");
+  UfTiling u;
+  u.enabled = 1;
+  u.F = t->frames; u.Hg = t->grid_h; u.Wg = t->grid_w; u.bt = t->bt; u.bh = t->bh; u.bw = t->bw;
+  u.nbt = uf_ceil_div(u.F, u.bt); u.nbh = uf_ceil_div(u.Hg, u.bh); u.nbw = uf_ceil_div(u.Wg, u.bw);
+  u.half = (t->window - 1) / 2;
+  if ((int64_t)u.nbt * u.nbh * u.nbw != c->BPC)
+    return fail(c, UF_ERR_INVALID_ARG, "uf_ctx_set_tiling: chunk_tokens_max must be N_b * block with N_b = ceil(F/bt) * ceil(Hg/bh) * ceil(Wg/bw)");
+  c->til = u;
+  c->sel_valid = false;
+  return UF_OK;
+}
+
+static int paper_budget(const uf_ctx* c, int n_blocks, int topk_count, int rho_permille, int* k_eff) {
+  int64_t k;
+  if (topk_count >= 0) k = topk_count;
+  else {
+    if (rho_permille < 0 || rho_permille > 100000) return UF_ERR_INVALID_ARG;
+    // repaired Eq. 10 (R-34): tau_k = max(k_min, floor(rho * 0.42 * N_blocks)), integers only
+    k = ((int64_t)rho_permille * 420 * n_blocks) / 1000000;
+    if (k < c->cfg.k_min) k = c->cfg.k_min;
+  }
+  if (k > n_blocks) k = n_blocks;
+  *k_eff = (int)k;
+  return UF_OK;
+}
+
+int32_t uf_query_budget_paper(const uf_ctx* c, int32_t topk_count, int32_t rho_permille, int32_t* n_blocks,
+                              int32_t* k_eff) {
+  if (!c) return UF_ERR_INVALID_ARG;
+  if (!c->til.enabled) return UF_ERR_STATE;
+  UfView v;
+  if (!make_view(c, &v, true)) return UF_ERR_STATE;
+  int k = 0;
+  int r = paper_budget(c, v.n_cand, topk_count, rho_permille, &k);
+  if (r) return r;
+  if (n_blocks) *n_blocks = v.n_cand;
+  if (k_eff) *k_eff = k;
+  return UF_OK;
+}
+
+int32_t uf_select_blocks_paper(uf_ctx* c, const void* q, int32_t n_tokens, int64_t tok_stride, int64_t head_stride,
+                               int32_t topk_count, int32_t rho_permille, int32_t* idx_out, int32_t idx_stride,
+                               int32_t* cnt_out, void* stream) {
+  if (!c) return UF_ERR_INVALID_ARG;
+  if (c->host_only) return fail(c, UF_ERR_STATE, "uf_select_blocks_paper: host-only ctx has no device path");
+  if (!c->til.enabled) return fail(c, UF_ERR_STATE, "uf_select_blocks_paper: call uf_ctx_set_tiling first");
+  UfView v;
+  if (!make_view(c, &v, true)) return fail(c, UF_ERR_STATE, "uf_select_blocks_paper: no chunk appended yet");
+  if (n_tokens != v.cur_ntok) return fail(c, UF_ERR_INVALID_ARG, "uf_select_blocks_paper: n_tokens differs from the last append");
+  int r = check_tensor_args(c, q, tok_stride, head_stride, "uf_select_blocks_paper q");
+  if (r) return r;
+  int k = 0;
+  r = paper_budget(c, v.n_cand, topk_count, rho_permille, &k);
+  if (r) return fail(c, r, "uf_select_blocks_paper: rho_permille outside 0..100000");
+  const int max_row = (k + 1 < v.n_cand ? k + 1 : v.n_cand);          // tau_k blocks + the own block
+  if (idx_out && idx_stride < max_row)
+    return fail(c, UF_ERR_CAPACITY, "uf_select_blocks_paper: idx_stride < min(k + 1, N_blocks)");
+  UF_CUDA(c, cudaSetDevice(c->cfg.device));
+  cudaError_t e = uf_launch_select(c, v, (const __nv_bfloat16*)q, tok_stride, head_stride, k, idx_out, cnt_out,
+                                   true, idx_stride, (cudaStream_t)stream);
+  if (e != cudaSuccess) return fail_cuda(c, e, "uf_select_blocks_paper kernel launch");
+  c->sel_valid = true; c->sel_k = k; c->sel_ntok = n_tokens; c->sel_paper = true;
+  return UF_OK;
+}
+
+static int32_t tile_call(uf_ctx* c, const void* src, void* dst, int64_t src_ts, int64_t src_hs, int64_t dst_ts,
+                         int64_t dst_hs, bool untile, void* stream, const char* name) {
+  if (!c) return UF_ERR_INVALID_ARG;
+  if (c->host_only) return fail(c, UF_ERR_STATE, std::string(name) + ": host-only ctx has no device path");
+  if (!c->til.enabled) return fail(c, UF_ERR_STATE, std::string(name) + ": call uf_ctx_set_tiling first");
+  int r = check_tensor_args(c, src, src_ts, src_hs, name);
+  if (r) return r;
+  r = check_tensor_args(c, dst, dst_ts, dst_hs, name);
+  if (r) return r;
+  UF_CUDA(c, cudaSetDevice(c->cfg.device));
+  cudaError_t e = uf_launch_tile(c, (const __nv_bfloat16*)src, (__nv_bfloat16*)dst, src_ts, src_hs, dst_ts, dst_hs,
+                                 untile, (cudaStream_t)stream);
+  if (e != cudaSuccess) return fail_cuda(c, e, name);
+  return UF_OK;
+}
+
+int32_t uf_tile_tokens(uf_ctx* c, const void* raster, void* tiled, int64_t raster_tok_stride,
+                       int64_t raster_head_stride, int64_t tiled_tok_stride, int64_t tiled_head_stride, void* stream) {
+  return tile_call(c, raster, tiled, raster_tok_stride, raster_head_stride, tiled_tok_stride, tiled_head_stride, false,
+                   stream, "uf_tile_tokens");
+}
+
+int32_t uf_untile_tokens(uf_ctx* c, const void* tiled, void* raster, int64_t tiled_tok_stride,
+                         int64_t tiled_head_stride, int64_t raster_tok_stride, int64_t raster_head_stride, void* stream) {
+  return tile_call(c, tiled, raster, tiled_tok_stride, tiled_head_stride, raster_tok_stride, raster_head_stride, true,
+                   stream, "uf_untile_tokens");
 }
 
 int32_t uf_sparse_attn_fwd(uf_ctx* c, const void* q, void* o, float* lse, int32_t n_tokens,
@@ -299,7 +413,7 @@ int32_t uf_sparse_attn_fwd(uf_ctx* c, const void* q, void* o, float* lse, int32_
   if (c->host_only) return fail(c, UF_ERR_STATE, "uf_sparse_attn_fwd: host-only ctx has no device path");
   UfView v;
   if (!make_view(c, &v)) return fail(c, UF_ERR_STATE, "uf_sparse_attn_fwd: no chunk appended yet");
-  if (!c->sel_valid) return fail(c, UF_ERR_STATE, "uf_sparse_attn_fwd: uf_select_blocks must run after the last append");
+  if (!c->sel_valid) return fail(c, UF_ERR_STATE, "uf_sparse_attn_fwd: uf_select_blocks / uf_select_blocks_paper must run after the last append");
   if (n_tokens != c->sel_ntok) return fail(c, UF_ERR_INVALID_ARG, "uf_sparse_attn_fwd: n_tokens differs from the selection's");
   int r = check_tensor_args(c, q, tok_stride, head_stride, "uf_sparse_attn_fwd q");
   if (r) return r;

@@ -31,14 +31,14 @@ __global__ void __launch_bounds__(kThreads)
 uf_append_kernel(const __nv_bfloat16* __restrict__ k, const __nv_bfloat16* __restrict__ v,
                  int64_t tok_stride, int64_t head_stride,
                  __nv_bfloat16* __restrict__ kc, __nv_bfloat16* __restrict__ vc, double* __restrict__ kpool,
-                 int B, int P, int ntok, int phys0, int sink_copy_blocks) {
+                 int B, int P, int ntok, int phys0, int sink_copy_blocks, UfTiling til) {
   constexpr int VPR = D / 8;               // 16-byte vectors per row
   constexpr int RPP = kThreads / VPR;      // rows per pass
   __shared__ double red[RPP][D + 2];
   const int b = blockIdx.x, h = blockIdx.y;
   const int vcx = threadIdx.x % VPR, rg = threadIdx.x / VPR;
   const int row0 = b * B;
-  const int nvalid = min(B, ntok - row0);
+  const int nvalid = til.enabled ? uf_tile_nvalid(til, b) : min(B, ntok - row0);   // tiled: rows [0, nvalid) of the block
   const int phys = phys0 + b;
   const bool to_sink = b < sink_copy_blocks;          // chunk 0: blocks 0..S-1 also go to the sink region
   const int64_t dst = (((int64_t)h * P + phys) * B) * D;
@@ -78,7 +78,53 @@ uf_append_kernel(const __nv_bfloat16* __restrict__ k, const __nv_bfloat16* __res
   }
 }
 
+// ---- raster <-> tiled token order (paper-mask mode, R-29) ------------------------------------------
+// One warp per (tiled row, head).  Tiled row R = b*B + r holds, for r < nvalid(b), the r-th token of tile b in
+// raster order inside the tile; rows r >= nvalid(b) are pad (written as zeros when tiling, skipped when untiling).
+constexpr int kTileWarps = 8;
+__global__ void __launch_bounds__(kTileWarps * 32)
+uf_tile_kernel(const __nv_bfloat16* __restrict__ src, __nv_bfloat16* __restrict__ dst, int64_t src_ts, int64_t src_hs,
+               int64_t dst_ts, int64_t dst_hs, UfTiling til, int B, int H, int d, int n_rows, bool untile) {
+  const int lane = threadIdx.x & 31;
+  const int64_t wid = (int64_t)blockIdx.x * kTileWarps + (threadIdx.x >> 5);
+  if (wid >= (int64_t)n_rows * H) return;
+  const int R = (int)(wid / H), h = (int)(wid % H);
+  const int b = R / B, r = R % B;
+  int it, ih, iw;
+  uf_tile_coords(til, b, &it, &ih, &iw);
+  const int vh = min(til.bh, til.Hg - ih * til.bh), vw = min(til.bw, til.Wg - iw * til.bw);
+  const int nvalid = uf_tile_nvalid(til, b);
+  const int words = d / 2;
+  if (r >= nvalid) {
+    if (!untile) {
+      uint32_t* o = reinterpret_cast<uint32_t*>(dst + (int64_t)R * dst_ts + (int64_t)h * dst_hs);
+      for (int w = lane; w < words; w += 32) o[w] = 0u;
+    }
+    return;
+  }
+  const int dt = r / (vh * vw), dy = (r / vw) % vh, dx = r % vw;
+  const int64_t n = ((int64_t)(it * til.bt + dt) * til.Hg + (ih * til.bh + dy)) * til.Wg + (iw * til.bw + dx);
+  const int64_t tiled_off = (int64_t)R, raster_off = n;
+  const uint32_t* in = reinterpret_cast<const uint32_t*>(
+      src + (untile ? tiled_off : raster_off) * src_ts + (int64_t)h * src_hs);
+  uint32_t* out = reinterpret_cast<uint32_t*>(dst + (untile ? raster_off : tiled_off) * dst_ts + (int64_t)h * dst_hs);
+  for (int w = lane; w < words; w += 32) out[w] = in[w];
+}
+
 }  // namespace
+
+cudaError_t uf_launch_tile(uf_ctx* c, const __nv_bfloat16* src, __nv_bfloat16* dst, int64_t src_tok_stride,
+                           int64_t src_head_stride, int64_t dst_tok_stride, int64_t dst_head_stride, bool untile,
+                           cudaStream_t s) {
+  const UfTiling& t = c->til;
+  const int n_rows = t.nbt * t.nbh * t.nbw * c->cfg.block;
+  const int64_t warps = (int64_t)n_rows * c->cfg.n_heads;
+  uf_tile_kernel<<<(unsigned)((warps + kTileWarps - 1) / kTileWarps), kTileWarps * 32, 0, s>>>(
+      src, dst, src_tok_stride, src_head_stride, dst_tok_stride, dst_head_stride, t, c->cfg.block, c->cfg.n_heads,
+      c->cfg.head_dim, n_rows, untile);
+  c->launches += 1;
+  return cudaGetLastError();
+}
 
 cudaError_t uf_launch_append(uf_ctx* c, const UfView& v, const __nv_bfloat16* k, const __nv_bfloat16* vv,
                              int64_t tok_stride, int64_t head_stride, cudaStream_t s) {
@@ -89,7 +135,8 @@ cudaError_t uf_launch_append(uf_ctx* c, const UfView& v, const __nv_bfloat16* k,
 #define UF_APPEND_CASE(DD)                                                                              \
   case DD:                                                                                              \
     uf_append_kernel<DD><<<grid, kThreads, 0, s>>>(k, vv, tok_stride, head_stride, c->kc, c->vc,        \
-                                                   c->kpool, v.B, v.P, v.cur_ntok, phys0, sink_copy);   \
+                                                   c->kpool, v.B, v.P, v.cur_ntok, phys0, sink_copy,    \
+                                                   v.til);                                              \
     break;
   switch (v.d) {
     UF_APPEND_CASE(32)

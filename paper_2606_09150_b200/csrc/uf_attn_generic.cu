@@ -13,7 +13,8 @@ __global__ void __launch_bounds__(kWarps * 32)
 uf_attn_generic_kernel(UfView v, const __nv_bfloat16* __restrict__ q, __nv_bfloat16* __restrict__ o,
                        float* __restrict__ lse, int64_t tok_stride, int64_t head_stride,
                        const __nv_bfloat16* __restrict__ kc, const __nv_bfloat16* __restrict__ vc,
-                       const int32_t* __restrict__ sel_q, int kcap, int k_eff, float scale) {
+                       const int32_t* __restrict__ sel_q, const int32_t* __restrict__ sel_cnt, int kcap, int k_eff,
+                       float scale) {
   constexpr int EPL = D / 32;                 // elements per lane
   const int i = blockIdx.x, h = blockIdx.y;
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
@@ -22,7 +23,10 @@ uf_attn_generic_kernel(UfView v, const __nv_bfloat16* __restrict__ q, __nv_bfloa
   const int rows = min(B, v.cur_ntok - i * B);
   const float sl2 = scale * 1.4426950408889634f;      // logits are handled in the log2 domain
   const int32_t* list = sel_q + ((int64_t)h * v.BPC + i) * kcap;
-  const int n_steps = v.n_sink_blocks + k_eff + nqb;
+  // paper-mask mode (sel_cnt != null): only the row's own list (its length in sel_cnt), no SINK, no implicit CUR
+  if (sel_cnt) k_eff = sel_cnt[(int64_t)h * v.BPC + i];
+  const int n_sink = sel_cnt ? 0 : v.n_sink_blocks;
+  const int n_steps = n_sink + k_eff + (sel_cnt ? 0 : nqb);
   const int64_t head_base = (int64_t)h * v.P * B * D;
 
   for (int r = w; r < rows; r += kWarps) {
@@ -33,13 +37,13 @@ uf_attn_generic_kernel(UfView v, const __nv_bfloat16* __restrict__ q, __nv_bfloa
     float m = -INFINITY, l = 0.f;
     for (int st = 0; st < n_steps; ++st) {
       int phys, nvalid;
-      if (st < v.n_sink_blocks) {                               // SINK
+      if (st < n_sink) {                                        // SINK
         phys = st; nvalid = min(B, v.sink_ntok - st * B);
-      } else if (st < v.n_sink_blocks + k_eff) {                // TOPK[h, i]
-        const int32_t e = list[st - v.n_sink_blocks];
+      } else if (st < n_sink + k_eff) {                         // TOPK[h, i]
+        const int32_t e = list[st - n_sink];
         phys = uf_entry_phys(e); nvalid = uf_entry_nvalid(e);
       } else {                                                  // CUR
-        const int b = st - v.n_sink_blocks - k_eff;
+        const int b = st - n_sink - k_eff;
         phys = v.S + v.cur_slot * v.BPC + b; nvalid = min(B, v.cur_ntok - b * B);
       }
       const __nv_bfloat16* kb = kc + head_base + (int64_t)phys * B * D + lane * EPL;
@@ -77,7 +81,9 @@ cudaError_t uf_launch_attn_generic(uf_ctx* c, const UfView& v, const __nv_bfloat
 #define UF_GEN_CASE(DD)                                                                                     \
   case DD:                                                                                                  \
     uf_attn_generic_kernel<DD><<<grid, kWarps * 32, 0, s>>>(v, q, o, lse, tok_stride, head_stride, c->kc,   \
-                                                            c->vc, c->sel_q, c->kcap, c->sel_k, scale);     \
+                                                            c->vc, c->sel_q,                                \
+                                                            c->sel_paper ? c->sel_cnt : nullptr, c->kcap,   \
+                                                            c->sel_k, scale);                               \
     break;
   switch (v.d) {
     UF_GEN_CASE(32)

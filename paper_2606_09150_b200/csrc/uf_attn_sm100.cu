@@ -38,7 +38,9 @@
 // O_t += P_t V(prev) and may overwrite it).
 //
 // Key blocks of an item: first the merged TOPK union of the pair (per entry a 2-bit mask says which
-// tile attends it), then SINK, then CUR (both tiles).  All K/V come from the ctx cache.
+// tile attends it), then SINK, then CUR (both tiles).  All K/V come from the ctx cache.  In paper-mask
+// mode (uf_select_blocks_paper) there is no SINK and no implicit CUR: every kept block, the query
+// block's own included, is in the lists, with its valid-row count.
 #include "uf_internal.h"
 
 namespace {
@@ -348,6 +350,7 @@ struct AttnParams {
   int H, NP, kcap, np_cur;
   int ntok, nqb;
   int n_sink, sink_ntok;
+  int n_cur;                 // CUR blocks every query block attends implicitly (nqb; 0 in paper-mask mode: all in the lists)
   int cur_phys0;
   float sl2;                 // softmax scale * log2(e)
 };
@@ -454,7 +457,7 @@ uf_attn_sm100_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_cons
           for (int j = 0; j < cnt; ++j) load_kv(uf_entry_phys(__shfl_sync(0xffffffffu, mine, j)), h);
         }
         for (int j = 0; j < a.n_sink; ++j) load_kv(j, h);
-        for (int j = 0; j < a.nqb; ++j) load_kv(a.cur_phys0 + j, h);
+        for (int j = 0; j < a.n_cur; ++j) load_kv(a.cur_phys0 + j, h);
       UF_ITEM_LOOP_END
     } else if (warp == 9) {
       // ================================ MMA issuer ==================================
@@ -536,7 +539,7 @@ uf_attn_sm100_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_cons
           const int cnt = min(32, n_u - st0);
           for (int j = 0; j < cnt; ++j) step(uf_entry_mask(__shfl_sync(0xffffffffu, mine, j)));
         }
-        for (int j = 0; j < a.n_sink + a.nqb; ++j) step(full_mask);
+        for (int j = 0; j < a.n_sink + a.n_cur; ++j) step(full_mask);
 #pragma unroll
         for (int t = 0; t < 2; ++t) {
           if (pend[t]) do_pv(t);
@@ -693,7 +696,7 @@ uf_attn_sm100_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_cons
           if (msk & 1) softmax_step(0, m0, l0, d0, par0, first0, sph0, nvalid);
           if (msk & 2) softmax_step(1, m1, l1, d1, par1, first1, sph1, nvalid);
         }
-        for (int j = 0; j < a.n_sink + a.nqb; ++j) {
+        for (int j = 0; j < a.n_sink + a.n_cur; ++j) {
           const int nvalid = (j < a.n_sink) ? min(128, a.sink_ntok - j * 128) : min(128, a.ntok - (j - a.n_sink) * 128);
           softmax_step(0, m0, l0, d0, par0, first0, sph0, nvalid);
           if (full_mask & 2) softmax_step(1, m1, l1, d1, par1, first1, sph1, nvalid);
@@ -838,6 +841,7 @@ int uf_launch_attn_sm100(uf_ctx* c, const UfView& v, const __nv_bfloat16* q, __n
   a.H = v.H; a.NP = (v.BPC + 1) / 2; a.kcap = c->kcap;
   a.ntok = v.cur_ntok; a.nqb = uf_ceil_div(v.cur_ntok, 128); a.np_cur = (a.nqb + 1) / 2;
   a.n_sink = v.n_sink_blocks; a.sink_ntok = v.sink_ntok;
+  a.n_cur = c->sel_paper ? 0 : a.nqb;
   a.cur_phys0 = v.S + v.cur_slot * v.BPC;
   a.sl2 = scale * 1.4426950408889634f;
   const int n_items = a.H * a.np_cur;

@@ -31,8 +31,40 @@ __host__ __device__ inline int uf_entry_phys(int32_t e)   { return (int)((uint32
 __host__ __device__ inline int uf_entry_nvalid(int32_t e) { return (int)(((uint32_t)e >> 20) & 0xFFu) + 1; }
 __host__ __device__ inline int uf_entry_mask(int32_t e)   { return (int)(((uint32_t)e >> 28) & 0x3u); }
 
+// Paper-mask mode (R-29/R-30): every chunk is a (nbt x nbh x nbw) grid of (bt, bh, bw) tiles over an
+// (F, Hg, Wg) token grid; block b = (it*nbh + ih)*nbw + iw holds the tokens of its tile that exist, in
+// raster order, at rows [0, nvalid) of a B-row block (the caller's Q/K/V/O are in this tiled, padded layout).
+struct UfTiling {
+  int enabled;                    // 0: flat blocks of B consecutive tokens (BJ)
+  int F, Hg, Wg, bt, bh, bw;
+  int nbt, nbh, nbw;
+  int half;                       // (r - 1) / 2: M_local keeps |dih| <= half and |diw| <= half
+};
+__host__ __device__ inline void uf_tile_coords(const UfTiling& t, int b, int* it, int* ih, int* iw) {
+  *it = b / (t.nbh * t.nbw);
+  const int rem = b - *it * (t.nbh * t.nbw);
+  *ih = rem / t.nbw;
+  *iw = rem - *ih * t.nbw;
+}
+__host__ __device__ inline int uf_tile_nvalid(const UfTiling& t, int b) {
+  int it, ih, iw;
+  uf_tile_coords(t, b, &it, &ih, &iw);
+  const int vt = t.F - it * t.bt < t.bt ? t.F - it * t.bt : t.bt;
+  const int vh = t.Hg - ih * t.bh < t.bh ? t.Hg - ih * t.bh : t.bh;
+  const int vw = t.Wg - iw * t.bw < t.bw ? t.Wg - iw * t.bw : t.bw;
+  return vt * vh * vw;
+}
+__host__ __device__ inline bool uf_tile_local(const UfTiling& t, int bi, int bj) {
+  int ti, hi, wi, tj, hj, wj;
+  uf_tile_coords(t, bi, &ti, &hi, &wi);
+  uf_tile_coords(t, bj, &tj, &hj, &wj);
+  const int dh = hi > hj ? hi - hj : hj - hi, dw = wi > wj ? wi - wj : wj - wi;
+  return dh <= t.half && dw <= t.half;
+}
+
 // Snapshot of the cache state for one step, passed by value to kernels.
 struct UfView {
+  UfTiling til;
   int H, d, B, BPC, S, P;
   int n_prior;                    // resident chunks older than the current one, ascending id
   int prior_chunk[UF_MAXC];       // chunk id
@@ -56,7 +88,14 @@ __host__ __device__ inline void uf_cand_lookup(const UfView& v, int j, int* g, i
   *g = v.prior_chunk[i] * v.BPC + b;
   *phys = v.S + v.prior_slot[i] * v.BPC + b;
   int rem = v.prior_ntok[i] - b * v.B;
-  *nvalid = rem < v.B ? rem : v.B;
+  *nvalid = v.til.enabled ? uf_tile_nvalid(v.til, b) : (rem < v.B ? rem : v.B);
+}
+
+// valid rows of block b of the current chunk
+__host__ __device__ inline int uf_cur_nvalid(const UfView& v, int b) {
+  if (v.til.enabled) return uf_tile_nvalid(v.til, b);
+  const int rem = v.cur_ntok - b * v.B;
+  return rem < v.B ? rem : v.B;
 }
 
 struct uf_ctx {
@@ -72,6 +111,9 @@ struct uf_ctx {
   int32_t* sel_rank = nullptr;    // candidate index of every sel_q entry (merge key); [H][BPC][kcap]
   int32_t* sel_pair = nullptr;    // per (h, q-block pair): merged union list with tile masks; [H][NP][2*kcap]
   int32_t* pair_cnt = nullptr;    // [H][NP]
+  int32_t* sel_cnt = nullptr;     // [H][BPC]: entries of every sel_q row (paper-mask mode: rows differ in length)
+  UfTiling til = {};              // paper-mask mode when til.enabled
+  bool sel_paper = false;         // the stored selection came from uf_select_blocks_paper
   int32_t* panic_item = nullptr;  // [H][NP]: == attn_seq when the safe attention kernel must redo the item
   int32_t* panic_last = nullptr;  // [1]: == attn_seq when the last fast launch flagged anything
   int32_t attn_seq = 0;           // sm100 attention launch sequence number
@@ -96,16 +138,22 @@ struct uf_ctx {
   static constexpr int kTmCache = 8;
   TmEntry tm_cache[kTmCache];
   int tm_cache_n = 0, tm_cache_next = 0;
-  size_t score_smem_attr[3][4] = {};   // dynamic-smem limit already set on uf_score_topk_kernel<d, QG>
+  size_t score_smem_attr[2][3][4] = {};   // dynamic-smem limit already set on uf_score_topk_kernel<d, QG>
   std::string err;
 };
 
 // --- kernels (each launcher returns cudaGetLastError()) -------------------------------------------
 cudaError_t uf_launch_append(uf_ctx* c, const UfView& v, const __nv_bfloat16* k, const __nv_bfloat16* vv,
                              int64_t tok_stride, int64_t head_stride, cudaStream_t s);
+// paper: Eq. 4 mode (candidates include the current chunk, top-k then M_local, own block always kept;
+// idx_out rows are out_stride entries long, padded with -1)
 cudaError_t uf_launch_select(uf_ctx* c, const UfView& v, const __nv_bfloat16* q, int64_t tok_stride,
                              int64_t head_stride, int k_eff, int32_t* idx_out, int32_t* cnt_out,
-                             cudaStream_t s);
+                             bool paper, int out_stride, cudaStream_t s);
+// raster [F*Hg*Wg, H, d] <-> tiled, padded [NB*B, H, d] (pad rows zero)
+cudaError_t uf_launch_tile(uf_ctx* c, const __nv_bfloat16* src, __nv_bfloat16* dst, int64_t src_tok_stride,
+                           int64_t src_head_stride, int64_t dst_tok_stride, int64_t dst_head_stride, bool untile,
+                           cudaStream_t s);
 cudaError_t uf_launch_attn_generic(uf_ctx* c, const UfView& v, const __nv_bfloat16* q, __nv_bfloat16* o,
                                    float* lse, int64_t tok_stride, int64_t head_stride, float scale,
                                    cudaStream_t s);

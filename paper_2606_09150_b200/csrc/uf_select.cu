@@ -23,14 +23,14 @@ __device__ __forceinline__ uint4 ld_stream(const uint4* p) {
 template <int D>
 __global__ void __launch_bounds__(kPoolThreads)
 uf_pool_q_kernel(const __nv_bfloat16* __restrict__ q, int64_t tok_stride, int64_t head_stride,
-                 double* __restrict__ qbar, int B, int BPC, int ntok) {
+                 double* __restrict__ qbar, int B, int BPC, int ntok, UfTiling til) {
   constexpr int VPR = D / 8;
   constexpr int RPP = kPoolThreads / VPR;
   __shared__ double red[RPP][D + 2];
   const int i = blockIdx.x, h = blockIdx.y;
   const int vcx = threadIdx.x % VPR, rg = threadIdx.x / VPR;
   const int row0 = i * B;
-  const int nvalid = min(B, ntok - row0);
+  const int nvalid = til.enabled ? uf_tile_nvalid(til, i) : min(B, ntok - row0);
   double acc[8];
 #pragma unroll
   for (int t = 0; t < 8; ++t) acc[t] = 0.0;
@@ -65,11 +65,16 @@ __device__ __forceinline__ unsigned long long sortable(double x) {
 // ---- a3 + a4: scores and top-k.  grid (ceil(nqb / kQG), H) ------------------------------------------
 // kQG query blocks are scored per CTA (each pooled-K load is re-used kQG times).
 // dynamic smem: double qs[kQG][D]; unsigned long long key[kQG][n_cand]
-template <int D, int kQG>
+// kPaper (Eq. 4 as written; R-32/R-33): the candidates are ALL blocks in the causal mask (the view lists the
+// current chunk as its last "prior"), the top-k' is taken over all of them and THEN intersected with the r x r
+// window M_local; the query block's own key block is always kept.  Rows then differ in length: sel_cnt holds
+// each row's count and idx_out rows (out_stride entries) are padded with -1.
+template <int D, int kQG, bool kPaper>
 __global__ void __launch_bounds__(kScoreThreads)
 uf_score_topk_kernel(UfView v, const double* __restrict__ qbar, const double* __restrict__ kpool,
                      int nqb, int k_eff, int32_t* __restrict__ sel_q, int32_t* __restrict__ sel_rank, int kcap,
-                     int32_t* __restrict__ idx_out, int32_t* __restrict__ cnt_out) {
+                     int32_t* __restrict__ sel_cnt, int32_t* __restrict__ idx_out, int32_t* __restrict__ cnt_out,
+                     int out_stride) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   double* qs = reinterpret_cast<double*>(smem_raw);                                  // [kQG][D]
   unsigned long long* key = reinterpret_cast<unsigned long long*>(qs + kQG * D);     // [kQG][n_cand]
@@ -155,20 +160,30 @@ uf_score_topk_kernel(UfView v, const double* __restrict__ qbar, const double* __
       const unsigned long long mine = j < nc ? kg[j] : 0ull;
       const bool gt = j < nc && mine > T, eq = j < nc && mine == T;
       const unsigned beq = __ballot_sync(0xffffffffu, eq);
-      const bool keep = gt || (eq && eq_seen + __popc(beq & ((1u << lane) - 1u)) < need_eq);
+      bool keep = gt || (eq && eq_seen + __popc(beq & ((1u << lane) - 1u)) < need_eq);
+      int gid = 0, phys = 0, nval = 1;
+      if (kPaper && j < nc) {
+        uf_cand_lookup(v, j, &gid, &phys, &nval);
+        const int bj = gid % v.BPC;                    // block of its chunk (every chunk has the same tile grid)
+        keep = (keep && uf_tile_local(v.til, i, bj)) || gid == v.cur_chunk * v.BPC + i;
+      }
       const unsigned ball = __ballot_sync(0xffffffffu, keep);
       if (keep) {
         const int pos = pos0 + __popc(ball & ((1u << lane) - 1u));
-        int gid, phys, nval;
-        uf_cand_lookup(v, j, &gid, &phys, &nval);
+        if (!kPaper) uf_cand_lookup(v, j, &gid, &phys, &nval);
         sel_q[rowq + pos] = uf_entry_pack(phys, nval, 0);
         sel_rank[rowq + pos] = j;                      // candidate index: the merge key
-        if (idx_out) idx_out[((int64_t)h * nqb + i) * k_eff + pos] = gid;
+        if (idx_out) idx_out[((int64_t)h * nqb + i) * out_stride + pos] = gid;
       }
       pos0 += __popc(ball);
       eq_seen += __popc(beq);
     }
-    if (lane == 0 && cnt_out) cnt_out[(int64_t)h * nqb + i] = k_eff;
+    if (kPaper) {
+      if (idx_out)
+        for (int x = pos0 + lane; x < out_stride; x += 32) idx_out[((int64_t)h * nqb + i) * out_stride + x] = -1;
+      if (lane == 0) sel_cnt[(int64_t)h * v.BPC + i] = pos0;
+    }
+    if (lane == 0 && cnt_out) cnt_out[(int64_t)h * nqb + i] = kPaper ? pos0 : k_eff;
   }
 }
 
@@ -182,8 +197,8 @@ uf_score_topk_kernel(UfView v, const double* __restrict__ qbar, const double* __
 // block, valid rows) is recomputed from the candidate index.  dynamic smem: uint32 [warps][2][ceil(n_cand / 32)]
 constexpr int kMergeWarps = 4;
 __global__ void __launch_bounds__(kMergeWarps * 32)
-uf_pair_merge_kernel(UfView v, const int32_t* __restrict__ sel_rank, int32_t* __restrict__ sel_pair,
-                     int32_t* __restrict__ pair_cnt, int nqb, int k_eff, int kcap) {
+uf_pair_merge_kernel(UfView v, const int32_t* __restrict__ sel_rank, const int32_t* __restrict__ sel_cnt,
+                     int32_t* __restrict__ sel_pair, int32_t* __restrict__ pair_cnt, int nqb, int k_eff, int kcap) {
   extern __shared__ uint32_t bm_raw[];
   const int NP = (v.BPC + 1) / 2;
   const int np_cur = (nqb + 1) / 2;
@@ -199,10 +214,15 @@ uf_pair_merge_kernel(UfView v, const int32_t* __restrict__ sel_rank, int32_t* __
   const int32_t* ra = sel_rank + ((int64_t)h * v.BPC + 2 * p) * kcap;
   const int32_t* rb = ra + kcap;
   const bool has1 = 2 * p + 1 < nqb;
-  for (int e = lane; e < k_eff; e += 32) {
-    const int ja = ra[e];
-    atomicOr(&bma[ja >> 5], 1u << (ja & 31));
-    if (has1) {
+  // rows of equal length k_eff (flat mode) or of their own length (paper-mask mode: sel_cnt)
+  const int na = sel_cnt ? sel_cnt[(int64_t)h * v.BPC + 2 * p] : k_eff;
+  const int nb = !has1 ? 0 : (sel_cnt ? sel_cnt[(int64_t)h * v.BPC + 2 * p + 1] : k_eff);
+  for (int e = lane; e < max(na, nb); e += 32) {
+    if (e < na) {
+      const int ja = ra[e];
+      atomicOr(&bma[ja >> 5], 1u << (ja & 31));
+    }
+    if (e < nb) {
       const int jb = rb[e];
       atomicOr(&bmb[jb >> 5], 1u << (jb & 31));
     }
@@ -255,10 +275,10 @@ uf_pair_merge_kernel(UfView v, const int32_t* __restrict__ sel_rank, int32_t* __
 
 cudaError_t uf_launch_select(uf_ctx* c, const UfView& v, const __nv_bfloat16* q, int64_t tok_stride,
                              int64_t head_stride, int k_eff, int32_t* idx_out, int32_t* cnt_out,
-                             cudaStream_t s) {
+                             bool paper, int out_stride, cudaStream_t s) {
   const int nqb = uf_ceil_div(v.cur_ntok, v.B);
   const int NP = (v.BPC + 1) / 2;
-  if (k_eff == 0) {
+  if (k_eff == 0 && !paper) {
     // no candidates (chunk 0, or window 1): counts are zero, nothing to score
     if (cnt_out) {
       cudaError_t e = cudaMemsetAsync(cnt_out, 0, (size_t)v.H * nqb * sizeof(int32_t), s);
@@ -274,22 +294,28 @@ cudaError_t uf_launch_select(uf_ctx* c, const UfView& v, const __nv_bfloat16* q,
   const size_t smem = smem_for(qg);
   if (smem > 200 * 1024) return cudaErrorInvalidConfiguration;     // > ~25k candidates: not supported
   dim3 gs(uf_ceil_div(nqb, qg), v.H);
-#define UF_SCORE_LAUNCH(DD, QG)                                                                              \
+#define UF_SCORE_LAUNCH2(DD, QG, PP)                                                                         \
   {                                                                                                          \
-    size_t& attr = c->score_smem_attr[DD == 32 ? 0 : DD == 64 ? 1 : 2][QG == 8 ? 0 : QG == 4 ? 1 : QG == 2 ? 2 : 3]; \
+    size_t& attr = c->score_smem_attr[PP ? 1 : 0][DD == 32 ? 0 : DD == 64 ? 1 : 2]                           \
+                                     [QG == 8 ? 0 : QG == 4 ? 1 : QG == 2 ? 2 : 3];                          \
     if (smem > 48 * 1024 && smem > attr) {          /* raise the limit once, not on every call */             \
-      e = cudaFuncSetAttribute(uf_score_topk_kernel<DD, QG>, cudaFuncAttributeMaxDynamicSharedMemorySize,    \
+      e = cudaFuncSetAttribute(uf_score_topk_kernel<DD, QG, PP>, cudaFuncAttributeMaxDynamicSharedMemorySize,\
                                (int)smem);                                                                   \
       if (e != cudaSuccess) return e;                                                                        \
       attr = smem;                                                                                           \
     }                                                                                                        \
-    uf_score_topk_kernel<DD, QG><<<gs, kScoreThreads, smem, s>>>(v, c->qbar, c->kpool, nqb, k_eff, c->sel_q, \
-                                                                 c->sel_rank, c->kcap, idx_out, cnt_out);    \
+    uf_score_topk_kernel<DD, QG, PP><<<gs, kScoreThreads, smem, s>>>(                                        \
+        v, c->qbar, c->kpool, nqb, k_eff, c->sel_q, c->sel_rank, c->kcap, c->sel_cnt, idx_out, cnt_out,      \
+        out_stride);                                                                                         \
+  }
+#define UF_SCORE_LAUNCH(DD, QG)                                                                              \
+  {                                                                                                          \
+    if (paper) UF_SCORE_LAUNCH2(DD, QG, true) else UF_SCORE_LAUNCH2(DD, QG, false)                           \
   }
 #define UF_SELECT_CASE(DD)                                                                                   \
   case DD:                                                                                                   \
     uf_pool_q_kernel<DD><<<gp, kPoolThreads, 0, s>>>(q, tok_stride, head_stride, c->qbar, v.B, v.BPC,        \
-                                                     v.cur_ntok);                                            \
+                                                     v.cur_ntok, v.til);                                     \
     if (qg == 8) UF_SCORE_LAUNCH(DD, 8)                                                                      \
     else if (qg == 4) UF_SCORE_LAUNCH(DD, 4)                                                                 \
     else if (qg == 2) UF_SCORE_LAUNCH(DD, 2)                                                                 \
@@ -303,6 +329,7 @@ cudaError_t uf_launch_select(uf_ctx* c, const UfView& v, const __nv_bfloat16* q,
   }
 #undef UF_SELECT_CASE
 #undef UF_SCORE_LAUNCH
+#undef UF_SCORE_LAUNCH2
   c->launches += 2;
   e = cudaGetLastError();
   if (e != cudaSuccess) return e;
@@ -310,7 +337,7 @@ cudaError_t uf_launch_select(uf_ctx* c, const UfView& v, const __nv_bfloat16* q,
     const int np_cur = (nqb + 1) / 2;
     const size_t msmem = (size_t)kMergeWarps * 2 * uf_ceil_div(v.n_cand, 32) * sizeof(uint32_t);
     uf_pair_merge_kernel<<<uf_ceil_div(v.H * np_cur, kMergeWarps), kMergeWarps * 32, msmem, s>>>(
-        v, c->sel_rank, c->sel_pair, c->pair_cnt, nqb, k_eff, c->kcap);
+        v, c->sel_rank, paper ? c->sel_cnt : nullptr, c->sel_pair, c->pair_cnt, nqb, k_eff, c->kcap);
     c->launches += 1;
     e = cudaGetLastError();
   }

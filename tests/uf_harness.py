@@ -8,6 +8,7 @@ import numpy as np
 
 import uf_workloads as wl
 from oracle.uf_oracle import UFOracle
+from oracle.uf_paper_mask import UFPaperOracle
 
 # BASELINE.json north_star: attention outputs within max-abs 2e-2 and mean-abs 2e-3 of the fp64 oracle
 O_MAX_ABS = 2e-2
@@ -144,3 +145,108 @@ def compare_step(got: dict, ref: dict, where: str = "", o_max_abs: float = O_MAX
             assert lerr.max() <= LSE_MAX_ABS, f"{where} LSE max-abs {lerr.max():.3e} > {LSE_MAX_ABS}"
         return float(err.max()), float(err.mean())
     return None
+
+
+# ------------------------------------------------------------------------------------ paper-mask mode (NEXT-1)
+def tiled_rows(w: wl.Workload) -> np.ndarray:
+    """The ABI's tiled layout (include/uf.h, uf_tiling), written out independently of both implementations: raster token
+    index of every tiled row, -1 for pad rows.  int64 [N_b * block]."""
+    bt, bh, bw = w.tile
+    F, Hg, Wg = w.frames_per_chunk, w.grid_h, w.grid_w
+    nbt, nbh, nbw = w.tile_grid
+    out = np.full(nbt * nbh * nbw * w.block, -1, dtype=np.int64)
+    b = 0
+    for it in range(nbt):
+        for ih in range(nbh):
+            for iw in range(nbw):
+                t, y, x = np.meshgrid(np.arange(it * bt, min((it + 1) * bt, F)), np.arange(ih * bh, min((ih + 1) * bh, Hg)),
+                                      np.arange(iw * bw, min((iw + 1) * bw, Wg)), indexing="ij")
+                n = ((t * Hg + y) * Wg + x).reshape(-1)
+                out[b * w.block:b * w.block + n.size] = n
+                b += 1
+    return out
+
+
+class PaperCudaStream:
+    """A tiled ctx (uf_ctx_set_tiling): raster chunks in, raster outputs back; every step through the C ABI, the
+    raster <-> tiled conversion included (uf_tile_tokens / uf_untile_tokens)."""
+
+    def __init__(self, w: wl.Workload, device: int = 0):
+        import torch
+        import paper_2606_09150_b200 as uf
+        self.torch, self.uf, self.w = torch, uf, w
+        self.dev = torch.device("cuda", device)
+        self.nt = w.n_tiles * w.block
+        self.ctx = uf.uf_ctx_create(w.n_heads, w.head_dim, w.block, self.nt, w.capacity_chunks, 0, w.k_min, device)
+        uf.uf_ctx_set_tiling(self.ctx, w.frames_per_chunk, w.grid_h, w.grid_w, *w.tile, w.window)
+        self.stream = torch.cuda.current_stream(self.dev)
+        self.rows = tiled_rows(w)
+
+    def close(self):
+        if self.ctx is not None:
+            self.uf.uf_ctx_destroy(self.ctx)
+            self.ctx = None
+
+    def tile(self, bits: np.ndarray):
+        torch, w = self.torch, self.w
+        n, H, d = bits.shape
+        src = torch.from_numpy(bits.view(np.int16)).to(self.dev).view(torch.bfloat16)
+        dst = torch.full((self.nt, H, d), float("nan"), dtype=torch.bfloat16, device=self.dev)
+        self.uf.uf_tile_tokens(self.ctx, src, dst, H * d, d, H * d, d, self.stream)
+        return dst
+
+    def step(self, Qb, Kb, Vb, topk_count=-1, rho_permille=1000, window=0, impl=0, scale=0.0):
+        torch, uf, w = self.torch, self.uf, self.w
+        n, H, d = Qb.shape
+        q, k, v = self.tile(Qb), self.tile(Kb), self.tile(Vb)
+        ts, hs = H * d, d
+        uf.uf_kv_append(self.ctx, k, v, self.nt, ts, hs, window, self.stream)
+        slot_map = uf.uf_get_slot_map(self.ctx, w.capacity_chunks)
+        n_blocks, k_eff = uf.uf_query_budget_paper(self.ctx, topk_count, rho_permille)
+        stride = min(k_eff + 1, n_blocks)
+        NB = w.n_tiles
+        idx = torch.full((H, NB, stride), -7, dtype=torch.int32, device=self.dev)
+        cnt = torch.full((H, NB), -7, dtype=torch.int32, device=self.dev)
+        uf.uf_select_blocks_paper(self.ctx, q, self.nt, ts, hs, topk_count, rho_permille, idx, stride, cnt, self.stream)
+        o = torch.full((self.nt, H, d), float("nan"), dtype=torch.bfloat16, device=self.dev)
+        lse = torch.full((H, self.nt), float("nan"), dtype=torch.float32, device=self.dev)
+        uf.uf_set_attn_impl(self.ctx, impl)
+        uf.uf_sparse_attn_fwd(self.ctx, q, o, lse, self.nt, ts, hs, scale, self.stream)
+        o_r = torch.full((n, H, d), float("nan"), dtype=torch.bfloat16, device=self.dev)
+        uf.uf_untile_tokens(self.ctx, o, o_r, ts, hs, ts, hs, self.stream)
+        torch.cuda.synchronize(self.dev)
+        lse_t = lse.cpu().numpy()
+        lse_r = np.full((H, n), np.nan, dtype=np.float32)
+        valid = self.rows >= 0
+        lse_r[:, self.rows[valid]] = lse_t[:, valid]
+        return {"slot_map": slot_map, "n_cand": n_blocks, "k_eff": k_eff, "idx": idx.cpu().numpy(),
+                "cnt": cnt.cpu().numpy(), "O": o_r.float().cpu().numpy(), "lse": lse_r,
+                "O_tiled": o, "q_tiled": q}
+
+
+def make_paper_oracle(w: wl.Workload) -> UFPaperOracle:
+    return UFPaperOracle(w.n_heads, w.head_dim, w.frames_per_chunk, w.grid_h, w.grid_w, w.capacity_chunks,
+                         block=w.tile, window=w.window, k_min=w.k_min)
+
+
+def paper_oracle_step(orc: UFPaperOracle, Qb, Kb, Vb, topk_count=-1, rho_permille=1000, window=0, heads=None,
+                      qblocks=None, scale=0.0, attn=True):
+    Q, K, V = bits_to_f64(Qb), bits_to_f64(Kb), bits_to_f64(Vb)
+    orc.kv_append(K, V, window)
+    idx, cnt = orc.select_blocks(Q, topk_count, rho_permille)
+    out = {"slot_map": orc.slot_map(), "idx": idx, "cnt": cnt}
+    if attn:
+        out["O"], out["lse"] = orc.sparse_attn(Q, heads=heads, qblocks=qblocks, softmax_scale=scale)
+    return out
+
+
+def compare_paper_step(got: dict, ref: dict, where: str = ""):
+    """idx rows: the oracle pads to its own longest row, the CUDA path to the stride the caller gave: compare the
+    common prefix and require -1 beyond."""
+    kmax = ref["idx"].shape[2]
+    g = got["idx"]
+    assert g.shape[2] >= kmax, f"{where} idx stride {g.shape[2]} < longest oracle row {kmax}"
+    assert (g[:, :, kmax:] == -1).all(), f"{where} entries beyond the longest oracle row must be -1"
+    got2 = dict(got)
+    got2["idx"] = g[:, :, :kmax]
+    return compare_step(got2, ref, where)

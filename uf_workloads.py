@@ -37,6 +37,21 @@ class Workload:
     sink_blocks: int = 1
     k_min: int = 4                 # PAPER.md:818 (k_min = 4), floor in percent mode only
     n_stream_chunks: int = 0       # >0: rolling-stream config (config 3)
+    # paper-mask variants: 3-D tiles of the chunk's token grid, r x r block window, rho
+    tile: tuple | None = None      # (b_t, b_h, b_w), PAPER.md:343 (2, 8, 8); None = flat blocks (BASELINE.json)
+    window: int = 9                # PAPER.md:343 "local window 9 x 9"
+    rho_permille: int = 1000       # PAPER.md:343 rho = 1.0
+
+    @property
+    def tile_grid(self) -> tuple[int, int, int]:
+        """(nbt, nbh, nbw): tiles per chunk along t, y, x (edge tiles ragged)"""
+        bt, bh, bw = self.tile
+        return -(-self.frames_per_chunk // bt), -(-self.grid_h // bh), -(-self.grid_w // bw)
+
+    @property
+    def n_tiles(self) -> int:
+        a, b, c = self.tile_grid
+        return a * b * c
 
     @property
     def chunk_tokens(self) -> int:
@@ -73,6 +88,13 @@ CONFIGS: dict[str, Workload] = {
     # configs[4]: wide model, 40 heads, 2 prior chunks + sink, top 20 %, amplitude 3
     "wide": Workload("wide", 40, 128, 128, 3, _G1K[0], _G1K[1], capacity_chunks=3, prior_chunks=2,
                      topk_count=-1, topk_percent=20, amp=3.0),
+    # paper-mask variants of configs[1] / configs[2]: same grids, heads, chunking and cache as BASELINE.json, but the
+    # mask of PAPER.md section 2.3.1 (tiles (2,8,8), 9 x 9 window as an intersection, budget from the repaired Eq. 10
+    # at rho = 1.0, no sink).  1K: 2 x 9 x 15 = 270 tiles per chunk, 2K: 2 x 12 x 20 = 480.
+    "1k_paper": Workload("1k_paper", 12, 128, 128, 3, _G1K[0], _G1K[1], capacity_chunks=2, prior_chunks=1,
+                         topk_count=-1, topk_percent=-1, amp=2.0, sink_blocks=0, tile=(2, 8, 8)),
+    "2k_paper": Workload("2k_paper", 12, 128, 128, 3, _G2K[0], _G2K[1], capacity_chunks=3, prior_chunks=2,
+                         topk_count=-1, topk_percent=-1, amp=2.0, sink_blocks=0, tile=(2, 8, 8)),
 }
 
 
