@@ -30,11 +30,40 @@ if ROOT not in sys.path:
 
 import uf_workloads as wl  # noqa: E402
 
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE uf_attn_sm100_kernel<false> launch, from the committed
-# `ncu --set full` capture of this command (profiles/r1e_ncu_full_all_kernels.txt, command in profiles/README.md);
-# null for workloads not captured.
-NCU_ATTN_DRAM_BYTES = {"1k": 476.457984e6 + 66.498048e6,      # profiles/r1e_ncu_full_all_kernels.txt
-                       "2k": 1.735499e9 + 131.152896e6}        # profiles/r1e_2k_attn_sm100_ncu_full.txt
+PROFILE_TRAFFIC = os.path.join(ROOT, "profiles", "attn_dram_traffic.txt")
+KERNEL_SOURCES = ["include/uf.h"] + ["paper_2606_09150_b200/csrc/" + f for f in (
+    "uf_internal.h", "uf_api.cu", "uf_append.cu", "uf_select.cu", "uf_attn_generic.cu", "uf_attn_sm100.cu")]
+
+
+def kernel_source_hash() -> str:
+    """sha256 over the CUDA sources + the ABI header: ties an ncu capture under profiles/ to the code it profiled."""
+    import hashlib
+    h = hashlib.sha256()
+    for rel in KERNEL_SOURCES:
+        with open(os.path.join(ROOT, rel), "rb") as f:
+            h.update(rel.encode() + b"\0" + f.read())
+    return h.hexdigest()
+
+
+def ncu_attn_dram_bytes(workload: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum of ONE uf_attn_sm100_kernel<false> launch, read from the
+    committed summary of an `ncu --set full` capture (profiles/attn_dram_traffic.txt: `key: value` lines, the command
+    that made it, and the sha256 of the sources it profiled).  None when there is no capture of this workload or when
+    the sources have changed since: a stale number is not reported."""
+    try:
+        kv = {}
+        for line in open(PROFILE_TRAFFIC):
+            if ":" in line and not line.startswith("#"):
+                k, v = line.split(":", 1)
+                kv[k.strip()] = v.strip()
+        if kv.get("source_sha256") != kernel_source_hash():
+            return None, "capture is of other sources (profiles/attn_dram_traffic.txt): not reported"
+        if workload not in kv:
+            return None, "no capture of this workload"
+        return float(kv[workload]), "ncu --set full capture, profiles/attn_dram_traffic.txt (sources match)"
+    except OSError:
+        return None, "no capture committed"
+
 
 METRIC = "effective TFLOP/s on kept blocks, sparse causal chunk attention step (ms/chunk in ms_per_step)"
 UNIT = "TFLOP/s"
@@ -151,45 +180,86 @@ def barrier():
 
 
 # --------------------------------------------------------------------------------------------------
-class HotPath:
-    """The step bench.py times: uf_kv_append -> uf_select_blocks -> uf_sparse_attn_fwd via the C ABI."""
+_CHUNKS: dict = {}
 
-    def __init__(self, w: wl.Workload, device: int, n_distinct: int):
+
+def get_chunks(w: wl.Workload, ids):
+    """Seeded chunks (bf16 bits) of a workload, generated on a thread pool and shared between workloads that have
+    the same recipe (1k / 1k_stream / 1k_paper draw identical chunks: same grid, heads, amplitude, seeds)."""
+    from concurrent.futures import ThreadPoolExecutor
+    key = lambda c: (w.n_heads, w.head_dim, w.frames_per_chunk, w.grid_h, w.grid_w, w.amp, c)  # noqa: E731
+    todo = [c for c in ids if key(c) not in _CHUNKS]
+    if todo:
+        with ThreadPoolExecutor(min(8, len(todo))) as ex:
+            for c, ch in zip(todo, ex.map(lambda c: wl.make_chunk(w, c), todo)):
+                _CHUNKS[key(c)] = ch
+    return [_CHUNKS[key(c)] for c in ids]
+
+
+def tile_sizes(w: wl.Workload) -> np.ndarray:
+    """valid tokens of every tile of a chunk (paper-mask workloads), tile-major: bookkeeping for the FLOP count"""
+    bt, bh, bw = w.tile
+    vt = np.minimum(bt, w.frames_per_chunk - np.arange(w.tile_grid[0]) * bt)
+    vh = np.minimum(bh, w.grid_h - np.arange(w.tile_grid[1]) * bh)
+    vw = np.minimum(bw, w.grid_w - np.arange(w.tile_grid[2]) * bw)
+    return (vt[:, None, None] * vh[None, :, None] * vw[None, None, :]).reshape(-1).astype(np.int64)
+
+
+class HotPath:
+    """The step bench.py times: uf_kv_append -> uf_select_blocks -> uf_sparse_attn_fwd via the C ABI
+    (paper-mask workloads: a tiled ctx, uf_select_blocks_paper, chunks converted once by uf_tile_tokens)."""
+
+    def __init__(self, w: wl.Workload, device: int, chunk_ids, pinned_host: bool):
         import torch
         import paper_2606_09150_b200 as uf
         self.torch, self.uf, self.w = torch, uf, w
         self.dev = torch.device("cuda", device)
         torch.cuda.set_device(self.dev)
-        self.ctx = uf.uf_ctx_create(w.n_heads, w.head_dim, w.block, w.chunk_tokens, w.capacity_chunks,
-                                    w.sink_blocks, w.k_min, device)
+        self.paper = w.tile is not None
+        self.H, self.d = w.n_heads, w.head_dim
+        self.n = w.n_tiles * w.block if self.paper else w.chunk_tokens      # rows the library sees per chunk
+        self.ctx = uf.uf_ctx_create(w.n_heads, w.head_dim, w.block, self.n, w.capacity_chunks,
+                                    0 if self.paper else w.sink_blocks, w.k_min, device)
         self.stream = torch.cuda.current_stream(self.dev)
-        self.n, self.H, self.d = w.chunk_tokens, w.n_heads, w.head_dim
+        if self.paper:
+            uf.uf_ctx_set_tiling(self.ctx, w.frames_per_chunk, w.grid_h, w.grid_w, *w.tile, w.window)
         self.ts, self.hs = self.H * self.d, self.d
-        self.host = []      # pinned host chunks (int16 views of bf16 bits)
+        self.host = []      # pinned host chunks (int16 views of bf16 bits), only for the e2e leg
         self.devc = []      # device-resident chunks
-        for c in range(n_distinct):
-            qb, kb, vb = wl.make_chunk(w, c)
-            hq, hk, hv = (torch.from_numpy(x.view(np.int16)).pin_memory() for x in (qb, kb, vb))
-            self.host.append((hq, hk, hv))
-            self.devc.append(tuple(t.to(self.dev, non_blocking=True).view(torch.bfloat16) for t in (hq, hk, hv)))
+        for qb, kb, vb in get_chunks(w, chunk_ids):
+            hq, hk, hv = (torch.from_numpy(x.view(np.int16)) for x in (qb, kb, vb))
+            if pinned_host:
+                hq, hk, hv = hq.pin_memory(), hk.pin_memory(), hv.pin_memory()
+                self.host.append((hq, hk, hv))
+            dq, dk, dv = (t.to(self.dev, non_blocking=True).view(torch.bfloat16) for t in (hq, hk, hv))
+            if self.paper:
+                tiled = []
+                for t in (dq, dk, dv):
+                    o = torch.empty((self.n, self.H, self.d), dtype=torch.bfloat16, device=self.dev)
+                    uf.uf_tile_tokens(self.ctx, t, o, self.ts, self.hs, self.ts, self.hs, self.stream)
+                    tiled.append(o)
+                dq, dk, dv = tiled
+            self.devc.append((dq, dk, dv))
         nqb = -(-self.n // w.block)
-        kmax = max(1, (w.capacity_chunks - 1) * w.bpc)
+        kmax = max(1, w.capacity_chunks * w.bpc if not self.paper else w.capacity_chunks * w.n_tiles)
         self.idx = torch.zeros((self.H, nqb, kmax), dtype=torch.int32, device=self.dev)
         self.cnt = torch.zeros((self.H, nqb), dtype=torch.int32, device=self.dev)
+        self.idx_stride = kmax
         self.o = torch.zeros((self.n, self.H, self.d), dtype=torch.bfloat16, device=self.dev)
         self.lse = torch.zeros((self.H, self.n), dtype=torch.float32, device=self.dev)
-        # e2e staging: device inputs filled by H2D, pinned host output
-        # two sets (double buffering): while step i computes, step i+1's inputs arrive and step i-1's O leaves
-        mk = lambda: torch.empty((self.n, self.H, self.d), dtype=torch.bfloat16, device=self.dev)  # noqa: E731
-        self.stage = [tuple(mk() for _ in range(3)) for _ in range(2)]
-        self.o_e2e = [mk() for _ in range(2)]
-        self.o_host = [torch.empty((self.n, self.H, self.d), dtype=torch.bfloat16).pin_memory() for _ in range(2)]
-        self.s_in, self.s_out = torch.cuda.Stream(self.dev), torch.cuda.Stream(self.dev)
-        E = lambda: torch.cuda.Event()  # noqa: E731
-        self.ev_in = [E(), E()]      # inputs of set b are on the device
-        self.ev_free = [E(), E()]    # the step that read set b's inputs has finished
-        self.ev_done = [E(), E()]    # O of set b is complete
-        self.ev_out = [E(), E()]     # O of set b has been copied to the host
+        if pinned_host:
+            # e2e staging: two sets (double buffering): while step i computes, step i+1's inputs arrive and
+            # step i-1's O leaves
+            mk = lambda: torch.empty((self.n, self.H, self.d), dtype=torch.bfloat16, device=self.dev)  # noqa: E731
+            self.stage = [tuple(mk() for _ in range(3)) for _ in range(2)]
+            self.o_e2e = [mk() for _ in range(2)]
+            self.o_host = [torch.empty((self.n, self.H, self.d), dtype=torch.bfloat16).pin_memory() for _ in range(2)]
+            self.s_in, self.s_out = torch.cuda.Stream(self.dev), torch.cuda.Stream(self.dev)
+            E = lambda: torch.cuda.Event()  # noqa: E731
+            self.ev_in = [E(), E()]      # inputs of set b are on the device
+            self.ev_free = [E(), E()]    # the step that read set b's inputs has finished
+            self.ev_done = [E(), E()]    # O of set b is complete
+            self.ev_out = [E(), E()]     # O of set b has been copied to the host
         self.e2e_no = 0
         self.step_no = 0
         torch.cuda.synchronize(self.dev)
@@ -206,8 +276,12 @@ class HotPath:
         uf.uf_kv_append(self.ctx, k, v, self.n, self.ts, self.hs, 0, self.stream)
         if ev_pre is not None:
             ev_pre[1].record(self.stream)
-        uf.uf_select_blocks(self.ctx, q, self.n, self.ts, self.hs, w.topk_count, w.topk_percent,
-                            self.idx, self.cnt, self.stream)
+        if self.paper:
+            uf.uf_select_blocks_paper(self.ctx, q, self.n, self.ts, self.hs, -1, w.rho_permille, self.idx,
+                                      self.idx_stride, self.cnt, self.stream)
+        else:
+            uf.uf_select_blocks(self.ctx, q, self.n, self.ts, self.hs, w.topk_count, w.topk_percent,
+                                self.idx, self.cnt, self.stream)
         if ev is not None:
             ev[0].record(self.stream)
         uf.uf_sparse_attn_fwd(self.ctx, q, self.o, self.lse, self.n, self.ts, self.hs, 0.0, self.stream)
@@ -253,15 +327,26 @@ class HotPath:
             self.stream.wait_event(self.ev_in[b])
 
     def current_kept_flop(self):
-        """FLOP of the step just run, from the returned index lists."""
+        """FLOP of the step just run, from the returned index lists -> (kept FLOP, N candidates, k', extra)."""
         uf, w = self.uf, self.w
         self.torch.cuda.synchronize(self.dev)
+        if self.paper:
+            n_cand, k_eff = uf.uf_query_budget_paper(self.ctx, -1, w.rho_permille)
+            idx, cnt = self.idx.cpu().numpy(), self.cnt.cpu().numpy()
+            nv = tile_sizes(w)
+            keys = np.where(idx >= 0, nv[np.maximum(idx, 0) % w.n_tiles], 0).sum(axis=2)          # [H, NB]
+            flop = int(4 * self.d * (nv[None, :] * keys).sum())
+            extra = {"mean_kept_blocks_per_row": float(cnt.mean()),
+                     "tensor_pipe_tflop_incl_tile_padding": float(4 * self.d * 128 * 128 * cnt.sum()) / 1e12,
+                     "tile_fill": float(nv.sum()) / float(nv.size * w.block)}
+            return flop, n_cand, k_eff, extra
         n_cand, k_eff = uf.uf_query_topk(self.ctx, w.topk_count, w.topk_percent)
-        idx = self.idx.cpu().numpy().reshape(-1)[: self.H * self.idx.shape[1] * k_eff].reshape(self.H, self.idx.shape[1], k_eff)
+        nqb = self.idx.shape[1]
+        idx = self.idx.cpu().numpy().reshape(-1)[: self.H * nqb * k_eff].reshape(self.H, nqb, k_eff)
         slot_map, _, newest = uf.uf_get_slot_map(self.ctx, w.capacity_chunks)
         prior = {c: self.n for c in slot_map if c >= 0}
         sink_tok = min(w.sink_blocks * w.block, self.n) if newest > 0 else 0
-        return kept_flop(w, self.n, idx, sink_tok, prior), n_cand, k_eff
+        return kept_flop(w, self.n, idx, sink_tok, prior), n_cand, k_eff, {}
 
 
 def time_steps(hp: HotPath, steps: int, warmup: int, e2e: bool):
@@ -307,7 +392,7 @@ def call_breakdown(hp: HotPath, steps: int, hbm_gbs: float):
     nhd2 = hp.n * hp.H * hp.d * 2
     nb = -(-hp.n // w.block)
     app_bytes = 4 * nhd2 + 8 * hp.H * hp.d * nb                       # read K,V + write both caches + pooled K
-    n_cand, k_eff = hp.uf.uf_query_topk(hp.ctx, w.topk_count, w.topk_percent)
+    _, n_cand, k_eff, _ = hp.current_kept_flop()
     sel_bytes = nhd2 + 8 * hp.H * hp.d * (nb + n_cand) + 4 * hp.H * nb * (k_eff + 1)   # read Q, pooled Q/K, write ids
     return {
         "append": {"ms": app, "algorithmic_bytes": app_bytes, "achieved_gbs": app_bytes / app / 1e6,
@@ -321,7 +406,8 @@ def call_breakdown(hp: HotPath, steps: int, hbm_gbs: float):
 
 
 def stream_percentiles(hp: HotPath, repeats: int):
-    """configs[3]: 20-chunk rolling stream, per-chunk ms; p50/p99 over steady-state chunks (c >= C)."""
+    """configs[3]: the 20-chunk rolling stream (per-chunk seeds 0..19) run `repeats` times after one untimed pass,
+    CUDA events around every chunk; p50 / p99 over the steady-state chunks (c >= C), ramp-up chunks listed apart."""
     torch, w = hp.torch, hp.w
     per = []
     for rep in range(repeats + 1):
@@ -338,22 +424,34 @@ def stream_percentiles(hp: HotPath, repeats: int):
     per = np.asarray(per)
     steady = per[:, w.capacity_chunks:].reshape(-1)
     return {"p50_ms": float(np.percentile(steady, 50)), "p99_ms": float(np.percentile(steady, 99)),
-            "rampup_ms": [float(x) for x in per[:, :w.capacity_chunks].mean(axis=0)], "repeats": repeats}
+            "mean_ms": float(steady.mean()), "max_ms": float(steady.max()), "steady_state_chunks_timed": int(steady.size),
+            "rampup_ms": [float(x) for x in per[:, :w.capacity_chunks].mean(axis=0)], "repeats": repeats,
+            "chunks_per_stream": w.n_stream_chunks}
 
 
 # --------------------------------------------------------------------------------------------------
-def cpu_oracle_sample(w: wl.Workload, budget_s: float = 20.0, max_pairs: int = 16):
-    """The fp64 oracle as it stands, on this box's host cores, on a bounded sample of the workload:
-    all prior appends + full selection of the timed chunk + attention on sampled (head, query-block) pairs.
-    Returns (TFLOP/s over the sample's kept FLOP, cores, description)."""
+def blas_threads() -> int:
+    try:
+        from threadpoolctl import threadpool_info
+        return max([int(x.get("num_threads", 1)) for x in threadpool_info()] or [1])
+    except Exception:
+        return 0
+
+
+def cpu_oracle_sample(w: wl.Workload, n_random: int = 64, budget_s: float = 25.0):
+    """The fp64 oracle as it stands, on this box's host cores: append and the FULL selection of
+    the timed chunk, then attention on a seeded sample of (head, query-block) pairs: block 0, the ragged last block
+    and `n_random` random pairs (cut short after `budget_s` seconds of attention, never below the two fixed pairs).
+    Returns a dict with the measured seconds and the extrapolation to the full chunk by kept-FLOP ratio."""
     from oracle.uf_oracle import UFOracle
     cores = len(os.sched_getaffinity(0))
     orc = UFOracle(w.n_heads, w.head_dim, w.block, w.chunk_tokens, w.capacity_chunks, w.sink_blocks, w.k_min)
     f64 = lambda b: wl.bf16_bits_to_f32(b).astype(np.float64)  # noqa: E731
+    chunks = get_chunks(w, range(w.prior_chunks + 1))
     for c in range(w.prior_chunks):
-        _, kb, vb = wl.make_chunk(w, c)
+        _, kb, vb = chunks[c]
         orc.kv_append(f64(kb), f64(vb))
-    qb, kb, vb = wl.make_chunk(w, w.prior_chunks)
+    qb, kb, vb = chunks[w.prior_chunks]
     Q, K, V = f64(qb), f64(kb), f64(vb)
     t0 = time.perf_counter()
     orc.kv_append(K, V)
@@ -363,41 +461,58 @@ def cpu_oracle_sample(w: wl.Workload, budget_s: float = 20.0, max_pairs: int = 1
     t_sel = time.perf_counter() - t0
     rng = np.random.default_rng(0)
     nqb = w.bpc
-    t_attn, flop, pairs = 0.0, 0, 0
-    while pairs < max_pairs and (t_attn < budget_s or pairs < 2):
-        h, i = int(rng.integers(0, w.n_heads)), int(rng.integers(0, nqb))
+    pairs = [(0, 0), (w.n_heads - 1, nqb - 1)]
+    pairs += [(int(rng.integers(0, w.n_heads)), int(rng.integers(0, nqb))) for _ in range(n_random)]
+
+    def pair_flop(h, i):
+        rows = min((i + 1) * w.block, w.chunk_tokens) - i * w.block
+        keys = sum(orc.block_kv(g, fs)[0].shape[0] for g, fs in orc.kept_blocks(h, i))
+        return 4 * w.head_dim * rows * keys
+
+    t_attn, flop, done = 0.0, 0, 0
+    for h, i in pairs:
+        if done >= 2 and t_attn > budget_s:
+            break
         t0 = time.perf_counter()
         orc.sparse_attn(Q, heads=[h], qblocks=[i])
         t_attn += time.perf_counter() - t0
-        rows = min((i + 1) * w.block, w.chunk_tokens) - i * w.block
-        keys = sum(orc.block_kv(g, fs)[0].shape[0] for g, fs in orc.kept_blocks(h, i))
-        flop += 4 * w.head_dim * rows * keys
-        pairs += 1
-    desc = (f"oracle/uf_oracle.py (NumPy fp64): append {t_app:.2f}s + full selection {t_sel:.2f}s (not in value) + "
-            f"attention on {pairs} random (head, query-block) pairs of {w.n_heads * nqb} in {t_attn:.2f}s; "
-            f"value = sampled kept FLOP / attention time")
-    return flop / t_attn / 1e12, cores, desc, t_attn, pairs
+        flop += pair_flop(h, i)
+        done += 1
+    total_flop = orc.kept_flop()
+    attn_full = t_attn * total_flop / flop
+    return {
+        "value": flop / t_attn / 1e12, "unit": UNIT, "cores": cores, "kind": "oracle", "blas_threads": blas_threads(),
+        "append_s": t_app, "select_full_s": t_sel, "attention_sample_s": t_attn, "attention_sample_pairs": done,
+        "attention_pairs_total": w.n_heads * nqb, "attention_sample_flop": flop, "chunk_kept_flop": total_flop,
+        "attention_s_per_chunk_extrapolated": attn_full,
+        "chunk_s_extrapolated": t_app + t_sel + attn_full,
+        "sample": (f"oracle/uf_oracle.py (NumPy fp64) on workload {w.name}: append and full selection timed in full; "
+                   f"attention on {done} (head, query-block) pairs = block 0, the ragged last block and "
+                   f"{max(done - 2, 0)} seeded random pairs of {w.n_heads * nqb}; value = sampled kept FLOP / attention "
+                   f"seconds; *_extrapolated = sample time x (kept FLOP of the chunk / kept FLOP of the sample) — an "
+                   f"extrapolation, not a measurement"),
+    }
 
 
 def run_reference(args, w):
-    """--impl reference: the oracle timed on host cores; rank 0 only."""
+    """--impl reference: the oracle timed on host cores; rank 0 only.  Each step = one bounded sample."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    vals = []
-    for _ in range(args.warmup if args.warmup < 1 else 1):
-        cpu_oracle_sample(w, budget_s=1.0, max_pairs=2)
-    t_all = 0.0
-    for _ in range(max(1, min(args.steps, 3))):
-        v, cores, desc, t, pairs = cpu_oracle_sample(w, budget_s=8.0, max_pairs=8)
-        vals.append(v); t_all += t
-    value = float(np.mean(vals))
+    steps = max(1, min(args.steps, 3))
+    for _ in range(1 if args.warmup >= 1 else 0):
+        cpu_oracle_sample(w, n_random=2, budget_s=2.0)
+    runs = [cpu_oracle_sample(w, n_random=16, budget_s=8.0) for _ in range(steps)]
+    value = float(np.mean([r["value"] for r in runs]))
+    t_all = float(np.sum([r["attention_sample_s"] for r in runs]))
+    cb = dict(runs[-1])
+    cb["value"] = value
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
-        "steps": len(vals), "warmup": 1, "ms_per_step": 1e3 * t_all / len(vals), "higher_is_better": True,
+        "steps": steps, "warmup": 1, "ms_per_step": 1e3 * t_all / steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": w.name, "note": "each step = a bounded sample of the workload (see cpu_baseline.sample)"},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+        "cpu_baseline": cb,
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -405,29 +520,60 @@ def run_reference(args, w):
 
 
 # --------------------------------------------------------------------------------------------------
-def measure_workload(w, device, steps, warmup, with_e2e=True):
-    n_distinct = w.capacity_chunks + 1 if not w.n_stream_chunks else min(w.n_stream_chunks, 4)
-    hp = HotPath(w, device, n_distinct)
+def measure_workload(w, device, steps, warmup, with_e2e=True, stream_repeats=5):
+    """device-resident steps (+ attention events), per-call breakdown, optional e2e leg, optional rolling stream"""
+    ids = range(w.n_stream_chunks) if w.n_stream_chunks else range(w.capacity_chunks + 1)
+    hp = HotPath(w, device, ids, pinned_host=with_e2e)
     try:
         # reach steady state (chunk 0 evicted, all slots used) before anything is timed
         for _ in range(w.capacity_chunks + 1):
             hp.step_resident()
         with ClockSampler(device) as cs:
             total_ms, attn_ms, launches = time_steps(hp, steps, warmup, e2e=False)
-        flop, n_cand, k_eff = hp.current_kept_flop()
+        flop, n_cand, k_eff, extra = hp.current_kept_flop()
         out = {"total_ms": total_ms, "attn_ms": attn_ms, "launches": launches, "flop": flop, "n_cand": n_cand,
-               "k_eff": k_eff, "clocks": cs.summary(), "device_bytes": hp.uf.uf_ctx_device_bytes(hp.ctx)}
+               "k_eff": k_eff, "clocks": cs.summary(), "device_bytes": hp.uf.uf_ctx_device_bytes(hp.ctx),
+               "extra": extra, "steps": steps}
         out["calls"] = call_breakdown(hp, min(steps, 10), load_peaks()["hbm_gbs"])
+        out["h2d"] = 3 * hp.n * hp.H * hp.d * 2
+        out["d2h"] = hp.n * hp.H * hp.d * 2
         if with_e2e:
             e2e_ms, _, _ = time_steps(hp, steps, min(warmup, 3), e2e=True)
             out["e2e_ms"] = e2e_ms
-            out["h2d"] = 3 * hp.n * hp.H * hp.d * 2
-            out["d2h"] = hp.n * hp.H * hp.d * 2
         if w.n_stream_chunks:
-            out["stream"] = stream_percentiles(hp, repeats=3)
+            out["stream"] = stream_percentiles(hp, repeats=stream_repeats)
         return out
     finally:
         hp.close()
+
+
+def roofline_obj(w, m, peaks):
+    t = m["flop"] / (m["attn_ms"] * 1e-3) / 1e12
+    traffic, src = ncu_attn_dram_bytes(w.name)
+    return {
+        "kernel": "uf_attn_sm100_kernel", "bound": "tensor", "achieved": t, "peak": peaks["bf16_burst"],
+        "unit": "TFLOP/s", "frac": t / peaks["bf16_burst"], "traffic": traffic, "traffic_source": src,
+        "peak_source": peaks["source"] + ", bf16 burst; sustained %.1f -> frac %.3f" % (
+            peaks["bf16_sustained"], t / peaks["bf16_sustained"]),
+        "algorithmic_flop_per_launch": m["flop"], "launch_ms": m["attn_ms"],
+    }
+
+
+def also_entry(w, m, peaks):
+    """one secondary workload under `also`: the same quantities as the main line, compact"""
+    steps = m["steps"]
+    e = {"workload": w.name, "steps": steps, "ms_per_step": m["total_ms"] / steps, "attn_ms": m["attn_ms"],
+         "kept_tflop_per_step": m["flop"] / 1e12, "value": m["flop"] * steps / (m["total_ms"] * 1e-3) / 1e12,
+         "unit": UNIT, "k_eff": m["k_eff"], "n_cand": m["n_cand"], "gpu_launches": m["launches"],
+         "roofline": roofline_obj(w, m, peaks), "calls": m["calls"], "clocks": m["clocks"]}
+    if "e2e_ms" in m:
+        e["e2e"] = {"value": m["flop"] * steps / (m["e2e_ms"] * 1e-3) / 1e12, "unit": UNIT,
+                    "ms_per_step": m["e2e_ms"] / steps, "h2d_bytes_per_step": m["h2d"], "d2h_bytes_per_step": m["d2h"]}
+    if "stream" in m:
+        e["stream"] = m["stream"]
+    if m["extra"]:
+        e["paper_mask"] = m["extra"]
+    return e
 
 
 def main():
@@ -435,14 +581,15 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=5)
-    ap.add_argument("--workload", default="1k", choices=["1k", "2k", "wide", "1k_stream"])
+    ap.add_argument("--workload", default="1k", choices=["1k", "2k", "wide", "1k_stream", "1k_paper", "2k_paper"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-also", action="store_true", help="skip the secondary 2K measurement")
+    ap.add_argument("--no-also", action="store_true", help="skip the secondary workloads (2k, wide, 1k_stream, paper-mask variants)")
+    ap.add_argument("--also", default="2k,1k_stream,wide,1k_paper,2k_paper", help="comma list of secondary workloads")
     args = ap.parse_args()
     w = wl.CONFIGS[args.workload]
     if args.impl == "reference":
-        run_reference(args, w)
+        run_reference(args, wl.CONFIGS["1k"] if w.tile else w)
         return
     warmup = max(3, args.warmup)
 
@@ -460,16 +607,19 @@ def main():
     n_ranks = world
     value = units / (total_ms * 1e-3) / 1e12
     e2e_value = units / (e2e_ms * 1e-3) / 1e12
-    attn_tflops = m["flop"] / (m["attn_ms"] * 1e-3) / 1e12
 
+    if w.tile:
+        what = (f"paper mask: tiles {w.tile}, window {w.window}, rho {w.rho_permille / 1000:.2f} -> tau_k {m['k_eff']} "
+                f"of {m['n_cand']} blocks in the causal mask")
+    else:
+        what = f"keep {w.topk_percent}% of {m['n_cand']} cache blocks = {m['k_eff']}"
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": n_ranks, "steps": args.steps, "warmup": warmup,
         "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "bf16", "data": "synthetic",
         "config": {
             "workload": f"{w.name} (BASELINE.json configs: {w.n_heads} heads x {w.head_dim}, chunk {w.chunk_tokens} tokens, "
-                        f"block {w.block}, capacity {w.capacity_chunks} chunks + sink, keep {w.topk_percent}% of {m['n_cand']} "
-                        f"cache blocks = {m['k_eff']})",
+                        f"block {w.block}, capacity {w.capacity_chunks} chunks{'' if w.tile else ' + sink'}, {what})",
             "step": "uf_kv_append -> uf_select_blocks -> uf_sparse_attn_fwd, steady-state rolling cache",
             "kept_tflop_per_step": m["flop"] / 1e12,
             "l2": "inputs larger than L2 (Q,K,V 3 x %.0f MB + cache %.0f MB per step; no explicit flush)" % (
@@ -482,32 +632,22 @@ def main():
                 "h2d_bytes_per_step": m["h2d"], "d2h_bytes_per_step": m["d2h"]},
         "gpu_launches": m["launches"],
         "clocks": m["clocks"],
-        "roofline": {
-            "kernel": "uf_attn_sm100_kernel", "bound": "tensor", "achieved": attn_tflops, "peak": peaks["bf16_burst"],
-            "unit": "TFLOP/s", "frac": attn_tflops / peaks["bf16_burst"], "traffic": NCU_ATTN_DRAM_BYTES.get(w.name),
-            "peak_source": peaks["source"] + ", bf16 burst; sustained %.1f -> frac %.3f" % (
-                peaks["bf16_sustained"], attn_tflops / peaks["bf16_sustained"]),
-            "algorithmic_flop_per_launch": m["flop"],
-        },
+        "roofline": roofline_obj(w, m, peaks),
         "calls": m["calls"],
     }
-    if rank == 0 and not args.no_also and args.workload == "1k":
-        m2 = measure_workload(wl.CONFIGS["2k"], device, max(3, args.steps // 2), 3, with_e2e=False)
-        t2 = m2["flop"] / (m2["attn_ms"] * 1e-3) / 1e12
-        line["also"] = {"2k": {"ms_per_step": m2["total_ms"] / max(3, args.steps // 2), "attn_ms": m2["attn_ms"],
-                               "kept_tflop_per_step": m2["flop"] / 1e12,
-                               "value": m2["flop"] / (m2["total_ms"] / max(3, args.steps // 2) * 1e-3) / 1e12,
-                               "attn_tflops": t2, "attn_frac_of_burst_peak": t2 / peaks["bf16_burst"],
-                               "roofline": {"kernel": "uf_attn_sm100_kernel", "bound": "tensor", "achieved": t2,
-                                            "peak": peaks["bf16_burst"], "unit": "TFLOP/s", "frac": t2 / peaks["bf16_burst"],
-                                            "traffic": NCU_ATTN_DRAM_BYTES.get("2k"),
-                                            "algorithmic_flop_per_launch": m2["flop"]},
-                               "k_eff": m2["k_eff"], "n_cand": m2["n_cand"], "clocks": m2["clocks"]}}
+    if m["extra"]:
+        line["config"]["paper_mask"] = m["extra"]
     if "stream" in m:
         line["stream"] = m["stream"]
+    if rank == 0 and n_ranks == 1 and not args.no_also and args.workload == "1k":
+        line["also"] = {}
+        for name in [x for x in args.also.split(",") if x]:
+            w2 = wl.CONFIGS[name]
+            steps2 = max(3, args.steps // 2)
+            m2 = measure_workload(w2, device, steps2, 3, with_e2e=(name == "2k"))
+            line["also"][name] = also_entry(w2, m2, peaks)
     if rank == 0 and n_ranks == 1 and not args.no_cpu_baseline:
-        v, cores, desc, _, _ = cpu_oracle_sample(w)
-        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
+        line["cpu_baseline"] = cpu_oracle_sample(wl.CONFIGS["1k"] if w.tile else w)
     if rank == 0:
         print(json.dumps(line), flush=True)
     if world > 1:
