@@ -267,13 +267,13 @@ class HotPath:
     def close(self):
         self.uf.uf_ctx_destroy(self.ctx)
 
-    def step(self, q, k, v, ev=None, ev_pre=None):
+    def step(self, q, k, v, ev=None, ev_pre=None, window=0):
         """ev = (before attention, after attention); ev_pre = (before append, before select) for the
         per-call breakdown pass (not used inside the timed region)."""
         uf, w = self.uf, self.w
         if ev_pre is not None:
             ev_pre[0].record(self.stream)
-        uf.uf_kv_append(self.ctx, k, v, self.n, self.ts, self.hs, 0, self.stream)
+        uf.uf_kv_append(self.ctx, k, v, self.n, self.ts, self.hs, window, self.stream)
         if ev_pre is not None:
             ev_pre[1].record(self.stream)
         if self.paper:
@@ -429,6 +429,44 @@ def stream_percentiles(hp: HotPath, repeats: int):
             "chunks_per_stream": w.n_stream_chunks}
 
 
+def window_policy_curve(hp: HotPath):
+    """NEXT-3: the 20-chunk rolling stream under each cache-window policy (uf_next_window feeding uf_kv_append's
+    window_chunks): mean ms/chunk over chunks c >= C and mean resident K+V cache bytes, against the fixed window."""
+    torch, uf, w = hp.torch, hp.uf, hp.w
+    slot = 2 * hp.H * w.bpc * w.block * hp.d * 2
+    policies = {
+        "fixed": dict(kind=uf.UF_WIN_FIXED),
+        "position(warm=3,compact=2)": dict(kind=uf.UF_WIN_POSITION, warm_chunks=3, compact_window=2),
+        "memory(budget=2 slots)": dict(kind=uf.UF_WIN_MEMORY, budget_bytes=2 * slot),
+        "content(min_share=300 permille,compact=1)": dict(kind=uf.UF_WIN_CONTENT, compact_window=1, min_share_permille=300),
+    }
+    out = {}
+    for name, kw in policies.items():
+        per, res, wins = [], [], []
+        for rep in range(2):
+            uf.uf_ctx_reset(hp.ctx, hp.stream)
+            hp.step_no = 0
+            evs = []
+            for c in range(w.n_stream_chunks):
+                W = uf.uf_next_window(hp.ctx, stream=hp.stream, **kw)       # content: one stream sync per chunk
+                e = (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+                e[0].record(hp.stream)
+                q, k, v = hp.devc[hp.step_no % len(hp.devc)]
+                hp.step(q, k, v, window=W)
+                e[1].record(hp.stream)
+                evs.append(e)
+                if rep:
+                    wins.append(W)
+                    res.append(uf.uf_get_slot_map(hp.ctx, w.capacity_chunks)[1])
+            torch.cuda.synchronize(hp.dev)
+            if rep:
+                per = [a.elapsed_time(b) for a, b in evs]
+        steady = per[w.capacity_chunks:]
+        out[name] = {"ms_per_chunk_mean": float(np.mean(steady)), "resident_chunks_mean": float(np.mean(res[w.capacity_chunks:])),
+                     "cache_bytes_mean": float(np.mean(res[w.capacity_chunks:])) * slot, "windows": wins}
+    return out
+
+
 # --------------------------------------------------------------------------------------------------
 def blas_threads() -> int:
     try:
@@ -542,6 +580,7 @@ def measure_workload(w, device, steps, warmup, with_e2e=True, stream_repeats=5):
             out["e2e_ms"] = e2e_ms
         if w.n_stream_chunks:
             out["stream"] = stream_percentiles(hp, repeats=stream_repeats)
+            out["stream"]["window_policies"] = window_policy_curve(hp)
         return out
     finally:
         hp.close()

@@ -192,6 +192,49 @@ int32_t uf_untile_tokens(uf_ctx* ctx, const void* tiled, void* raster,
                          int64_t tiled_tok_stride, int64_t tiled_head_stride,
                          int64_t raster_tok_stride, int64_t raster_head_stride, void* stream);
 
+/* ---- SR cache window policy --------------------------------------------------------------
+ * The paper states the idea three times and gives no rule: P:136 (iii) "dynamically selecting a compact cache window,
+ * trading minimal quality for significant memory and compute savings", "SR cache window: dynamically selected
+ * based on content complexity", "Select compact SR KV window based on chunk position and memory budget".
+ * Reading R-36: one small host function maps a stated policy to the `window_chunks` argument of the
+ * NEXT uf_kv_append; the mechanism (FIFO, shrinking evicts several, growing never resurrects) is R-17's.
+ *   UF_WIN_FIXED     W = C.
+ *   UF_WIN_POSITION  W = C for chunks 0 .. warm_chunks-1, compact_window afterwards ("chunk position").
+ *   UF_WIN_MEMORY    W = floor(budget_bytes / bytes of one cache slot), slot = K + V = 2 * H * BPC * B * d * 2 bytes
+ *                    ("memory budget"); clamped to 1 .. C.
+ *   UF_WIN_CONTENT   ("content complexity") uses an exact integer statistic of the LAST selection: how many of the kept
+ *                    top-k blocks, over all heads and query blocks, lie in each listed chunk (uf_get_select_usage).
+ *                    T = min(C, resident + 1) chunks would be resident after the next append under plain FIFO (its
+ *                    victim, if the cache is full, goes anyway).  Then, oldest survivor first: while that chunk holds
+ *                    fewer than min_share_permille of the kept blocks and T > compact_window, it is evicted too
+ *                    (T -= 1).  W = T.  Content whose top-k picks concentrate on recent chunks thus runs with a short
+ *                    window; the window grows again (by one chunk per append) when old chunks are being used.
+ * All results are clamped to 1 .. C.  UF_WIN_CONTENT synchronises `stream` (it reads 128 bytes of counters);
+ * a caller evaluates it once per chunk (on one layer) and applies the window to every layer.  The rule itself has
+ * no counterpart in the paper to check against: parity unpinned for the RULE; the statistic and the integer
+ * arithmetic are compared bit-exactly with oracle/uf_window_policy.py. */
+#define UF_WIN_FIXED     0
+#define UF_WIN_POSITION  1
+#define UF_WIN_MEMORY    2
+#define UF_WIN_CONTENT   3
+
+typedef struct uf_window_policy {
+  int32_t kind;                /* UF_WIN_*                                                             */
+  int32_t warm_chunks;         /* POSITION                                                             */
+  int32_t compact_window;      /* POSITION: W after the warm phase; CONTENT: smallest resident count   */
+  int32_t min_share_permille;  /* CONTENT: 0 .. 1000                                                   */
+  int64_t budget_bytes;        /* MEMORY: cap on resident non-sink K + V cache bytes                   */
+} uf_window_policy;
+
+/* window_chunks (host pointer) receives the W to pass to the next uf_kv_append. */
+int32_t uf_next_window(uf_ctx* ctx, const uf_window_policy* policy, int32_t* window_chunks, void* stream);
+
+/* Kept top-k blocks of the last selection per listed chunk (ascending chunk id; the candidates' chunks: resident
+ * prior chunks, in paper-mask mode also the newest).  Host outputs: kept_per_chunk[n], chunk_ids[n] (either may be
+ * NULL), *n_chunks = n <= capacity.  Synchronises `stream`.  UF_ERR_STATE without a valid selection. */
+int32_t uf_get_select_usage(uf_ctx* ctx, int64_t* kept_per_chunk, int32_t* chunk_ids, int32_t* n_chunks,
+                            void* stream);
+
 /* impl: 0 = tcgen05 kernel only (default; shapes it does not cover -> UF_ERR_UNSUPPORTED),
  *       1 = the generic CUDA-core attention kernel (any supported shape; slow). */
 int32_t uf_set_attn_impl(uf_ctx* ctx, int32_t impl);

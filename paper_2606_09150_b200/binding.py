@@ -24,6 +24,7 @@ SYMBOLS = [
     "uf_ctx_create", "uf_ctx_destroy", "uf_ctx_reset", "uf_kv_append", "uf_query_topk", "uf_select_blocks",
     "uf_sparse_attn_fwd", "uf_set_attn_impl", "uf_get_slot_map", "uf_get_cache_block", "uf_get_pooled_k",
     "uf_attn_redone_items", "uf_ctx_device_bytes", "uf_ctx_launch_count", "uf_last_error", "uf_version",
+    "uf_next_window", "uf_get_select_usage",
     "uf_ctx_set_tiling", "uf_query_budget_paper", "uf_select_blocks_paper", "uf_tile_tokens", "uf_untile_tokens",
 ]
 
@@ -41,6 +42,14 @@ class uf_config(Structure):
 
 class uf_tiling(Structure):
     _fields_ = [(n, c_int32) for n in ("frames", "grid_h", "grid_w", "bt", "bh", "bw", "window")]
+
+
+UF_WIN_FIXED, UF_WIN_POSITION, UF_WIN_MEMORY, UF_WIN_CONTENT = range(4)
+
+
+class uf_window_policy(Structure):
+    _fields_ = [("kind", c_int32), ("warm_chunks", c_int32), ("compact_window", c_int32),
+                ("min_share_permille", c_int32), ("budget_bytes", c_int64)]
 
 
 _lib = None
@@ -79,6 +88,8 @@ def load_library() -> ctypes.CDLL:
     lib.uf_select_blocks_paper.argtypes = [P, P, c_int32, c_int64, c_int64, c_int32, c_int32, P, c_int32, P, P]
     lib.uf_tile_tokens.argtypes = [P, P, P, c_int64, c_int64, c_int64, c_int64, P]
     lib.uf_untile_tokens.argtypes = [P, P, P, c_int64, c_int64, c_int64, c_int64, P]
+    lib.uf_next_window.argtypes = [P, POINTER(uf_window_policy), POINTER(c_int32), P]
+    lib.uf_get_select_usage.argtypes = [P, POINTER(c_int64), POINTER(c_int32), POINTER(c_int32), P]
     lib.uf_version.argtypes = []
     lib.uf_version.restype = c_char_p
     for name in SYMBOLS:
@@ -150,6 +161,24 @@ def uf_select_blocks(ctx, q, n_tokens: int, tok_stride: int, head_stride: int, t
                      topk_percent: int = -1, idx_out=None, cnt_out=None, stream=None) -> None:
     _check(ctx, load_library().uf_select_blocks(ctx, _ptr(q), n_tokens, tok_stride, head_stride, topk_count,
                                                 topk_percent, _ptr(idx_out), _ptr(cnt_out), _stream(stream)))
+
+
+def uf_next_window(ctx, kind: int, warm_chunks: int = 0, compact_window: int = 1, min_share_permille: int = 0,
+                   budget_bytes: int = 0, stream=None) -> int:
+    """-> window_chunks for the next uf_kv_append"""
+    p = uf_window_policy(kind, warm_chunks, compact_window, min_share_permille, budget_bytes)
+    w = c_int32(0)
+    _check(ctx, load_library().uf_next_window(ctx, byref(p), byref(w), _stream(stream)))
+    return int(w.value)
+
+
+def uf_get_select_usage(ctx, stream=None) -> tuple[list[int], list[int]]:
+    """-> (kept top-k blocks per listed chunk, the chunks' ids), ascending chunk id"""
+    kept = (c_int64 * UF_MAX_CAPACITY_CHUNKS)()
+    ids = (c_int32 * UF_MAX_CAPACITY_CHUNKS)()
+    n = c_int32(0)
+    _check(ctx, load_library().uf_get_select_usage(ctx, kept, ids, byref(n), _stream(stream)))
+    return list(kept[:n.value]), list(ids[:n.value])
 
 
 def uf_ctx_set_tiling(ctx, frames: int, grid_h: int, grid_w: int, bt: int = 2, bh: int = 8, bw: int = 8,
@@ -234,4 +263,5 @@ def uf_last_error(ctx=None) -> str:
     return msg.decode() if msg else ""
 
 
-__all__ = ["LIB_PATH", "SYMBOLS", "UFError", "load_library", "uf_config", "uf_tiling"] + SYMBOLS
+__all__ = ["LIB_PATH", "SYMBOLS", "UFError", "load_library", "uf_config", "uf_tiling", "uf_window_policy",
+           "UF_WIN_FIXED", "UF_WIN_POSITION", "UF_WIN_MEMORY", "UF_WIN_CONTENT"] + SYMBOLS

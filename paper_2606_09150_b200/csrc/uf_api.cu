@@ -102,6 +102,7 @@ int check_tensor_args(uf_ctx* c, const void* p, int64_t tok_stride, int64_t head
 void clear_host_state(uf_ctx* c) {
   for (int s = 0; s < UF_MAXC; ++s) { c->slot_chunk[s] = -1; c->slot_ntok[s] = 0; }
   c->next_chunk = 0; c->sink_ntok = 0; c->sel_valid = false; c->sel_k = 0; c->sel_ntok = 0;
+  c->usage_n = 0;
 }
 
 }  // namespace
@@ -154,6 +155,7 @@ int32_t uf_ctx_create(const uf_config* cfg, uf_ctx** out) {
       {(void**)&c->sel_pair, H * NP * 2 * (int64_t)c->kcap * 4},
       {(void**)&c->pair_cnt, H * NP * 4},
       {(void**)&c->sel_cnt, H * BPC * 4},
+      {(void**)&c->usage, 2 * UF_MAXC * 8},
       {(void**)&c->panic_item, H * NP * 4},
       {(void**)&c->panic_last, 4},
   };
@@ -171,6 +173,7 @@ int32_t uf_ctx_create(const uf_config* cfg, uf_ctx** out) {
   if (e == cudaSuccess) e = cudaMemset(c->kpool, 0, (size_t)(H * d * P * 8));
   if (e == cudaSuccess) e = cudaMemset(c->panic_item, 0, (size_t)(H * NP * 4));
   if (e == cudaSuccess) e = cudaMemset(c->panic_last, 0, 4);
+  if (e == cudaSuccess) e = cudaMemset(c->usage, 0, 2 * UF_MAXC * 8);
   if (e == cudaSuccess) e = cudaDeviceSynchronize();
   if (e != cudaSuccess) { int r = fail_cuda(nullptr, e, "cudaMemset"); uf_ctx_destroy(c); return r; }
   if (cfg->block == 128 && cfg->head_dim == 128) {
@@ -187,7 +190,7 @@ int32_t uf_ctx_destroy(uf_ctx* c) {
     cudaSetDevice(c->cfg.device);
     cudaFree(c->kc); cudaFree(c->vc); cudaFree(c->kpool); cudaFree(c->qbar);
     cudaFree(c->sel_q); cudaFree(c->sel_rank); cudaFree(c->sel_pair); cudaFree(c->pair_cnt);
-    cudaFree(c->panic_item); cudaFree(c->panic_last); cudaFree(c->sel_cnt);
+    cudaFree(c->panic_item); cudaFree(c->panic_last); cudaFree(c->sel_cnt); cudaFree(c->usage);
   }
   delete c;
   return UF_OK;
@@ -457,6 +460,75 @@ int32_t uf_sparse_attn_fwd(uf_ctx* c, const void* q, void* o, float* lse, int32_
                                          head_stride, scale, (cudaStream_t)stream);
   if (e != cudaSuccess) return fail_cuda(c, e, "uf_sparse_attn_fwd kernel launch");
   return UF_OK;
+}
+
+// ---- NEXT-3: SR cache window policy (P:136 (iii); reading R-17 + R-36) ----------------------
+
+int32_t uf_get_select_usage(uf_ctx* c, int64_t* kept_per_chunk, int32_t* chunk_ids, int32_t* n_chunks, void* stream) {
+  if (!c || !n_chunks) return UF_ERR_INVALID_ARG;
+  if (c->host_only) return fail(c, UF_ERR_STATE, "uf_get_select_usage: host-only ctx");
+  if (!c->sel_valid) return fail(c, UF_ERR_STATE, "uf_get_select_usage: no selection for the newest chunk");
+  *n_chunks = c->usage_n;
+  if (c->usage_n == 0) return UF_OK;
+  UF_CUDA(c, cudaSetDevice(c->cfg.device));
+  unsigned long long host[UF_MAXC];
+  UF_CUDA(c, cudaMemcpyAsync(host, c->usage + (size_t)c->usage_seq * UF_MAXC, sizeof(host), cudaMemcpyDeviceToHost,
+                             (cudaStream_t)stream));
+  UF_CUDA(c, cudaStreamSynchronize((cudaStream_t)stream));
+  for (int i = 0; i < c->usage_n; ++i) {
+    if (kept_per_chunk) kept_per_chunk[i] = (int64_t)host[i];
+    if (chunk_ids) chunk_ids[i] = c->usage_chunk[i];
+  }
+  return UF_OK;
+}
+
+int32_t uf_next_window(uf_ctx* c, const uf_window_policy* p, int32_t* window_chunks, void* stream) {
+  if (!c || !p || !window_chunks) return UF_ERR_INVALID_ARG;
+  const int C = c->cfg.capacity_chunks;
+  auto clampW = [&](int64_t w) { return (int32_t)(w < 1 ? 1 : (w > C ? C : w)); };
+  const int next = c->next_chunk;                       // id of the chunk the window is for
+  switch (p->kind) {
+    case UF_WIN_FIXED:
+      *window_chunks = C;
+      return UF_OK;
+    case UF_WIN_POSITION:
+      if (p->warm_chunks < 0 || p->compact_window < 1) return fail(c, UF_ERR_INVALID_ARG, "uf_next_window: bad position policy");
+      *window_chunks = next < p->warm_chunks ? C : clampW(p->compact_window);
+      return UF_OK;
+    case UF_WIN_MEMORY: {
+      if (p->budget_bytes < 0) return fail(c, UF_ERR_INVALID_ARG, "uf_next_window: negative budget");
+      const int64_t per_chunk = 2ll * c->cfg.n_heads * c->BPC * c->cfg.block * c->cfg.head_dim * 2;   // K + V slot
+      *window_chunks = clampW(p->budget_bytes / per_chunk);
+      return UF_OK;
+    }
+    case UF_WIN_CONTENT: {
+      if (p->compact_window < 1 || p->min_share_permille < 0 || p->min_share_permille > 1000)
+        return fail(c, UF_ERR_INVALID_ARG, "uf_next_window: bad content policy");
+      const int R = n_resident(c);
+      int T = clampW(R + 1);                            // resident chunks after the next append under plain FIFO
+      *window_chunks = T;
+      if (c->host_only || !c->sel_valid || c->usage_n == 0) return UF_OK;      // nothing measured yet: keep everything
+      int64_t kept[UF_MAXC];
+      int32_t ids[UF_MAXC], n = 0;
+      int r = uf_get_select_usage(c, kept, ids, &n, stream);
+      if (r) return r;
+      int64_t total = 0;
+      for (int i = 0; i < n; ++i) total += kept[i];
+      if (total == 0) return UF_OK;
+      // listed chunks ascend in id.  The FIFO victim (if the cache is full) goes anyway; after it, keep evicting the
+      // oldest survivor while it holds less than min_share_permille of the kept blocks.  The newest chunk (listed
+      // in paper-mask mode only) is never a victim.
+      int j = (R + 1 > C) ? 1 : 0;
+      while (j < n && ids[j] != c->next_chunk - 1 && T > p->compact_window &&
+             kept[j] * 1000 / total < p->min_share_permille) {
+        --T; ++j;
+      }
+      *window_chunks = clampW(T);
+      return UF_OK;
+    }
+    default:
+      return fail(c, UF_ERR_INVALID_ARG, "uf_next_window: unknown policy kind");
+  }
 }
 
 int32_t uf_set_attn_impl(uf_ctx* c, int32_t impl) {

@@ -91,6 +91,13 @@ __host__ __device__ inline void uf_cand_lookup(const UfView& v, int j, int* g, i
   *nvalid = v.til.enabled ? uf_tile_nvalid(v.til, b) : (rem < v.B ? rem : v.B);
 }
 
+// index (into the view's prior list, ascending chunk id) of the chunk candidate j belongs to
+__host__ __device__ inline int uf_cand_prior(const UfView& v, int j) {
+  int i = 0;
+  while (i + 1 < v.n_prior && j >= v.cand_prefix[i + 1]) ++i;
+  return i;
+}
+
 // valid rows of block b of the current chunk
 __host__ __device__ inline int uf_cur_nvalid(const UfView& v, int b) {
   if (v.til.enabled) return uf_tile_nvalid(v.til, b);
@@ -111,6 +118,11 @@ struct uf_ctx {
   int32_t* sel_rank = nullptr;    // candidate index of every sel_q entry (merge key); [H][BPC][kcap]
   int32_t* sel_pair = nullptr;    // per (h, q-block pair): merged union list with tile masks; [H][NP][2*kcap]
   int32_t* pair_cnt = nullptr;    // [H][NP]
+  unsigned long long* usage = nullptr;   // [2][UF_MAXC]: kept blocks per listed chunk in the last selection (NEXT-3);
+                                         // buffer usage_seq & 1 is current, the other one is zeroed for the next call
+  int usage_seq = 0;
+  int usage_chunk[UF_MAXC];       // chunk ids the current usage buffer refers to (host)
+  int usage_n = 0;
   int32_t* sel_cnt = nullptr;     // [H][BPC]: entries of every sel_q row (paper-mask mode: rows differ in length)
   UfTiling til = {};              // paper-mask mode when til.enabled
   bool sel_paper = false;         // the stored selection came from uf_select_blocks_paper

@@ -74,7 +74,9 @@ __global__ void __launch_bounds__(kScoreThreads)
 uf_score_topk_kernel(UfView v, const double* __restrict__ qbar, const double* __restrict__ kpool,
                      int nqb, int k_eff, int32_t* __restrict__ sel_q, int32_t* __restrict__ sel_rank, int kcap,
                      int32_t* __restrict__ sel_cnt, int32_t* __restrict__ idx_out, int32_t* __restrict__ cnt_out,
-                     int out_stride) {
+                     int out_stride, unsigned long long* __restrict__ usage) {
+  __shared__ unsigned int usage_s[UF_MAXC];            // kept blocks per listed chunk, this CTA (NEXT-3 statistic)
+  if (threadIdx.x < UF_MAXC) usage_s[threadIdx.x] = 0u;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   double* qs = reinterpret_cast<double*>(smem_raw);                                  // [kQG][D]
   unsigned long long* key = reinterpret_cast<unsigned long long*>(qs + kQG * D);     // [kQG][n_cand]
@@ -174,6 +176,7 @@ uf_score_topk_kernel(UfView v, const double* __restrict__ qbar, const double* __
         sel_q[rowq + pos] = uf_entry_pack(phys, nval, 0);
         sel_rank[rowq + pos] = j;                      // candidate index: the merge key
         if (idx_out) idx_out[((int64_t)h * nqb + i) * out_stride + pos] = gid;
+        atomicAdd(&usage_s[uf_cand_prior(v, j)], 1u);
       }
       pos0 += __popc(ball);
       eq_seen += __popc(beq);
@@ -185,6 +188,8 @@ uf_score_topk_kernel(UfView v, const double* __restrict__ qbar, const double* __
     }
     if (lane == 0 && cnt_out) cnt_out[(int64_t)h * nqb + i] = kPaper ? pos0 : k_eff;
   }
+  __syncthreads();
+  if (tid < v.n_prior && usage_s[tid]) atomicAdd(&usage[tid], (unsigned long long)usage_s[tid]);
 }
 
 // ---- merge the lists of query blocks (2p, 2p+1) into one union list with tile masks -----------------
@@ -198,8 +203,10 @@ uf_score_topk_kernel(UfView v, const double* __restrict__ qbar, const double* __
 constexpr int kMergeWarps = 4;
 __global__ void __launch_bounds__(kMergeWarps * 32)
 uf_pair_merge_kernel(UfView v, const int32_t* __restrict__ sel_rank, const int32_t* __restrict__ sel_cnt,
-                     int32_t* __restrict__ sel_pair, int32_t* __restrict__ pair_cnt, int nqb, int k_eff, int kcap) {
+                     int32_t* __restrict__ sel_pair, int32_t* __restrict__ pair_cnt, int nqb, int k_eff, int kcap,
+                     unsigned long long* __restrict__ usage_next) {
   extern __shared__ uint32_t bm_raw[];
+  if (blockIdx.x == 0 && threadIdx.x < UF_MAXC) usage_next[threadIdx.x] = 0ull;   // the next selection's counters
   const int NP = (v.BPC + 1) / 2;
   const int np_cur = (nqb + 1) / 2;
   const int nw = (v.n_cand + 31) / 32;
@@ -278,7 +285,17 @@ cudaError_t uf_launch_select(uf_ctx* c, const UfView& v, const __nv_bfloat16* q,
                              bool paper, int out_stride, cudaStream_t s) {
   const int nqb = uf_ceil_div(v.cur_ntok, v.B);
   const int NP = (v.BPC + 1) / 2;
+  // usage statistic (NEXT-3): this call counts into buffer `seq & 1`; the other buffer is zeroed for the next call
+  // (by the pair-merge kernel when it runs, else by a memset), so no extra launch sits on the hot path
+  c->usage_seq ^= 1;
+  unsigned long long* usage_cur = c->usage + (size_t)c->usage_seq * UF_MAXC;
+  unsigned long long* usage_next = c->usage + (size_t)(c->usage_seq ^ 1) * UF_MAXC;
+  c->usage_n = v.n_prior;
+  for (int i = 0; i < v.n_prior; ++i) c->usage_chunk[i] = v.prior_chunk[i];
   if (k_eff == 0 && !paper) {
+    c->usage_n = 0;
+    cudaError_t e0 = cudaMemsetAsync(c->usage, 0, 2 * UF_MAXC * sizeof(unsigned long long), s);
+    if (e0 != cudaSuccess) return e0;
     // no candidates (chunk 0, or window 1): counts are zero, nothing to score
     if (cnt_out) {
       cudaError_t e = cudaMemsetAsync(cnt_out, 0, (size_t)v.H * nqb * sizeof(int32_t), s);
@@ -306,7 +323,7 @@ cudaError_t uf_launch_select(uf_ctx* c, const UfView& v, const __nv_bfloat16* q,
     }                                                                                                        \
     uf_score_topk_kernel<DD, QG, PP><<<gs, kScoreThreads, smem, s>>>(                                        \
         v, c->qbar, c->kpool, nqb, k_eff, c->sel_q, c->sel_rank, c->kcap, c->sel_cnt, idx_out, cnt_out,      \
-        out_stride);                                                                                         \
+        out_stride, usage_cur);                                                                              \
   }
 #define UF_SCORE_LAUNCH(DD, QG)                                                                              \
   {                                                                                                          \
@@ -337,9 +354,11 @@ cudaError_t uf_launch_select(uf_ctx* c, const UfView& v, const __nv_bfloat16* q,
     const int np_cur = (nqb + 1) / 2;
     const size_t msmem = (size_t)kMergeWarps * 2 * uf_ceil_div(v.n_cand, 32) * sizeof(uint32_t);
     uf_pair_merge_kernel<<<uf_ceil_div(v.H * np_cur, kMergeWarps), kMergeWarps * 32, msmem, s>>>(
-        v, c->sel_rank, paper ? c->sel_cnt : nullptr, c->sel_pair, c->pair_cnt, nqb, k_eff, c->kcap);
+        v, c->sel_rank, paper ? c->sel_cnt : nullptr, c->sel_pair, c->pair_cnt, nqb, k_eff, c->kcap, usage_next);
     c->launches += 1;
     e = cudaGetLastError();
+  } else {
+    e = cudaMemsetAsync(usage_next, 0, UF_MAXC * sizeof(unsigned long long), s);
   }
   return e;
 }
