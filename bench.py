@@ -32,7 +32,7 @@ import uf_workloads as wl  # noqa: E402
 
 PROFILE_TRAFFIC = os.path.join(ROOT, "profiles", "attn_dram_traffic.txt")
 KERNEL_SOURCES = ["include/uf.h"] + ["paper_2606_09150_b200/csrc/" + f for f in (
-    "uf_internal.h", "uf_api.cu", "uf_append.cu", "uf_select.cu", "uf_attn_generic.cu", "uf_attn_sm100.cu")]
+    "uf_internal.h", "uf_api.cu", "uf_append.cu", "uf_fused_append.cu", "uf_select.cu", "uf_attn_generic.cu", "uf_attn_sm100.cu")]
 
 
 def kernel_source_hash() -> str:
@@ -209,13 +209,14 @@ class HotPath:
     """The step bench.py times: uf_kv_append -> uf_select_blocks -> uf_sparse_attn_fwd via the C ABI
     (paper-mask workloads: a tiled ctx, uf_select_blocks_paper, chunks converted once by uf_tile_tokens)."""
 
-    def __init__(self, w: wl.Workload, device: int, chunk_ids, pinned_host: bool):
+    def __init__(self, w: wl.Workload, device: int, chunk_ids, pinned_host: bool, fused: bool = False):
         import torch
         import paper_2606_09150_b200 as uf
         self.torch, self.uf, self.w = torch, uf, w
         self.dev = torch.device("cuda", device)
         torch.cuda.set_device(self.dev)
         self.paper = w.tile is not None
+        self.fused = fused          # NEXT-2: raw Q, K, V in; QK-norm + RoPE + append + pooling in one kernel
         self.H, self.d = w.n_heads, w.head_dim
         self.n = w.n_tiles * w.block if self.paper else w.chunk_tokens      # rows the library sees per chunk
         self.ctx = uf.uf_ctx_create(w.n_heads, w.head_dim, w.block, self.n, w.capacity_chunks,
@@ -260,6 +261,12 @@ class HotPath:
             self.ev_free = [E(), E()]    # the step that read set b's inputs has finished
             self.ev_done = [E(), E()]    # O of set b is complete
             self.ev_out = [E(), E()]     # O of set b has been copied to the host
+        if fused:
+            self.max_pos = 1024
+            cos, sin = wl.rope_tables(self.max_pos)
+            gq, gk = wl.norm_weights(w)
+            self.rope = tuple(torch.from_numpy(x).to(self.dev) for x in (cos, sin, gq, gk))
+            self.q_rot = torch.zeros((self.n, self.H, self.d), dtype=torch.bfloat16, device=self.dev)
         self.e2e_no = 0
         self.step_no = 0
         torch.cuda.synchronize(self.dev)
@@ -273,7 +280,13 @@ class HotPath:
         uf, w = self.uf, self.w
         if ev_pre is not None:
             ev_pre[0].record(self.stream)
-        uf.uf_kv_append(self.ctx, k, v, self.n, self.ts, self.hs, window, self.stream)
+        if self.fused:
+            t0 = (self.step_no % 300) * w.frames_per_chunk
+            uf.uf_qkv_rope_append(self.ctx, q, k, v, self.q_rot, self.n, self.ts, self.hs, self.ts, self.hs, *self.rope,
+                                  self.max_pos, t0, w.grid_h, w.grid_w, wl.ROPE_AXIS_DIMS, 1e-6, window, self.stream)
+            q = self.q_rot
+        else:
+            uf.uf_kv_append(self.ctx, k, v, self.n, self.ts, self.hs, window, self.stream)
         if ev_pre is not None:
             ev_pre[1].record(self.stream)
         if self.paper:
@@ -392,14 +405,19 @@ def call_breakdown(hp: HotPath, steps: int, hbm_gbs: float):
     nhd2 = hp.n * hp.H * hp.d * 2
     nb = -(-hp.n // w.block)
     app_bytes = 4 * nhd2 + 8 * hp.H * hp.d * nb                       # read K,V + write both caches + pooled K
+    if hp.fused:
+        app_bytes = 6 * nhd2 + 2 * 8 * hp.H * hp.d * nb               # + read raw Q, write post-RoPE Q, pooled Q
     _, n_cand, k_eff, _ = hp.current_kept_flop()
     sel_bytes = nhd2 + 8 * hp.H * hp.d * (nb + n_cand) + 4 * hp.H * nb * (k_eff + 1)   # read Q, pooled Q/K, write ids
+    if hp.fused:
+        sel_bytes -= nhd2                                             # Q was pooled by the fused append
     return {
         "append": {"ms": app, "algorithmic_bytes": app_bytes, "achieved_gbs": app_bytes / app / 1e6,
                    "frac_of_hbm_peak": app_bytes / app / 1e6 / hbm_gbs},
         "select": {"ms": sel, "algorithmic_bytes": sel_bytes, "achieved_gbs": sel_bytes / sel / 1e6,
                    "frac_of_hbm_peak": sel_bytes / sel / 1e6 / hbm_gbs,
-                   "note": "3 kernels: pool Q (HBM-bound), fp64 score + exact threshold-search top-k (latency/ALU-bound), pair merge"},
+                   "note": ("2 kernels: fp64 score + exact top-k, pair merge (Q pooled by the fused append)" if hp.fused else
+                            "3 kernels: pool Q (HBM-bound), fp64 score + exact threshold-search top-k (latency/ALU-bound), pair merge")},
         "attention": {"ms": att},
         "hbm_peak_gbs": hbm_gbs,
     }
@@ -558,10 +576,10 @@ def run_reference(args, w):
 
 
 # --------------------------------------------------------------------------------------------------
-def measure_workload(w, device, steps, warmup, with_e2e=True, stream_repeats=5):
+def measure_workload(w, device, steps, warmup, with_e2e=True, stream_repeats=5, fused=False):
     """device-resident steps (+ attention events), per-call breakdown, optional e2e leg, optional rolling stream"""
     ids = range(w.n_stream_chunks) if w.n_stream_chunks else range(w.capacity_chunks + 1)
-    hp = HotPath(w, device, ids, pinned_host=with_e2e)
+    hp = HotPath(w, device, ids, pinned_host=with_e2e, fused=fused)
     try:
         # reach steady state (chunk 0 evicted, all slots used) before anything is timed
         for _ in range(w.capacity_chunks + 1):
@@ -624,7 +642,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-also", action="store_true", help="skip the secondary workloads (2k, wide, 1k_stream, paper-mask variants)")
-    ap.add_argument("--also", default="2k,1k_stream,wide,1k_paper,2k_paper", help="comma list of secondary workloads")
+    ap.add_argument("--also", default="2k,1k_stream,wide,1k_paper,2k_paper,1k_fused,2k_fused",
+                    help="comma list of secondary workloads (x_fused = workload x through uf_qkv_rope_append)")
     args = ap.parse_args()
     w = wl.CONFIGS[args.workload]
     if args.impl == "reference":
@@ -681,10 +700,14 @@ def main():
     if rank == 0 and n_ranks == 1 and not args.no_also and args.workload == "1k":
         line["also"] = {}
         for name in [x for x in args.also.split(",") if x]:
-            w2 = wl.CONFIGS[name]
+            fused = name.endswith("_fused")
+            w2 = wl.CONFIGS[name[:-6] if fused else name]
             steps2 = max(3, args.steps // 2)
-            m2 = measure_workload(w2, device, steps2, 3, with_e2e=(name == "2k"))
+            m2 = measure_workload(w2, device, steps2, 3, with_e2e=(name == "2k"), fused=fused)
             line["also"][name] = also_entry(w2, m2, peaks)
+            if fused:
+                line["also"][name]["step"] = ("uf_qkv_rope_append (QK-norm + 3-D RoPE + append + pooled K, Q) -> "
+                                              "uf_select_blocks (score + top-k only) -> uf_sparse_attn_fwd")
     if rank == 0 and n_ranks == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_oracle_sample(wl.CONFIGS["1k"] if w.tile else w)
     if rank == 0:

@@ -192,6 +192,40 @@ int32_t uf_untile_tokens(uf_ctx* ctx, const void* tiled, void* raster,
                          int64_t tiled_tok_stride, int64_t tiled_head_stride,
                          int64_t raster_tok_stride, int64_t raster_head_stride, void* stream);
 
+/* ---- The step in front of the path, fused ------------------------------------------------
+ * P:343 "The SR model follows the Wan2.1 architecture ... 12 heads (head dim 128) ... 3D RoPE with axis dims
+ * (44,42,42)".  uf_qkv_rope_append takes the raw Q, K, V of the QKV projection and, in ONE pass over them, does what
+ * otherwise takes an elementwise kernel, uf_kv_append and the pooling pass of uf_select_blocks (readings R-37..R-40):
+ *   QK-norm  y = x / sqrt(mean over the token's H*d channels of x^2 + eps) * g   (q with gq, k with gk; v untouched)
+ *   RoPE     channel pairs (2i, 2i+1) of every head are complex numbers multiplied by cos + i sin of
+ *            pos * theta^(-2 i_a / D_a): the first dim_t/2 pairs follow the token's frame t0 + t, the next dim_h/2 its
+ *            row y, the last dim_w/2 its column x; the cos / sin values come from the caller's tables (model state)
+ *   round    to bf16, nearest even, ONCE, from fp64 (|result| < 2^-126 -> signed zero); all arithmetic before it is
+ *            IEEE fp64 in the stated order without fused multiply-add, so cache bytes and block indices are a fixed
+ *            function of the input bits
+ *   write    post-RoPE Q -> q_out; post-RoPE K and V -> the cache slot, exactly as uf_kv_append (same eviction policy,
+ *            sink copy, zero pad rows); block-mean pooled K and pooled Q -> the ctx.
+ * A following uf_select_blocks / uf_select_blocks_paper called with q == q_out (same strides) skips its pooling
+ * pass.  Token positions: raster order (t, y, x) over a grid_h x grid_w grid (token n: t = t0 + n / (gh*gw), ...); on a
+ * tiled ctx the tiling's grid and order are used and grid_h / grid_w are ignored.  head_dim must be 128.
+ * Errors as uf_kv_append, plus UF_ERR_CAPACITY when a position exceeds max_pos. */
+typedef struct uf_rope_spec {
+  const double* cos_tab;      /* device, fp64 [max_pos][head_dim/2]: column i = cos(row * freq_i)             */
+  const double* sin_tab;      /* device, fp64 [max_pos][head_dim/2]                                            */
+  const float* gq;            /* device, fp32 [n_heads*head_dim]: RMSNorm weight of q                          */
+  const float* gk;            /* device, fp32 [n_heads*head_dim]: RMSNorm weight of k                          */
+  double eps;                 /* 1e-6                                                                           */
+  int32_t max_pos;            /* rows of the tables                                                             */
+  int32_t t0;                 /* temporal position of the chunk's first latent frame (chunk c: c * F)          */
+  int32_t grid_h, grid_w;     /* token grid (raster mode)                                                       */
+  int32_t dim_t, dim_h, dim_w;/* axis dims, even, sum = head_dim (paper: 44, 42, 42)                            */
+} uf_rope_spec;
+
+int32_t uf_qkv_rope_append(uf_ctx* ctx, const void* q_in, const void* k_in, const void* v_in, void* q_out,
+                           int32_t n_tokens, int64_t in_tok_stride, int64_t in_head_stride,
+                           int64_t out_tok_stride, int64_t out_head_stride,
+                           const uf_rope_spec* rope, int32_t window_chunks, void* stream);
+
 /* ---- SR cache window policy --------------------------------------------------------------
  * The paper states the idea three times and gives no rule: P:136 (iii) "dynamically selecting a compact cache window,
  * trading minimal quality for significant memory and compute savings", "SR cache window: dynamically selected

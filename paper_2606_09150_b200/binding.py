@@ -24,7 +24,7 @@ SYMBOLS = [
     "uf_ctx_create", "uf_ctx_destroy", "uf_ctx_reset", "uf_kv_append", "uf_query_topk", "uf_select_blocks",
     "uf_sparse_attn_fwd", "uf_set_attn_impl", "uf_get_slot_map", "uf_get_cache_block", "uf_get_pooled_k",
     "uf_attn_redone_items", "uf_ctx_device_bytes", "uf_ctx_launch_count", "uf_last_error", "uf_version",
-    "uf_next_window", "uf_get_select_usage",
+    "uf_next_window", "uf_get_select_usage", "uf_qkv_rope_append",
     "uf_ctx_set_tiling", "uf_query_budget_paper", "uf_select_blocks_paper", "uf_tile_tokens", "uf_untile_tokens",
 ]
 
@@ -45,6 +45,12 @@ class uf_tiling(Structure):
 
 
 UF_WIN_FIXED, UF_WIN_POSITION, UF_WIN_MEMORY, UF_WIN_CONTENT = range(4)
+
+
+class uf_rope_spec(Structure):
+    _fields_ = [("cos_tab", c_void_p), ("sin_tab", c_void_p), ("gq", c_void_p), ("gk", c_void_p), ("eps", c_double),
+                ("max_pos", c_int32), ("t0", c_int32), ("grid_h", c_int32), ("grid_w", c_int32),
+                ("dim_t", c_int32), ("dim_h", c_int32), ("dim_w", c_int32)]
 
 
 class uf_window_policy(Structure):
@@ -88,6 +94,8 @@ def load_library() -> ctypes.CDLL:
     lib.uf_select_blocks_paper.argtypes = [P, P, c_int32, c_int64, c_int64, c_int32, c_int32, P, c_int32, P, P]
     lib.uf_tile_tokens.argtypes = [P, P, P, c_int64, c_int64, c_int64, c_int64, P]
     lib.uf_untile_tokens.argtypes = [P, P, P, c_int64, c_int64, c_int64, c_int64, P]
+    lib.uf_qkv_rope_append.argtypes = [P, P, P, P, P, c_int32, c_int64, c_int64, c_int64, c_int64,
+                                       POINTER(uf_rope_spec), c_int32, P]
     lib.uf_next_window.argtypes = [P, POINTER(uf_window_policy), POINTER(c_int32), P]
     lib.uf_get_select_usage.argtypes = [P, POINTER(c_int64), POINTER(c_int32), POINTER(c_int32), P]
     lib.uf_version.argtypes = []
@@ -161,6 +169,16 @@ def uf_select_blocks(ctx, q, n_tokens: int, tok_stride: int, head_stride: int, t
                      topk_percent: int = -1, idx_out=None, cnt_out=None, stream=None) -> None:
     _check(ctx, load_library().uf_select_blocks(ctx, _ptr(q), n_tokens, tok_stride, head_stride, topk_count,
                                                 topk_percent, _ptr(idx_out), _ptr(cnt_out), _stream(stream)))
+
+
+def uf_qkv_rope_append(ctx, q_in, k_in, v_in, q_out, n_tokens: int, in_tok_stride: int, in_head_stride: int,
+                       out_tok_stride: int, out_head_stride: int, cos_tab, sin_tab, gq, gk, max_pos: int, t0: int,
+                       grid_h: int, grid_w: int, dims=(44, 42, 42), eps: float = 1e-6, window_chunks: int = 0,
+                       stream=None) -> None:
+    rs = uf_rope_spec(_ptr(cos_tab), _ptr(sin_tab), _ptr(gq), _ptr(gk), eps, max_pos, t0, grid_h, grid_w, *dims)
+    _check(ctx, load_library().uf_qkv_rope_append(ctx, _ptr(q_in), _ptr(k_in), _ptr(v_in), _ptr(q_out), n_tokens,
+                                                  in_tok_stride, in_head_stride, out_tok_stride, out_head_stride,
+                                                  byref(rs), window_chunks, _stream(stream)))
 
 
 def uf_next_window(ctx, kind: int, warm_chunks: int = 0, compact_window: int = 1, min_share_permille: int = 0,
@@ -263,5 +281,5 @@ def uf_last_error(ctx=None) -> str:
     return msg.decode() if msg else ""
 
 
-__all__ = ["LIB_PATH", "SYMBOLS", "UFError", "load_library", "uf_config", "uf_tiling", "uf_window_policy",
+__all__ = ["LIB_PATH", "SYMBOLS", "UFError", "load_library", "uf_config", "uf_tiling", "uf_window_policy", "uf_rope_spec",
            "UF_WIN_FIXED", "UF_WIN_POSITION", "UF_WIN_MEMORY", "UF_WIN_CONTENT"] + SYMBOLS

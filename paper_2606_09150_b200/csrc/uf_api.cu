@@ -102,7 +102,62 @@ int check_tensor_args(uf_ctx* c, const void* p, int64_t tok_stride, int64_t head
 void clear_host_state(uf_ctx* c) {
   for (int s = 0; s < UF_MAXC; ++s) { c->slot_chunk[s] = -1; c->slot_ntok[s] = 0; }
   c->next_chunk = 0; c->sink_ntok = 0; c->sel_valid = false; c->sel_k = 0; c->sel_ntok = 0;
-  c->usage_n = 0;
+  c->usage_n = 0; c->qbar_chunk = -1;
+}
+
+// Steps shared by uf_kv_append and uf_qkv_rope_append: the integer cache policy on a copy of the slot state, the
+// device work (`launch`, given the view of the new state), commit / roll back.
+template <typename Launch>
+int32_t append_common(uf_ctx* c, int32_t n_tokens, int32_t window_chunks, const char* name, Launch launch) {
+  const int C = c->cfg.capacity_chunks;
+  if (n_tokens < 1) return fail(c, UF_ERR_INVALID_ARG, std::string(name) + ": n_tokens < 1");
+  if (n_tokens > c->cfg.chunk_tokens_max) return fail(c, UF_ERR_CAPACITY, std::string(name) + ": n_tokens > chunk_tokens_max");
+  if (window_chunks < 0 || window_chunks > C) return fail(c, UF_ERR_CAPACITY, std::string(name) + ": window_chunks outside 0..capacity_chunks");
+  if (c->til.enabled && n_tokens != c->BPC * c->cfg.block)
+    return fail(c, UF_ERR_INVALID_ARG, std::string(name) + ": a tiled ctx takes whole chunks in the tiled layout (n_tokens = N_b * block)");
+  // --- cache policy (host, integers only), computed on a copy of the slot state: it is committed only after
+  // the device work was enqueued, so a failing launch leaves the ctx as it was ---
+  const int cid = c->next_chunk;
+  const int W = window_chunks == 0 ? C : window_chunks;
+  int slot_chunk[UF_MAXC], slot_ntok[UF_MAXC];
+  for (int s = 0; s < UF_MAXC; ++s) { slot_chunk[s] = c->slot_chunk[s]; slot_ntok[s] = c->slot_ntok[s]; }
+  for (;;) {   // evict ids <= cid - W, oldest first
+    int oldest = -1;
+    for (int s = 0; s < C; ++s)
+      if (slot_chunk[s] >= 0 && (oldest < 0 || slot_chunk[s] < slot_chunk[oldest])) oldest = s;
+    if (oldest < 0 || slot_chunk[oldest] > cid - W) break;
+    slot_chunk[oldest] = -1; slot_ntok[oldest] = 0;
+  }
+  int slot = -1;
+  for (int s = 0; s < C; ++s) if (slot_chunk[s] < 0) { slot = s; break; }   // lowest free slot
+  if (slot < 0) return fail(c, UF_ERR_STATE, std::string(name) + ": no free slot (internal)");
+  slot_chunk[slot] = cid; slot_ntok[slot] = n_tokens;
+  int sink_ntok = c->sink_ntok;
+  if (cid == 0) {
+    int ns = c->cfg.sink_blocks * c->cfg.block;
+    sink_ntok = ns < n_tokens ? ns : n_tokens;
+  }
+  struct Saved { int slot_chunk[UF_MAXC], slot_ntok[UF_MAXC], next_chunk, sink_ntok; bool sel_valid; } old;
+  for (int s = 0; s < UF_MAXC; ++s) { old.slot_chunk[s] = c->slot_chunk[s]; old.slot_ntok[s] = c->slot_ntok[s]; }
+  old.next_chunk = c->next_chunk; old.sink_ntok = c->sink_ntok; old.sel_valid = c->sel_valid;
+  auto rollback = [&]() {
+    for (int s = 0; s < UF_MAXC; ++s) { c->slot_chunk[s] = old.slot_chunk[s]; c->slot_ntok[s] = old.slot_ntok[s]; }
+    c->sink_ntok = old.sink_ntok; c->next_chunk = old.next_chunk; c->sel_valid = old.sel_valid;
+  };
+  for (int s = 0; s < UF_MAXC; ++s) { c->slot_chunk[s] = slot_chunk[s]; c->slot_ntok[s] = slot_ntok[s]; }
+  c->sink_ntok = sink_ntok; c->next_chunk = cid + 1; c->sel_valid = false;
+  c->qbar_chunk = -1;                                   // pooled Q of an older chunk is stale now
+  if (c->host_only) return UF_OK;
+  // --- device ---
+  cudaError_t e = cudaSetDevice(c->cfg.device);
+  UfView view;
+  if (e == cudaSuccess && !make_view(c, &view)) { rollback(); return fail(c, UF_ERR_STATE, std::string(name) + ": inconsistent slot state (internal)"); }
+  if (e == cudaSuccess) e = launch(view);
+  if (e != cudaSuccess) {
+    rollback();                       // the chunk was not written: the ctx still describes the previous state
+    return fail_cuda(c, e, name);
+  }
+  return UF_OK;
 }
 
 }  // namespace
@@ -209,65 +264,57 @@ int32_t uf_ctx_reset(uf_ctx* c, void* stream) {
 int32_t uf_kv_append(uf_ctx* c, const void* k, const void* v, int32_t n_tokens,
                      int64_t tok_stride, int64_t head_stride, int32_t window_chunks, void* stream) {
   if (!c) return UF_ERR_INVALID_ARG;
-  const int C = c->cfg.capacity_chunks;
-  if (n_tokens < 1) return fail(c, UF_ERR_INVALID_ARG, "uf_kv_append: n_tokens < 1");
-  if (n_tokens > c->cfg.chunk_tokens_max) return fail(c, UF_ERR_CAPACITY, "uf_kv_append: n_tokens > chunk_tokens_max");
-  if (window_chunks < 0 || window_chunks > C) return fail(c, UF_ERR_CAPACITY, "uf_kv_append: window_chunks outside 0..capacity_chunks");
-  if (c->til.enabled && n_tokens != c->BPC * c->cfg.block)
-    return fail(c, UF_ERR_INVALID_ARG, "uf_kv_append: a tiled ctx takes whole chunks in the tiled layout (n_tokens = N_b * block)");
   if (!c->host_only) {
     int r = check_tensor_args(c, k, tok_stride, head_stride, "uf_kv_append k");
     if (r) return r;
     r = check_tensor_args(c, v, tok_stride, head_stride, "uf_kv_append v");
     if (r) return r;
   }
-  // --- cache policy (host, integers only), computed on a copy of the slot state: it is committed only after
-  // the device work was enqueued, so a failing launch leaves the ctx as it was ---
-  const int cid = c->next_chunk;
-  const int W = window_chunks == 0 ? C : window_chunks;
-  int slot_chunk[UF_MAXC], slot_ntok[UF_MAXC];
-  for (int s = 0; s < UF_MAXC; ++s) { slot_chunk[s] = c->slot_chunk[s]; slot_ntok[s] = c->slot_ntok[s]; }
-  for (;;) {   // evict ids <= cid - W, oldest first
-    int oldest = -1;
-    for (int s = 0; s < C; ++s)
-      if (slot_chunk[s] >= 0 && (oldest < 0 || slot_chunk[s] < slot_chunk[oldest])) oldest = s;
-    if (oldest < 0 || slot_chunk[oldest] > cid - W) break;
-    slot_chunk[oldest] = -1; slot_ntok[oldest] = 0;
+  return append_common(c, n_tokens, window_chunks, "uf_kv_append", [&](const UfView& view) {
+    return uf_launch_append(c, view, (const __nv_bfloat16*)k, (const __nv_bfloat16*)v, tok_stride, head_stride,
+                            (cudaStream_t)stream);
+  });
+}
+
+// NEXT-2 (R-37..R-40): QK-norm + 3-D RoPE + append + pooled K + pooled Q in one pass
+int32_t uf_qkv_rope_append(uf_ctx* c, const void* q_in, const void* k_in, const void* v_in, void* q_out,
+                           int32_t n_tokens, int64_t in_tok_stride, int64_t in_head_stride, int64_t out_tok_stride,
+                           int64_t out_head_stride, const uf_rope_spec* rs, int32_t window_chunks, void* stream) {
+  if (!c || !rs) return UF_ERR_INVALID_ARG;
+  if (c->host_only) return fail(c, UF_ERR_STATE, "uf_qkv_rope_append: host-only ctx has no device path");
+  if (c->cfg.head_dim != 128) return fail(c, UF_ERR_UNSUPPORTED, "uf_qkv_rope_append: head_dim must be 128");
+  int r = check_tensor_args(c, q_in, in_tok_stride, in_head_stride, "uf_qkv_rope_append q_in");
+  if (!r) r = check_tensor_args(c, k_in, in_tok_stride, in_head_stride, "uf_qkv_rope_append k_in");
+  if (!r) r = check_tensor_args(c, v_in, in_tok_stride, in_head_stride, "uf_qkv_rope_append v_in");
+  if (!r) r = check_tensor_args(c, q_out, out_tok_stride, out_head_stride, "uf_qkv_rope_append q_out");
+  if (r) return r;
+  if (!rs->cos_tab || !rs->sin_tab || !rs->gq || !rs->gk)
+    return fail(c, UF_ERR_INVALID_ARG, "uf_qkv_rope_append: null table / weight pointer");
+  if (rs->dim_t < 0 || rs->dim_h < 0 || rs->dim_w < 0 || (rs->dim_t & 1) || (rs->dim_h & 1) || (rs->dim_w & 1) ||
+      rs->dim_t + rs->dim_h + rs->dim_w != c->cfg.head_dim)
+    return fail(c, UF_ERR_INVALID_ARG, "uf_qkv_rope_append: axis dims must be even and sum to head_dim");
+  if (!(rs->eps >= 0.0) || rs->t0 < 0 || rs->max_pos < 1)
+    return fail(c, UF_ERR_INVALID_ARG, "uf_qkv_rope_append: bad eps / t0 / max_pos");
+  // the largest position any token of this chunk uses must be inside the tables
+  int frames, gh, gw;
+  if (c->til.enabled) { frames = c->til.F; gh = c->til.Hg; gw = c->til.Wg; }
+  else {
+    gh = rs->grid_h; gw = rs->grid_w;
+    if (gh < 1 || gw < 1) return fail(c, UF_ERR_INVALID_ARG, "uf_qkv_rope_append: grid_h, grid_w must be >= 1");
+    frames = uf_ceil_div(n_tokens, gh * gw);
   }
-  int slot = -1;
-  for (int s = 0; s < C; ++s) if (slot_chunk[s] < 0) { slot = s; break; }   // lowest free slot
-  if (slot < 0) return fail(c, UF_ERR_STATE, "uf_kv_append: no free slot (internal)");
-  slot_chunk[slot] = cid; slot_ntok[slot] = n_tokens;
-  int sink_ntok = c->sink_ntok;
-  if (cid == 0) {
-    int ns = c->cfg.sink_blocks * c->cfg.block;
-    sink_ntok = ns < n_tokens ? ns : n_tokens;
+  if (rs->t0 + frames > rs->max_pos || gh > rs->max_pos || gw > rs->max_pos)
+    return fail(c, UF_ERR_CAPACITY, "uf_qkv_rope_append: a position exceeds max_pos (the RoPE tables are too short)");
+  int32_t st = append_common(c, n_tokens, window_chunks, "uf_qkv_rope_append", [&](const UfView& view) {
+    return uf_launch_fused_append(c, view, (const __nv_bfloat16*)q_in, (const __nv_bfloat16*)k_in,
+                                  (const __nv_bfloat16*)v_in, (__nv_bfloat16*)q_out, in_tok_stride, in_head_stride,
+                                  out_tok_stride, out_head_stride, rs, (cudaStream_t)stream);
+  });
+  if (st == UF_OK) {
+    // the pooled Q of this chunk is already in the ctx: uf_select_blocks(q_out, ...) skips its pooling pass
+    c->qbar_chunk = c->next_chunk - 1; c->qbar_ptr = q_out; c->qbar_ts = out_tok_stride; c->qbar_hs = out_head_stride;
   }
-  struct Saved { int slot_chunk[UF_MAXC], slot_ntok[UF_MAXC], next_chunk, sink_ntok; bool sel_valid; } old;
-  for (int s = 0; s < UF_MAXC; ++s) { old.slot_chunk[s] = c->slot_chunk[s]; old.slot_ntok[s] = c->slot_ntok[s]; }
-  old.next_chunk = c->next_chunk; old.sink_ntok = c->sink_ntok; old.sel_valid = c->sel_valid;
-  auto commit = [&]() {
-    for (int s = 0; s < UF_MAXC; ++s) { c->slot_chunk[s] = slot_chunk[s]; c->slot_ntok[s] = slot_ntok[s]; }
-    c->sink_ntok = sink_ntok; c->next_chunk = cid + 1; c->sel_valid = false;
-  };
-  auto rollback = [&]() {
-    for (int s = 0; s < UF_MAXC; ++s) { c->slot_chunk[s] = old.slot_chunk[s]; c->slot_ntok[s] = old.slot_ntok[s]; }
-    c->sink_ntok = old.sink_ntok; c->next_chunk = old.next_chunk; c->sel_valid = old.sel_valid;
-  };
-  commit();
-  if (c->host_only) return UF_OK;
-  // --- device: copy + pooled K ---
-  cudaError_t e = cudaSetDevice(c->cfg.device);
-  UfView view;
-  if (e == cudaSuccess && !make_view(c, &view)) { rollback(); return fail(c, UF_ERR_STATE, "uf_kv_append: inconsistent slot state (internal)"); }
-  if (e == cudaSuccess)
-    e = uf_launch_append(c, view, (const __nv_bfloat16*)k, (const __nv_bfloat16*)v, tok_stride, head_stride,
-                         (cudaStream_t)stream);
-  if (e != cudaSuccess) {
-    rollback();                       // the chunk was not written: the ctx still describes the previous state
-    return fail_cuda(c, e, "uf_kv_append kernel launch");
-  }
-  return UF_OK;
+  return st;
 }
 
 int32_t uf_query_topk(const uf_ctx* c, int32_t topk_count, int32_t topk_percent, int32_t* n_cand, int32_t* k_eff) {
@@ -298,6 +345,7 @@ int32_t uf_select_blocks(uf_ctx* c, const void* q, int32_t n_tokens, int64_t tok
   if (r) return fail(c, r, "uf_select_blocks: topk_percent outside 0..100");
   if (k > c->kcap) return fail(c, UF_ERR_CAPACITY, "uf_select_blocks: k exceeds workspace (internal)");
   UF_CUDA(c, cudaSetDevice(c->cfg.device));
+  c->skip_pool_q = (c->qbar_chunk == v.cur_chunk && c->qbar_ptr == q && c->qbar_ts == tok_stride && c->qbar_hs == head_stride);
   cudaError_t e = uf_launch_select(c, v, (const __nv_bfloat16*)q, tok_stride, head_stride, k, idx_out, cnt_out,
                                    false, k, (cudaStream_t)stream);
   if (e != cudaSuccess) return fail_cuda(c, e, "uf_select_blocks kernel launch");
@@ -375,6 +423,7 @@ int32_t uf_select_blocks_paper(uf_ctx* c, const void* q, int32_t n_tokens, int64
   if (idx_out && idx_stride < max_row)
     return fail(c, UF_ERR_CAPACITY, "uf_select_blocks_paper: idx_stride < min(k + 1, N_blocks)");
   UF_CUDA(c, cudaSetDevice(c->cfg.device));
+  c->skip_pool_q = (c->qbar_chunk == v.cur_chunk && c->qbar_ptr == q && c->qbar_ts == tok_stride && c->qbar_hs == head_stride);
   cudaError_t e = uf_launch_select(c, v, (const __nv_bfloat16*)q, tok_stride, head_stride, k, idx_out, cnt_out,
                                    true, idx_stride, (cudaStream_t)stream);
   if (e != cudaSuccess) return fail_cuda(c, e, "uf_select_blocks_paper kernel launch");

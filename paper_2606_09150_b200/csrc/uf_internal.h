@@ -123,6 +123,10 @@ struct uf_ctx {
   int usage_seq = 0;
   int usage_chunk[UF_MAXC];       // chunk ids the current usage buffer refers to (host)
   int usage_n = 0;
+  int qbar_chunk = -1;            // chunk whose pooled Q is already in qbar (written by uf_qkv_rope_append), or -1
+  const void* qbar_ptr = nullptr; // ... for this post-RoPE Q buffer and these strides
+  int64_t qbar_ts = 0, qbar_hs = 0;
+  bool skip_pool_q = false;       // set per select call: qbar is valid for the q passed in
   int32_t* sel_cnt = nullptr;     // [H][BPC]: entries of every sel_q row (paper-mask mode: rows differ in length)
   UfTiling til = {};              // paper-mask mode when til.enabled
   bool sel_paper = false;         // the stored selection came from uf_select_blocks_paper
@@ -162,6 +166,9 @@ cudaError_t uf_launch_append(uf_ctx* c, const UfView& v, const __nv_bfloat16* k,
 cudaError_t uf_launch_select(uf_ctx* c, const UfView& v, const __nv_bfloat16* q, int64_t tok_stride,
                              int64_t head_stride, int k_eff, int32_t* idx_out, int32_t* cnt_out,
                              bool paper, int out_stride, cudaStream_t s);
+cudaError_t uf_launch_fused_append(uf_ctx* c, const UfView& v, const __nv_bfloat16* q, const __nv_bfloat16* k,
+                                   const __nv_bfloat16* vv, __nv_bfloat16* q_out, int64_t in_ts, int64_t in_hs,
+                                   int64_t out_ts, int64_t out_hs, const uf_rope_spec* rs, cudaStream_t s);
 // raster [F*Hg*Wg, H, d] <-> tiled, padded [NB*B, H, d] (pad rows zero)
 cudaError_t uf_launch_tile(uf_ctx* c, const __nv_bfloat16* src, __nv_bfloat16* dst, int64_t src_tok_stride,
                            int64_t src_head_stride, int64_t dst_tok_stride, int64_t dst_head_stride, bool untile,

@@ -331,8 +331,11 @@ cudaError_t uf_launch_select(uf_ctx* c, const UfView& v, const __nv_bfloat16* q,
   }
 #define UF_SELECT_CASE(DD)                                                                                   \
   case DD:                                                                                                   \
-    uf_pool_q_kernel<DD><<<gp, kPoolThreads, 0, s>>>(q, tok_stride, head_stride, c->qbar, v.B, v.BPC,        \
-                                                     v.cur_ntok, v.til);                                     \
+    if (!c->skip_pool_q) {               /* pooled Q already written by uf_qkv_rope_append: nothing to pool */ \
+      uf_pool_q_kernel<DD><<<gp, kPoolThreads, 0, s>>>(q, tok_stride, head_stride, c->qbar, v.B, v.BPC,      \
+                                                       v.cur_ntok, v.til);                                   \
+      c->launches += 1;                                                                                      \
+    }                                                                                                        \
     if (qg == 8) UF_SCORE_LAUNCH(DD, 8)                                                                      \
     else if (qg == 4) UF_SCORE_LAUNCH(DD, 4)                                                                 \
     else if (qg == 2) UF_SCORE_LAUNCH(DD, 2)                                                                 \
@@ -347,7 +350,7 @@ cudaError_t uf_launch_select(uf_ctx* c, const UfView& v, const __nv_bfloat16* q,
 #undef UF_SELECT_CASE
 #undef UF_SCORE_LAUNCH
 #undef UF_SCORE_LAUNCH2
-  c->launches += 2;
+  c->launches += 1;
   e = cudaGetLastError();
   if (e != cudaSuccess) return e;
   if (v.B == 128 && v.d == 128) {

@@ -1,0 +1,97 @@
+"""GPU parity of the fused QK-norm + 3-D RoPE + append + pooling step (NEXT-2, uf_qkv_rope_append) against
+oracle/uf_rope_norm.py followed by the ordinary oracle: post-RoPE Q bits, cache bytes, pooled K and every selected block
+id bit-exact; attention outputs within BASELINE.json's 2e-2 / 2e-3."""
+import numpy as np
+import pytest
+
+import uf_workloads as wl
+import uf_harness as hz
+from test_gpu_parity import _check_cache
+
+pytestmark = pytest.mark.gpu
+
+
+def _stream(w, n_chunks, lens=None, windows=None, fused_qkv=False, **sel):
+    cu, orc = hz.CudaStream(w), hz.make_oracle(w)
+    rs = hz.RopeState(w, 64, cu.dev)
+    try:
+        for c in range(n_chunks):
+            n = None if lens is None else lens[c]
+            win = 0 if windows is None else windows[c]
+            Qb, Kb, Vb = wl.make_chunk(w, c, n_tokens=n)
+            t0 = c * w.frames_per_chunk
+            got = hz.fused_step(cu, rs, Qb, Kb, Vb, t0, window=win, fused_qkv=fused_qkv, **sel)
+            ref = hz.oracle_fused_step(orc, rs, w, Qb, Kb, Vb, t0, window=win, **sel)
+            assert np.array_equal(got["q_out_bits"], ref["q_out_bits"]), \
+                f"chunk {c}: post-RoPE Q differs in {(got['q_out_bits'] != ref['q_out_bits']).sum()} elements"
+            hz.compare_step(got, ref, f"[{w.name} fused chunk {c}]")
+            # fused append (1) + score/top-k (1, no pooling pass) + pair merge (1) + attention (2); chunk 0 has no candidates
+            assert got["launches"] == (5 if got["k_eff"] > 0 else 3), got["launches"]
+        _check_cache(cu, orc, w)                           # cache bytes == oracle's post-RoPE K, V; pooled K bit-exact
+    finally:
+        cu.close()
+
+
+def test_fused_small_stream_ragged():
+    w = wl.scaled(wl.CONFIGS["1k"], "fz_small", n_heads=2, frames_per_chunk=2, grid_h=13, grid_w=21, capacity_chunks=3,
+                  topk_percent=50)
+    assert w.chunk_tokens == 546 and w.bpc == 5
+    _stream(w, 5, topk_percent=50)
+
+
+def test_fused_strided_qkv_variable_length_and_windows():
+    """Q, K, V as slices of one [n, 3, H, d] projection output; chunks of different lengths (the last frame partial);
+    shrinking windows; S = 2 sink blocks."""
+    w = wl.scaled(wl.CONFIGS["1k"], "fz_var", n_heads=3, frames_per_chunk=2, grid_h=10, grid_w=20, capacity_chunks=4,
+                  sink_blocks=2)
+    _stream(w, 6, lens=[400, 333, 400, 129, 257, 400], windows=[0, 0, 0, 2, 4, 3], fused_qkv=True, topk_count=2)
+
+
+def test_fused_error_codes():
+    import torch
+    import paper_2606_09150_b200 as uf
+    w = wl.scaled(wl.CONFIGS["1k"], "fz_err", n_heads=1, frames_per_chunk=1, grid_h=16, grid_w=16, capacity_chunks=2)
+    cu = hz.CudaStream(w)
+    rs = hz.RopeState(w, 16, cu.dev)
+    try:
+        Qb, Kb, Vb = wl.make_chunk(w, 0)
+        q, k, v = cu.to_dev(Qb), cu.to_dev(Kb), cu.to_dev(Vb)
+        qo = torch.empty_like(q)
+        args = (cu.ctx, q, k, v, qo, 256, 128, 128, 128, 128, rs.d_cos, rs.d_sin, rs.d_gq, rs.d_gk)
+        with pytest.raises(uf.UFError) as ei:                       # t0 + frames > max_pos
+            uf.uf_qkv_rope_append(*args, 16, 16, 16, 16, stream=cu.stream)
+        assert ei.value.code == uf.binding.UF_ERR_CAPACITY
+        with pytest.raises(uf.UFError) as ei:                       # axis dims do not sum to head_dim
+            uf.uf_qkv_rope_append(*args, 16, 0, 16, 16, dims=(44, 42, 40), stream=cu.stream)
+        assert ei.value.code == uf.binding.UF_ERR_INVALID_ARG
+        assert uf.uf_get_slot_map(cu.ctx, 2) == ([-1, -1], 0, -1)   # nothing was appended
+        uf.uf_qkv_rope_append(*args, 16, 0, 16, 16, stream=cu.stream)
+        assert uf.uf_get_slot_map(cu.ctx, 2) == ([0, -1], 1, 0)
+        # a select call with ANOTHER q buffer must not reuse the pooled Q of the fused call
+        l0 = uf.uf_ctx_launch_count(cu.ctx)
+        uf.uf_kv_append(cu.ctx, k, v, 256, 128, 128, 0, cu.stream)
+        uf.uf_select_blocks(cu.ctx, q, 256, 128, 128, 1, -1, None, None, cu.stream)
+        assert uf.uf_ctx_launch_count(cu.ctx) - l0 == 1 + 3         # append + pool + score + merge
+        torch.cuda.synchronize()
+    finally:
+        cu.close()
+
+
+def test_fused_full_size_1k():
+    """BASELINE.json configs[1] shapes through the fused entry: all 2 x 37.6 M post-RoPE Q elements, all selected block
+    ids, sampled cache blocks and pooled K bit-exact; attention on sampled (head, query block) pairs."""
+    w = wl.CONFIGS["1k"]
+    cu, orc = hz.CudaStream(w), hz.make_oracle(w)
+    rs = hz.RopeState(w, 128, cu.dev)
+    try:
+        for c in range(2):
+            Qb, Kb, Vb = wl.make_chunk(w, c)
+            got = hz.fused_step(cu, rs, Qb, Kb, Vb, 3 * c, topk_percent=w.topk_percent)
+            ref = hz.oracle_fused_step(orc, rs, w, Qb, Kb, Vb, 3 * c, topk_percent=w.topk_percent,
+                                       heads=[0, 5, 11], qblocks=[0, 1, 77, 190, 191], attn=(c == 1))
+            assert np.array_equal(got["q_out_bits"], ref["q_out_bits"])
+            r = hz.compare_step(got, ref, f"[1k fused chunk {c}]")
+        print(f"1k fused: sampled O max-abs {r[0]:.3e} mean-abs {r[1]:.3e}, min top-k gap {ref['min_gap']:.3e}")
+        _check_cache(cu, orc, w)
+    finally:
+        cu.close()

@@ -9,6 +9,7 @@ import numpy as np
 import uf_workloads as wl
 from oracle.uf_oracle import UFOracle
 from oracle.uf_paper_mask import UFPaperOracle
+from oracle import uf_rope_norm as rope_norm
 
 # BASELINE.json north_star: attention outputs within max-abs 2e-2 and mean-abs 2e-3 of the fp64 oracle
 O_MAX_ABS = 2e-2
@@ -250,3 +251,60 @@ def compare_paper_step(got: dict, ref: dict, where: str = ""):
     got2 = dict(got)
     got2["idx"] = g[:, :, :kmax]
     return compare_step(got2, ref, where)
+
+
+# ------------------------------------------------------------------------------------ fused QK-norm + RoPE + append (NEXT-2)
+class RopeState:
+    """Model state of the fused step on the device: fp64 cos / sin tables and fp32 norm weights (inputs of both sides)."""
+
+    def __init__(self, w: wl.Workload, max_pos: int, device):
+        import torch
+        self.max_pos = max_pos
+        self.cos, self.sin = wl.rope_tables(max_pos)
+        self.gq, self.gk = wl.norm_weights(w)
+        self.d_cos, self.d_sin = torch.from_numpy(self.cos).to(device), torch.from_numpy(self.sin).to(device)
+        self.d_gq, self.d_gk = torch.from_numpy(self.gq).to(device), torch.from_numpy(self.gk).to(device)
+
+
+def fused_step(cu: "CudaStream", rs: RopeState, Qb, Kb, Vb, t0, topk_count=-1, topk_percent=-1, window=0, scale=0.0,
+               fused_qkv=False):
+    """uf_qkv_rope_append -> uf_select_blocks(q_out) -> uf_sparse_attn_fwd(q_out) on raw (pre-norm, pre-RoPE) Q, K, V."""
+    torch, uf, w = cu.torch, cu.uf, cu.w
+    n, H, d = Qb.shape
+    if fused_qkv:
+        qkv = cu.to_dev(np.ascontiguousarray(np.stack([Qb, Kb, Vb], axis=1)))
+        q, k, v = qkv[:, 0], qkv[:, 1], qkv[:, 2]
+        its = 3 * H * d
+    else:
+        q, k, v = cu.to_dev(Qb), cu.to_dev(Kb), cu.to_dev(Vb)
+        its = H * d
+    q_out = torch.full((n, H, d), float("nan"), dtype=torch.bfloat16, device=cu.dev)
+    l0 = uf.uf_ctx_launch_count(cu.ctx)
+    uf.uf_qkv_rope_append(cu.ctx, q, k, v, q_out, n, its, d, H * d, d, rs.d_cos, rs.d_sin, rs.d_gq, rs.d_gk, rs.max_pos,
+                          t0, w.grid_h, w.grid_w, wl.ROPE_AXIS_DIMS, 1e-6, window, cu.stream)
+    slot_map = uf.uf_get_slot_map(cu.ctx, w.capacity_chunks)
+    n_cand, k_eff = uf.uf_query_topk(cu.ctx, topk_count, topk_percent)
+    nqb = -(-n // w.block)
+    idx = torch.full((H, nqb, max(k_eff, 1)), -1, dtype=torch.int32, device=cu.dev)
+    cnt = torch.full((H, nqb), -1, dtype=torch.int32, device=cu.dev)
+    uf.uf_select_blocks(cu.ctx, q_out, n, H * d, d, topk_count, topk_percent, idx, cnt, cu.stream)
+    o = torch.full((n, H, d), float("nan"), dtype=torch.bfloat16, device=cu.dev)
+    lse = torch.full((H, n), float("nan"), dtype=torch.float32, device=cu.dev)
+    uf.uf_set_attn_impl(cu.ctx, 0)
+    uf.uf_sparse_attn_fwd(cu.ctx, q_out, o, lse, n, H * d, d, scale, cu.stream)
+    torch.cuda.synchronize(cu.dev)
+    return {"slot_map": slot_map, "n_cand": n_cand, "k_eff": k_eff, "idx": idx.cpu().numpy()[:, :, :k_eff],
+            "cnt": cnt.cpu().numpy(), "O": o.float().cpu().numpy(), "lse": lse.cpu().numpy(),
+            "q_out_bits": q_out.view(torch.int16).cpu().numpy().view(np.uint16),
+            "launches": uf.uf_ctx_launch_count(cu.ctx) - l0}
+
+
+def oracle_fused_step(orc: UFOracle, rs: RopeState, w: wl.Workload, Qb, Kb, Vb, t0, **kw):
+    """oracle: norm + RoPE (oracle/uf_rope_norm.py) -> bf16 bits -> the ordinary oracle step on them"""
+    n = Qb.shape[0]
+    pos = rope_norm.raster_positions(n, w.grid_h, w.grid_w, t0)
+    q2 = rope_norm.apply(bits_to_f64(Qb), rs.gq.astype(np.float64), rs.cos, rs.sin, pos)
+    k2 = rope_norm.apply(bits_to_f64(Kb), rs.gk.astype(np.float64), rs.cos, rs.sin, pos)
+    out = oracle_step(orc, q2, k2, Vb, **kw)
+    out["q_out_bits"], out["k_bits"] = q2, k2
+    return out

@@ -178,3 +178,27 @@ def make_stream(w: Workload, n_chunks: int):
         rng = np.random.default_rng(0)
         return [make_chunk(w, c, rng=rng) for c in range(n_chunks)]
     return [make_chunk(w, c) for c in range(n_chunks)]
+
+
+# ---------------------------------------------------------------------------
+# Model state for the fused QK-norm + RoPE + append step: inputs, like weights
+# ---------------------------------------------------------------------------
+
+ROPE_AXIS_DIMS = (44, 42, 42)        # PAPER.md:343 "3D RoPE with axis dims (44,42,42)"
+
+
+def rope_tables(max_pos: int, dims=ROPE_AXIS_DIMS, theta: float = 10000.0):
+    """cos / sin tables a Wan2.1-style model precomputes once: fp64 [max_pos, d/2]; column i of the axis segment of
+    dim D holds cos / sin(pos * theta**(-2 i / D)).  An INPUT of the step (both sides read the same numbers); the
+    oracle states the definition they must satisfy (oracle/uf_rope_norm.py: rope_table) and a CPU test compares."""
+    freq = np.concatenate([theta ** (-(2.0 * np.arange(D // 2, dtype=np.float64)) / D) for D in dims])
+    ang = np.outer(np.arange(max_pos, dtype=np.float64), freq)
+    return np.cos(ang), np.sin(ang)
+
+
+def norm_weights(w: Workload, seed: int = 20_000):
+    """RMSNorm weights of q and k, fp32 [H*d]: 1 + 0.1 N(0,1) (random-init stand-in for trained weights)"""
+    g = np.random.default_rng(seed)
+    n = w.n_heads * w.head_dim
+    return ((1.0 + 0.1 * g.standard_normal(n)).astype(np.float32),
+            (1.0 + 0.1 * g.standard_normal(n)).astype(np.float32))
