@@ -200,9 +200,9 @@ int32_t uf_untile_tokens(uf_ctx* ctx, const void* tiled, void* raster,
  *   RoPE     channel pairs (2i, 2i+1) of every head are complex numbers multiplied by cos + i sin of
  *            pos * theta^(-2 i_a / D_a): the first dim_t/2 pairs follow the token's frame t0 + t, the next dim_h/2 its
  *            row y, the last dim_w/2 its column x; the cos / sin values come from the caller's tables (model state)
- *   round    to bf16, nearest even, ONCE, from fp64 (|result| < 2^-126 -> signed zero); all arithmetic before it is
- *            IEEE fp64 in the stated order without fused multiply-add, so cache bytes and block indices are a fixed
- *            function of the input bits
+ *   round    to bf16 (nearest even).  Everything before it is IEEE fp32, each operation rounded once, no fused
+ *            multiply-add, in the stated order (the sum of squares and the reciprocal square root run in fp64 and are
+ *            rounded to fp32 once), so cache bytes and block indices are a fixed function of the input bits
  *   write    post-RoPE Q -> q_out; post-RoPE K and V -> the cache slot, exactly as uf_kv_append (same eviction policy,
  *            sink copy, zero pad rows); block-mean pooled K and pooled Q -> the ctx.
  * A following uf_select_blocks / uf_select_blocks_paper called with q == q_out (same strides) skips its pooling
@@ -210,8 +210,8 @@ int32_t uf_untile_tokens(uf_ctx* ctx, const void* tiled, void* raster,
  * tiled ctx the tiling's grid and order are used and grid_h / grid_w are ignored.  head_dim must be 128.
  * Errors as uf_kv_append, plus UF_ERR_CAPACITY when a position exceeds max_pos. */
 typedef struct uf_rope_spec {
-  const double* cos_tab;      /* device, fp64 [max_pos][head_dim/2]: column i = cos(row * freq_i)             */
-  const double* sin_tab;      /* device, fp64 [max_pos][head_dim/2]                                            */
+  const float* cos_tab;       /* device, fp32 [max_pos][head_dim/2]: column i = cos(row * freq_i)             */
+  const float* sin_tab;       /* device, fp32 [max_pos][head_dim/2]                                            */
   const float* gq;            /* device, fp32 [n_heads*head_dim]: RMSNorm weight of q                          */
   const float* gk;            /* device, fp32 [n_heads*head_dim]: RMSNorm weight of k                          */
   double eps;                 /* 1e-6                                                                           */

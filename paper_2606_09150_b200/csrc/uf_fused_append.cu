@@ -6,18 +6,26 @@
 // HBM traffic: Q, K, V read once, Q', K-cache, V-cache written once (6 * N*H*d*2 bytes); the second look at Q, K
 // inside the CTA comes from L1/L2.
 //
-// Arithmetic (R-40): bf16 -> fp64, every operation IEEE fp64 rounded once, no FMA contraction, in the order
-//   ss = sum x^2;  r = 1 / sqrt(ss / C + eps);  u = (x * r) * g;  out_e = u_e*cos - u_o*sin;  out_o = u_e*sin + u_o*cos
-// then ONE rounding fp64 -> bf16 (nearest even, below 2^-126 -> signed zero), done on the bits, which also yields
-// the rounded value as a double for the pooled sums (exact, order-free, as in uf_append.cu).  This makes the cache
-// bytes and the pooled means a fixed function of the input bits: the oracle (oracle/uf_rope_norm.py) gets the same.
+// Arithmetic (R-40): the bf16 rounding of the result decides cache bytes and (through pooling) block indices, so it is
+// taken on a number that is a fixed function of the input bits: IEEE fp32, every operation rounded once, no FMA
+// contraction (__fmul_rn / __fadd_rn / __fsub_rn), in the order
+//   ss = sum x^2 (fp64, exact);  r = fl32(1 / sqrt(ss / C + eps)) (fp64 ops);  u = fl(fl(x r) g);
+//   out_e = fl(fl(u_e cos) - fl(u_o sin));  out_o = fl(fl(u_e sin) + fl(u_o cos));  result = bf16_rne(out)
+// and the oracle (oracle/uf_rope_norm.py) does the same in NumPy float32.  The pooled sums add the ROUNDED values in
+// fp64 (exact, order-free, as in uf_append.cu).
 //
-// One CTA per key block of the chunk (all heads).  Phase 1, token-major: one warp per token row streams the row's
-// H*d channels of Q and K (16-byte vectors, coalesced) and reduces the two sums of squares -> r_q[row], r_k[row] in
-// shared memory.  Phase 2, column-major per head (the layout of uf_append_kernel): thread = (16-byte column, row
-// group); it owns 4 RoPE pairs whose axis (t / y / x) is fixed, so it reads one cos/sin pair per (row, RoPE pair) from
-// the fp64 tables (model state, L1/L2 resident), and keeps the pooled sums of its 8 channels in registers.
+// Grid: a thread-block CLUSTER per key block of the chunk; the CS CTAs of a cluster split the heads (CS = the largest
+// divisor of H that is <= 8).  Phase 1, token-major: one warp per token row streams its CTA's heads of Q and K (16-byte
+// vectors, coalesced) and reduces the partial sums of squares; the partials of the CS CTAs are combined through
+// distributed shared memory (rank order) into r_q[row], r_k[row].  Phase 2, column-major per head (the layout of
+// uf_append_kernel): thread = (16-byte column, row group); it owns 4 RoPE pairs whose axis (t / y / x) is fixed, reads
+// one cos / sin pair per (row, RoPE pair) from the fp32 tables (model state, L1/L2 resident) and keeps the pooled sums
+// of its 8 channels in registers.  The second look at Q, K comes from L1 / L2.
 #include "uf_internal.h"
+
+#include <cooperative_groups.h>
+
+namespace cg = cooperative_groups;
 
 namespace {
 
@@ -32,30 +40,19 @@ __device__ __forceinline__ uint4 ld_stream(const uint4* p) {
 }
 __device__ __forceinline__ uint4 ld_keep(const uint4* p) { return __ldg(p); }
 
-__device__ __forceinline__ double bf16lo(uint32_t w) { return (double)__uint_as_float(w << 16); }
-__device__ __forceinline__ double bf16hi(uint32_t w) { return (double)__uint_as_float(w & 0xFFFF0000u); }
-
-// fp64 -> bf16, round to nearest even on the bits (R-40): returns the bf16 bits and, through *rounded, the rounded
-// value as a double.  keep = exponent (11 bits) + top 7 mantissa bits; the 45 bits below decide the rounding; a carry
-// into the exponent is the right result.  Magnitudes below 2^-126 after rounding become signed zero.
-__device__ __forceinline__ uint32_t round_bf16(double y, double* rounded) {
-  const uint32_t hi = (uint32_t)__double2hiint(y), lo = (uint32_t)__double2loint(y);
-  const uint32_t sign = hi & 0x80000000u, mag = hi & 0x7FFFFFFFu;
-  uint32_t keep = mag >> 13;
-  const uint32_t rest = mag & 0x1FFFu;
-  const bool up = rest > 0x1000u || (rest == 0x1000u && (lo != 0u || (keep & 1u)));
-  keep += up ? 1u : 0u;
-  const uint32_t bias = (1023u - 127u) << 7;
-  const bool small = keep < bias + 128u;
-  *rounded = small ? __hiloint2double((int)sign, 0) : __hiloint2double((int)(sign | (keep << 13)), 0);
-  return (sign >> 16) | (small ? 0u : keep - bias);
+__device__ __forceinline__ float bf16lo(uint32_t w) { return __uint_as_float(w << 16); }
+__device__ __forceinline__ float bf16hi(uint32_t w) { return __uint_as_float(w & 0xFFFF0000u); }
+__device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
+  uint32_t r;
+  asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
+  return r;
 }
 
 struct FusedParams {
   const __nv_bfloat16 *q, *k, *v;
   __nv_bfloat16* q_out;
   int64_t in_ts, in_hs, out_ts, out_hs;
-  const double *cos_tab, *sin_tab;     // [max_pos][D/2]
+  const float *cos_tab, *sin_tab;      // [max_pos][D/2]
   const float *gq, *gk;                // [H*D]
   double eps;
   int t0, Hg, Wg;                      // raster mode: token n -> (t0 + n / (Hg*Wg), (n / Wg) % Hg, n % Wg)
@@ -63,6 +60,7 @@ struct FusedParams {
   __nv_bfloat16 *kc, *vc;
   double *kpool, *qbar;
   int H, B, P, BPC, ntok, phys0, sink_copy_blocks;
+  int CS, HPC;                         // CTAs per cluster, heads per CTA (CS * HPC == H)
   UfTiling til;
 };
 
@@ -89,32 +87,38 @@ uf_fused_append_kernel(const FusedParams a) {
   constexpr int VPR = D / 8;                 // 16-byte vectors per head row
   constexpr int RPP = kThreads / VPR;        // row groups
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  double* r_q = reinterpret_cast<double*>(smem_raw);           // [B]
-  double* r_k = r_q + a.B;                                     // [B]
+  double* part_q = reinterpret_cast<double*>(smem_raw);        // [B] this CTA's partial sums of squares (own heads)
+  double* part_k = part_q + a.B;                               // [B]
+  float* r_q = reinterpret_cast<float*>(part_k + a.B);         // [B]
+  float* r_k = r_q + a.B;                                      // [B]
   int* pos_s = reinterpret_cast<int*>(r_k + a.B);              // [B][3]
   double* red = reinterpret_cast<double*>(pos_s + 3 * a.B + (a.B & 1));   // [2][RPP][D + 2]
-  const int b = blockIdx.x;
+  cg::cluster_group cluster = cg::this_cluster();
+  const int rank = (int)cluster.block_rank();
+  const int b = blockIdx.x / a.CS;
+  const int h0 = rank * a.HPC;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int row0 = b * a.B;
   const int nvalid = a.til.enabled ? uf_tile_nvalid(a.til, b) : min(a.B, a.ntok - row0);
   const int C = a.H * D;
-  const int VT = C / 8;                      // vectors per token row
+  const int VT = a.HPC * VPR;                // vectors of this CTA's heads per token row
 
-  // ---- phase 1: RMS factors of the block's rows (R-37), token-major --------------------------------------------
+  // ---- phase 1: partial sums of squares of this CTA's heads (R-37), token-major --------------------------------
   for (int r = warp; r < nvalid; r += kWarps) {
     const int64_t base = (int64_t)(row0 + r) * a.in_ts;
     double sq = 0.0, sk = 0.0;
     for (int v = lane; v < VT; v += 32) {
-      const int h = v / VPR, c8 = (v % VPR) * 8;
+      const int h = h0 + v / VPR, c8 = (v % VPR) * 8;
       const int64_t off = base + (int64_t)h * a.in_hs + c8;
       const uint4 uq = ld_keep(reinterpret_cast<const uint4*>(a.q + off));
       const uint4 uk = ld_keep(reinterpret_cast<const uint4*>(a.k + off));
       const uint32_t wq[4] = {uq.x, uq.y, uq.z, uq.w}, wk[4] = {uk.x, uk.y, uk.z, uk.w};
 #pragma unroll
       for (int i = 0; i < 4; ++i) {
-        const double q0 = bf16lo(wq[i]), q1 = bf16hi(wq[i]), k0 = bf16lo(wk[i]), k1 = bf16hi(wk[i]);
-        sq = fma(q0, q0, sq); sq = fma(q1, q1, sq);          // x*x is exact in fp64: fma == mul then add
-        sk = fma(k0, k0, sk); sk = fma(k1, k1, sk);
+        const float q0 = bf16lo(wq[i]), q1 = bf16hi(wq[i]), k0 = bf16lo(wk[i]), k1 = bf16hi(wk[i]);
+        // x*x is exact in fp32 (8 x 8 significant bits); the sum runs in fp64 (exact)
+        sq += (double)__fmul_rn(q0, q0); sq += (double)__fmul_rn(q1, q1);
+        sk += (double)__fmul_rn(k0, k0); sk += (double)__fmul_rn(k1, k1);
       }
     }
 #pragma unroll
@@ -123,14 +127,25 @@ uf_fused_append_kernel(const FusedParams a) {
       sk = __dadd_rn(sk, __shfl_xor_sync(0xffffffffu, sk, sh));
     }
     if (lane == 0) {
-      r_q[r] = __ddiv_rn(1.0, __dsqrt_rn(__dadd_rn(__ddiv_rn(sq, (double)C), a.eps)));
-      r_k[r] = __ddiv_rn(1.0, __dsqrt_rn(__dadd_rn(__ddiv_rn(sk, (double)C), a.eps)));
+      part_q[r] = sq; part_k[r] = sk;
       int t, y, x;
       row_pos(a, b, r, &t, &y, &x);
       pos_s[3 * r] = t; pos_s[3 * r + 1] = y; pos_s[3 * r + 2] = x;
     }
   }
-  __syncthreads();
+  cluster.sync();                            // every CTA's partials are visible cluster-wide
+  if (tid < nvalid) {
+    double sq = 0.0, sk = 0.0;
+    for (int k = 0; k < a.CS; ++k) {         // rank order (the sums are exact, so any order gives the same bits)
+      const double* rq = cluster.map_shared_rank(part_q, k);
+      const double* rk = cluster.map_shared_rank(part_k, k);
+      sq = __dadd_rn(sq, rq[tid]);
+      sk = __dadd_rn(sk, rk[tid]);
+    }
+    r_q[tid] = __double2float_rn(__ddiv_rn(1.0, __dsqrt_rn(__dadd_rn(__ddiv_rn(sq, (double)C), a.eps))));
+    r_k[tid] = __double2float_rn(__ddiv_rn(1.0, __dsqrt_rn(__dadd_rn(__ddiv_rn(sk, (double)C), a.eps))));
+  }
+  cluster.sync();                            // remote reads are done before any CTA moves on / exits
 
   // ---- phase 2: per head, column-major: norm * weight, RoPE, round, write, pool --------------------------------
   const int vcx = tid % VPR, rg = tid / VPR;
@@ -144,18 +159,19 @@ uf_fused_append_kernel(const FusedParams a) {
     axis[j] = p < a.pairs_t ? 0 : (p < a.pairs_th ? 1 : 2);
   }
   const uint4 zero = make_uint4(0, 0, 0, 0);
-  for (int h = 0; h < a.H; ++h) {
-    double gqv[8], gkv[8];
+  for (int h = h0; h < h0 + a.HPC; ++h) {
+    float gqv[8], gkv[8];
 #pragma unroll
     for (int e = 0; e < 8; ++e) {
-      gqv[e] = (double)__ldg(a.gq + h * D + vcx * 8 + e);
-      gkv[e] = (double)__ldg(a.gk + h * D + vcx * 8 + e);
+      gqv[e] = __ldg(a.gq + h * D + vcx * 8 + e);
+      gkv[e] = __ldg(a.gk + h * D + vcx * 8 + e);
     }
     double pq[8], pk[8];
 #pragma unroll
     for (int e = 0; e < 8; ++e) { pq[e] = 0.0; pk[e] = 0.0; }
     const int64_t dst = (((int64_t)h * a.P + phys) * a.B) * D;
     const int64_t dst_sink = (((int64_t)h * a.P + b) * a.B) * D;
+#pragma unroll 2
     for (int r = rg; r < a.B; r += RPP) {
       uint4 oq = zero, ok = zero, ov = zero;
       if (r < nvalid) {
@@ -165,33 +181,29 @@ uf_fused_append_kernel(const FusedParams a) {
         ov = ld_stream(reinterpret_cast<const uint4*>(a.v + src));
         const uint32_t wq[4] = {uq.x, uq.y, uq.z, uq.w}, wk[4] = {uk.x, uk.y, uk.z, uk.w};
         uint32_t rq[4], rk[4];
-        const double rq_f = r_q[r], rk_f = r_k[r];
+        const float rq_f = r_q[r], rk_f = r_k[r];
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
           const int pos = pos_s[3 * r + axis[j]];
           const int64_t ti = (int64_t)pos * (D / 2) + vcx * 4 + j;
-          const double cs = __ldg(a.cos_tab + ti), sn = __ldg(a.sin_tab + ti);
-          // q
+          const float cs = __ldg(a.cos_tab + ti), sn = __ldg(a.sin_tab + ti);
           {
-            const double ue = __dmul_rn(__dmul_rn(bf16lo(wq[j]), rq_f), gqv[2 * j]);
-            const double uo = __dmul_rn(__dmul_rn(bf16hi(wq[j]), rq_f), gqv[2 * j + 1]);
-            const double oe = __dsub_rn(__dmul_rn(ue, cs), __dmul_rn(uo, sn));
-            const double oo = __dadd_rn(__dmul_rn(ue, sn), __dmul_rn(uo, cs));
-            double re, ro;
-            const uint32_t be = round_bf16(oe, &re), bo = round_bf16(oo, &ro);
-            rq[j] = be | (bo << 16);
-            pq[2 * j] += re; pq[2 * j + 1] += ro;
+            const float ue = __fmul_rn(__fmul_rn(bf16lo(wq[j]), rq_f), gqv[2 * j]);
+            const float uo = __fmul_rn(__fmul_rn(bf16hi(wq[j]), rq_f), gqv[2 * j + 1]);
+            const float oe = __fsub_rn(__fmul_rn(ue, cs), __fmul_rn(uo, sn));
+            const float oo = __fadd_rn(__fmul_rn(ue, sn), __fmul_rn(uo, cs));
+            const uint32_t w = pack_bf16x2(oe, oo);
+            rq[j] = w;
+            pq[2 * j] += (double)bf16lo(w); pq[2 * j + 1] += (double)bf16hi(w);   // the ROUNDED values (exact sums)
           }
-          // k
           {
-            const double ue = __dmul_rn(__dmul_rn(bf16lo(wk[j]), rk_f), gkv[2 * j]);
-            const double uo = __dmul_rn(__dmul_rn(bf16hi(wk[j]), rk_f), gkv[2 * j + 1]);
-            const double oe = __dsub_rn(__dmul_rn(ue, cs), __dmul_rn(uo, sn));
-            const double oo = __dadd_rn(__dmul_rn(ue, sn), __dmul_rn(uo, cs));
-            double re, ro;
-            const uint32_t be = round_bf16(oe, &re), bo = round_bf16(oo, &ro);
-            rk[j] = be | (bo << 16);
-            pk[2 * j] += re; pk[2 * j + 1] += ro;
+            const float ue = __fmul_rn(__fmul_rn(bf16lo(wk[j]), rk_f), gkv[2 * j]);
+            const float uo = __fmul_rn(__fmul_rn(bf16hi(wk[j]), rk_f), gkv[2 * j + 1]);
+            const float oe = __fsub_rn(__fmul_rn(ue, cs), __fmul_rn(uo, sn));
+            const float oo = __fadd_rn(__fmul_rn(ue, sn), __fmul_rn(uo, cs));
+            const uint32_t w = pack_bf16x2(oe, oo);
+            rk[j] = w;
+            pk[2 * j] += (double)bf16lo(w); pk[2 * j + 1] += (double)bf16hi(w);
           }
         }
         oq = make_uint4(rq[0], rq[1], rq[2], rq[3]);
@@ -254,8 +266,22 @@ cudaError_t uf_launch_fused_append(uf_ctx* c, const UfView& v, const __nv_bfloat
   a.sink_copy_blocks = v.cur_chunk == 0 ? min(uf_ceil_div(v.sink_ntok, v.B), nb) : 0;
   a.til = v.til;
   constexpr int D = 128;
-  const size_t smem = (size_t)2 * v.B * 8 + (size_t)(3 * v.B + (v.B & 1)) * 4 + (size_t)2 * (kThreads / (D / 8)) * (D + 2) * 8;
-  uf_fused_append_kernel<D><<<nb, kThreads, smem, s>>>(a);
+  int cs = 1;
+  for (int k = 8; k >= 1; --k) if (v.H % k == 0) { cs = k; break; }   // largest divisor of H that fits a portable cluster
+  a.CS = cs; a.HPC = v.H / cs;
+  const size_t smem = (size_t)2 * v.B * 8 + (size_t)2 * v.B * 4 + (size_t)(3 * v.B + (v.B & 1)) * 4 +
+                      (size_t)2 * (kThreads / (D / 8)) * (D + 2) * 8;
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)(nb * cs));
+  cfg.blockDim = dim3(kThreads);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = s;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = (unsigned)cs; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  cudaError_t e = cudaLaunchKernelEx(&cfg, uf_fused_append_kernel<D>, a);
   c->launches += 1;
-  return cudaGetLastError();
+  return e != cudaSuccess ? e : cudaGetLastError();
 }

@@ -255,7 +255,7 @@ def compare_paper_step(got: dict, ref: dict, where: str = ""):
 
 # ------------------------------------------------------------------------------------ fused QK-norm + RoPE + append (NEXT-2)
 class RopeState:
-    """Model state of the fused step on the device: fp64 cos / sin tables and fp32 norm weights (inputs of both sides)."""
+    """Model state of the fused step on the device: fp32 cos / sin tables and fp32 norm weights (inputs of both sides)."""
 
     def __init__(self, w: wl.Workload, max_pos: int, device):
         import torch
@@ -303,8 +303,8 @@ def oracle_fused_step(orc: UFOracle, rs: RopeState, w: wl.Workload, Qb, Kb, Vb, 
     """oracle: norm + RoPE (oracle/uf_rope_norm.py) -> bf16 bits -> the ordinary oracle step on them"""
     n = Qb.shape[0]
     pos = rope_norm.raster_positions(n, w.grid_h, w.grid_w, t0)
-    q2 = rope_norm.apply(bits_to_f64(Qb), rs.gq.astype(np.float64), rs.cos, rs.sin, pos)
-    k2 = rope_norm.apply(bits_to_f64(Kb), rs.gk.astype(np.float64), rs.cos, rs.sin, pos)
+    q2 = rope_norm.apply(bits_to_f64(Qb), rs.gq, rs.cos, rs.sin, pos)
+    k2 = rope_norm.apply(bits_to_f64(Kb), rs.gk, rs.cos, rs.sin, pos)
     out = oracle_step(orc, q2, k2, Vb, **kw)
     out["q_out_bits"], out["k_bits"] = q2, k2
     return out

@@ -188,12 +188,13 @@ ROPE_AXIS_DIMS = (44, 42, 42)        # PAPER.md:343 "3D RoPE with axis dims (44,
 
 
 def rope_tables(max_pos: int, dims=ROPE_AXIS_DIMS, theta: float = 10000.0):
-    """cos / sin tables a Wan2.1-style model precomputes once: fp64 [max_pos, d/2]; column i of the axis segment of
-    dim D holds cos / sin(pos * theta**(-2 i / D)).  An INPUT of the step (both sides read the same numbers); the
-    oracle states the definition they must satisfy (oracle/uf_rope_norm.py: rope_table) and a CPU test compares."""
+    """cos / sin tables a Wan2.1-style model precomputes once: float32 [max_pos, d/2] (computed in fp64, stored in
+    fp32); column i of the axis segment of dim D holds cos / sin(pos * theta**(-2 i / D)).  An INPUT of the step
+    (both sides read the same numbers); the oracle states the definition they must satisfy
+    (oracle/uf_rope_norm.py: rope_table) and a CPU test compares."""
     freq = np.concatenate([theta ** (-(2.0 * np.arange(D // 2, dtype=np.float64)) / D) for D in dims])
     ang = np.outer(np.arange(max_pos, dtype=np.float64), freq)
-    return np.cos(ang), np.sin(ang)
+    return np.cos(ang).astype(np.float32), np.sin(ang).astype(np.float32)
 
 
 def norm_weights(w: Workload, seed: int = 20_000):
