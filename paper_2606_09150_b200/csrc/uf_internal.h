@@ -154,7 +154,7 @@ struct uf_ctx {
   static constexpr int kTmCache = 8;
   TmEntry tm_cache[kTmCache];
   int tm_cache_n = 0, tm_cache_next = 0;
-  size_t score_smem_attr[2][3][4] = {};   // dynamic-smem limit already set on uf_score_topk_kernel<d, QG>
+  size_t score_smem_attr[4][3][4] = {};   // dynamic-smem limit already set on uf_score_topk_kernel<d, QG>
   std::string err;
 };
 

@@ -69,7 +69,7 @@ __device__ __forceinline__ unsigned long long sortable(double x) {
 // current chunk as its last "prior"), the top-k' is taken over all of them and THEN intersected with the r x r
 // window M_local; the query block's own key block is always kept.  Rows then differ in length: sel_cnt holds
 // each row's count and idx_out rows (out_stride entries) are padded with -1.
-template <int D, int kQG, bool kPaper>
+template <int D, int kQG, bool kPaper, int kPF>
 __global__ void __launch_bounds__(kScoreThreads)
 uf_score_topk_kernel(UfView v, const double* __restrict__ qbar, const double* __restrict__ kpool,
                      int nqb, int k_eff, int32_t* __restrict__ sel_q, int32_t* __restrict__ sel_rank, int kcap,
@@ -100,16 +100,28 @@ uf_score_topk_kernel(UfView v, const double* __restrict__ qbar, const double* __
     double acc[kQG];
 #pragma unroll
     for (int g = 0; g < kQG; ++g) acc[g] = 0.0;
-    // 16 pooled-K loads in flight at a time; the additions stay in index order (R-4)
-    for (int t0 = 0; t0 < D; t0 += 16) {
-      double kv[16];
+    // pooled-K loads run one batch of kPF ahead of the arithmetic (the loads are L2 hits ~700 cycles away; the dot
+    // product itself is a dependent chain); the additions stay in index order (R-4)
+    double kv[kPF], kn[kPF];
 #pragma unroll
-      for (int u = 0; u < 16; ++u) kv[u] = __ldg(kp + (int64_t)(t0 + u) * v.P);
+    for (int u = 0; u < kPF; ++u) kv[u] = __ldg(kp + (int64_t)u * v.P);
+#pragma unroll 1
+    for (int t0 = 0; t0 < D; t0 += kPF) {
+      if (t0 + kPF < D) {
 #pragma unroll
-      for (int u = 0; u < 16; ++u) {
-#pragma unroll
-        for (int g = 0; g < kQG; ++g) acc[g] = __dadd_rn(acc[g], __dmul_rn(qs[g * D + t0 + u], kv[u]));
+        for (int u = 0; u < kPF; ++u) kn[u] = __ldg(kp + (int64_t)(t0 + kPF + u) * v.P);
       }
+#pragma unroll
+      for (int u = 0; u < kPF; u += 2) {
+#pragma unroll
+        for (int g = 0; g < kQG; ++g) {
+          const double2 q2 = *reinterpret_cast<const double2*>(qs + g * D + t0 + u);   // one 16-byte broadcast read
+          acc[g] = __dadd_rn(acc[g], __dmul_rn(q2.x, kv[u]));
+          acc[g] = __dadd_rn(acc[g], __dmul_rn(q2.y, kv[u + 1]));
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < kPF; ++u) kv[u] = kn[u];
     }
 #pragma unroll
     for (int g = 0; g < kQG; ++g) key[(int64_t)g * nc + j] = sortable(__ddiv_rn(acc[g], inv) + 0.0);
@@ -305,25 +317,34 @@ cudaError_t uf_launch_select(uf_ctx* c, const UfView& v, const __nv_bfloat16* q,
   }
   dim3 gp(nqb, v.H);
   cudaError_t e = cudaSuccess;
-  int qg = 8;
+#ifndef UF_SCORE_QG_MAX
+#define UF_SCORE_QG_MAX 8
+#endif
+  int qg = UF_SCORE_QG_MAX;
   auto smem_for = [&](int g) { return (size_t)g * v.d * 8 + (size_t)g * v.n_cand * 8; };
   while (qg > 1 && smem_for(qg) > 160 * 1024) qg >>= 1;
   const size_t smem = smem_for(qg);
   if (smem > 200 * 1024) return cudaErrorInvalidConfiguration;     // > ~25k candidates: not supported
   dim3 gs(uf_ceil_div(nqb, qg), v.H);
-#define UF_SCORE_LAUNCH2(DD, QG, PP)                                                                         \
+  const bool deep_prefetch = (int64_t)gs.x * gs.y <= 2 * (int64_t)c->sm_count;
+#define UF_SCORE_LAUNCH3(DD, QG, PP, PF)                                                                     \
   {                                                                                                          \
-    size_t& attr = c->score_smem_attr[PP ? 1 : 0][DD == 32 ? 0 : DD == 64 ? 1 : 2]                           \
+    size_t& attr = c->score_smem_attr[(PP ? 1 : 0) + (PF == 16 ? 2 : 0)][DD == 32 ? 0 : DD == 64 ? 1 : 2]    \
                                      [QG == 8 ? 0 : QG == 4 ? 1 : QG == 2 ? 2 : 3];                          \
     if (smem > 48 * 1024 && smem > attr) {          /* raise the limit once, not on every call */             \
-      e = cudaFuncSetAttribute(uf_score_topk_kernel<DD, QG, PP>, cudaFuncAttributeMaxDynamicSharedMemorySize,\
-                               (int)smem);                                                                   \
+      e = cudaFuncSetAttribute(uf_score_topk_kernel<DD, QG, PP, PF>,                                         \
+                               cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);                      \
       if (e != cudaSuccess) return e;                                                                        \
       attr = smem;                                                                                           \
     }                                                                                                        \
-    uf_score_topk_kernel<DD, QG, PP><<<gs, kScoreThreads, smem, s>>>(                                        \
+    uf_score_topk_kernel<DD, QG, PP, PF><<<gs, kScoreThreads, smem, s>>>(                                    \
         v, c->qbar, c->kpool, nqb, k_eff, c->sel_q, c->sel_rank, c->kcap, c->sel_cnt, idx_out, cnt_out,      \
         out_stride, usage_cur);                                                                              \
+  }
+  /* few CTAs per SM: latency-bound, prefetch deep (16 loads ahead, 122 registers); many: keep the occupancy */
+#define UF_SCORE_LAUNCH2(DD, QG, PP)                                                                         \
+  {                                                                                                          \
+    if (deep_prefetch) UF_SCORE_LAUNCH3(DD, QG, PP, 16) else UF_SCORE_LAUNCH3(DD, QG, PP, 4)                 \
   }
 #define UF_SCORE_LAUNCH(DD, QG)                                                                              \
   {                                                                                                          \
@@ -350,6 +371,7 @@ cudaError_t uf_launch_select(uf_ctx* c, const UfView& v, const __nv_bfloat16* q,
 #undef UF_SELECT_CASE
 #undef UF_SCORE_LAUNCH
 #undef UF_SCORE_LAUNCH2
+#undef UF_SCORE_LAUNCH3
   c->launches += 1;
   e = cudaGetLastError();
   if (e != cudaSuccess) return e;
