@@ -203,3 +203,89 @@ def norm_weights(w: Workload, seed: int = 20_000):
     n = w.n_heads * w.head_dim
     return ((1.0 + 0.1 * g.standard_normal(n)).astype(np.float32),
             (1.0 + 0.1 * g.standard_normal(n)).astype(np.float32))
+
+
+# ---------------------------------------------------------------------------
+# Causal memory network: shapes, random-init weights, input frames
+# ---------------------------------------------------------------------------
+
+@dataclasses.dataclass(frozen=True)
+class CmnWorkload:
+    """One causal-memory-network configuration on a latent grid.  Input generation only."""
+    name: str
+    in_ch: int
+    out_ch: int
+    stage_channels: tuple          # per stage (+ optionally the width after the last channel transition)
+    n_blocks: int
+    spatial_factors: tuple
+    temporal_factors: tuple
+    height: int                    # input latent grid
+    width: int
+    frames_per_chunk: int
+
+
+# PAPER.md:345: the streaming latent upsampler; input = the LR latent of BASELINE.json's 1K workload (the HR latent
+# grid 136 x 240 of 1088 x 1920 halved), chunk = 3 latent frames as in BASELINE.json configs[1]
+CMN_CONFIGS = {
+    "cmn_tiny": CmnWorkload("cmn_tiny", 16, 16, (64, 64), 2, (2, 1), (1, 2), 12, 20, 2),
+    "cmn_upsampler_1k": CmnWorkload("cmn_upsampler_1k", 16, 16, (256, 128, 64), 3, (2, 1, 1), (1, 1, 1), 68, 120, 3),
+    # PAPER.md:347: the HR decoder, on a quarter-area crop of the 1K HR latent (the full 136 x 240 input makes
+    # 1088 x 1920 x 12 frames of 64-channel activations per chunk)
+    "cmn_decoder_crop": CmnWorkload("cmn_decoder_crop", 16, 3, (256, 128, 64, 64), 3, (2, 2, 2), (1, 2, 2), 68, 120, 1),
+}
+
+
+def cmn_param_shapes(c: CmnWorkload):
+    """[(name, shape)] in network order; `<name>.b` biases exist for every entry except `*.skip`"""
+    n_stages = len(c.spatial_factors)
+    ch = list(c.stage_channels)
+    out = [("in", (ch[0], c.in_ch, 3, 3))]
+    for s in range(n_stages):
+        for b in range(c.n_blocks):
+            p = f"s{s}.b{b}."
+            out += [(p + "c1", (ch[s], 2 * ch[s], 3, 3)), (p + "c2", (ch[s], ch[s], 3, 3)),
+                    (p + "c3", (ch[s], ch[s], 3, 3)), (p + "skip", (ch[s], ch[s]))]
+        r, t = c.spatial_factors[s], c.temporal_factors[s]
+        out.append((f"s{s}.up", (ch[s] * r * r, ch[s], 3, 3)))
+        if t > 1:
+            out.append((f"s{s}.texp", (ch[s] * t, ch[s])))
+        nxt = ch[s + 1] if s + 1 < len(ch) else ch[s]
+        out.append((f"s{s}.ch", (nxt, ch[s])))
+    last = ch[n_stages] if n_stages < len(ch) else ch[n_stages - 1]
+    out.append(("out", (c.out_ch, last, 3, 3)))
+    return out
+
+
+def cmn_weights(c: CmnWorkload, seed: int = 30_000) -> dict:
+    """Random-init stand-in for the trained network: every weight ~ N(0, gain / fan_in) rounded to bf16 (stored as
+    float32 holding bf16 values), biases ~ 0.05 N(0,1) as float32.  gain 2 keeps ReLU activations O(1) through the
+    depth (He init); W_skip and the 1x1 / output layers use gain 1."""
+    g = np.random.default_rng(seed)
+    wt = {}
+    for name, shape in cmn_param_shapes(c):
+        fan_in = int(np.prod(shape[1:]))
+        gain = 2.0 if name.endswith(("c1", "c2", "in")) else 1.0
+        w = g.standard_normal(shape).astype(np.float32) * np.float32(math.sqrt(gain / fan_in))
+        wt[name] = bf16_bits_to_f32(f32_to_bf16_bits(w))
+        if not name.endswith("skip"):
+            wt[name + ".b"] = (0.05 * g.standard_normal(shape[0])).astype(np.float32)
+    return wt
+
+
+def cmn_frames(c: CmnWorkload, chunk: int, frames: int | None = None) -> np.ndarray:
+    """bf16 bit patterns [F, H, W, in_ch] of chunk `chunk`: N(0,1) + a smooth field drifting over time (a latent video
+    stand-in: neighbouring frames correlate, so the memory path matters)"""
+    F = c.frames_per_chunk if frames is None else frames
+    g = np.random.default_rng(40_000 + chunk)
+    x = g.standard_normal((F, c.height, c.width, c.in_ch)).astype(np.float32) * np.float32(0.5)
+    t = (chunk * c.frames_per_chunk + np.arange(F, dtype=np.float32))[:, None, None, None]
+    yy = np.arange(c.height, dtype=np.float32)[None, :, None, None] / c.height
+    xx = np.arange(c.width, dtype=np.float32)[None, None, :, None] / c.width
+    ph = np.arange(c.in_ch, dtype=np.float32)[None, None, None, :]
+    x += np.sin(2 * np.pi * (yy * (1 + ph % 3) + xx * (1 + ph % 2) + 0.05 * t) + ph).astype(np.float32)
+    return f32_to_bf16_bits(x)
+
+
+def scaled_cmn(c: CmnWorkload, name: str | None = None, **kw) -> CmnWorkload:
+    """the same network on another grid / chunk length (CPU-seconds parity cases)"""
+    return dataclasses.replace(c, name=name or c.name, **kw)
