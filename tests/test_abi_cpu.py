@@ -32,6 +32,25 @@ def test_library_exports_every_declared_symbol(lib):
     assert "sm_100a" in uf.uf_version()
 
 
+def test_library_exports_every_symbol_of_uf_cmn_h(lib):
+    from paper_2606_09150_b200 import cmn_binding
+    hdr = open(os.path.join(ROOT, "include", "uf_cmn.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = sorted(set(re.findall(r"\b(uf_cmn_[a-z_0-9]+)\s*\(", hdr)))
+    assert declared == sorted(cmn_binding.CMN_SYMBOLS), (declared, sorted(cmn_binding.CMN_SYMBOLS))
+    for name in declared:
+        assert hasattr(lib, name), f"libuf.so does not export {name}"
+    # no GPU here: creating a network fails loudly (no CPU fallback), unsupported widths are refused first
+    with pytest.raises(uf.UFError) as e:
+        uf.uf_cmn_create(16, 16, (48,), 1, (1,), (1,), 8, 8, 1)
+    assert e.value.code == binding.UF_ERR_UNSUPPORTED
+    import torch
+    if not torch.cuda.is_available():
+        with pytest.raises(uf.UFError) as e:
+            uf.uf_cmn_create(16, 16, (64,), 1, (1,), (1,), 8, 8, 1)
+        assert e.value.code == binding.UF_ERR_CUDA
+
+
 def test_library_contains_sm100a_tensor_core_code():
     """The shipped binary holds sm_100a SASS with tcgen05 MMA (UTC*MMA), TMEM loads (LDTM) and TMA."""
     import shutil

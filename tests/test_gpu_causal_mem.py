@@ -1,0 +1,129 @@
+"""GPU parity of the causal memory network streaming step (NEXT-4, include/uf_cmn.h) against
+oracle/uf_causal_mem.py on the same seeded weights and frames: every layer element by element on identical inputs
+(one bf16 ulp), network outputs and per-block memories end to end (rounding-noise bound), over streams cut into
+ragged chunks; grids that span several CTA tiles with ragged edges; the paper's
+two configurations (P:345 upsampler, P:347 decoder) on reduced grids and the upsampler at BASELINE.json's 1K size."""
+import numpy as np
+import pytest
+
+import uf_workloads as wl
+import uf_harness as hz
+
+pytestmark = pytest.mark.gpu
+
+
+def _run_stream(c, chunks, frames_max=None, layerwise=True):
+    """stream of sum(chunks) frames cut into the given chunk lengths.  Per chunk: (1) every layer of the step against
+    the oracle's layer function on the same inputs (one-ulp bound, uf_harness.cmn_layer_check); (2) the network
+    output against the oracle's variant A over the whole stream (rounding-noise bound, uf_harness.compare_cmn);
+    at the end (3) every block memory against the streaming oracle (variant B)."""
+    cm, cfg, wt = hz.cmn_oracle(c)
+    T = sum(chunks)
+    zb = wl.cmn_frames(c, 0, T)
+    z = hz.bits_to_f64(zb)
+    ref = cm.forward_parallel(z, cfg, wt)
+    cu = hz.CmnCuda(c, frames_max=frames_max or max(chunks))
+    ts, nl = cu.ts, cu.uf.uf_cmn_n_layers(cu.net)
+    try:
+        f0, stats, mem_prev = 0, [], {}
+        for i, n in enumerate(chunks):
+            got = cu.step(zb[f0:f0 + n])
+            st = hz.compare_cmn(got, ref[f0 * ts:(f0 + n) * ts], nl, f"[{c.name} chunk {i}]")
+            if layerwise:
+                st["layer_min_frac_equal"] = hz.cmn_layerwise(cu, cm, cfg, wt, z[f0:f0 + n], got, mem_prev,
+                                                              f"[{c.name} chunk {i}]")
+            stats.append(st)
+            f0 += n
+        # memory of every block == the block's input at the last frame (R-41), from the streaming oracle
+        so = cm.CausalMemStream(cfg, wt)
+        so.step(z)
+        for s in range(cfg.n_stages):
+            for b in range(cfg.n_blocks):
+                hz.compare_cmn(cu.memory(s, b)[None], so.mem[f"s{s}.b{b}."], nl, f"[{c.name} memory s{s}.b{b}]")
+        assert cu.uf.uf_cmn_launches(cu.net) == len(chunks) * nl
+        assert cu.uf.uf_cmn_flops(cu.net, 1) == cm.flop_count(cfg, c.height, c.width, 1)
+        return stats
+    finally:
+        cu.close()
+
+
+def test_tiny_network_ragged_chunks_and_memories():
+    c = wl.CMN_CONFIGS["cmn_tiny"]                      # 12 x 20 grid: ragged in both directions, r = (2,1), s = (1,2)
+    print(_run_stream(c, [2, 1, 2]))
+
+
+def test_reset_starts_a_new_stream_and_single_frames():
+    c = wl.CMN_CONFIGS["cmn_tiny"]
+    cm, cfg, wt = hz.cmn_oracle(c)
+    zb = wl.cmn_frames(c, 0, 3)
+    ref = cm.forward_parallel(hz.bits_to_f64(zb), cfg, wt)
+    cu = hz.CmnCuda(c, frames_max=3)
+    try:
+        a = cu.step(zb)
+        cu.reset()
+        b = np.concatenate([cu.step(zb[i:i + 1]) for i in range(3)], axis=0)     # frame by frame after a reset
+        assert np.array_equal(a, b)
+        hz.compare_cmn(a, ref, cu.uf.uf_cmn_n_layers(cu.net), "[reset]")
+        # without the reset the first frame sees the previous stream's last frame: a different result
+        c2 = cu.step(zb[:1])
+        assert not np.array_equal(c2, a[:cu.ts])
+    finally:
+        cu.close()
+
+
+def test_multi_tile_grid_with_ragged_edges():
+    # 37 x 75: 5 tile rows (last 5 of 8 rows), 2 CTA tiles of 64 columns (MT = 4; last 11 of 64), several frames
+    c = wl.scaled_cmn(wl.CMN_CONFIGS["cmn_tiny"], "cmn_ragged", height=37, width=75, frames_per_chunk=3)
+    _run_stream(c, [3, 2])
+
+
+@pytest.mark.parametrize("r", [1, 3])
+def test_spatial_factors_1_and_3(r):
+    c = wl.CmnWorkload(f"cmn_r{r}", 16, 16, (64,), 1, (r,), (1,), 10, 18, 2)
+    _run_stream(c, [2, 2])
+
+
+def test_wide_channels_n256_and_n128_paths():
+    # the upsampler's widths on a small grid: N = 256 tiles with MT = 2, the 1024-column PixelShuffle conv
+    # in 4 N tiles, N = 128 with MT = 4, N = 64 double-buffered
+    c = wl.scaled_cmn(wl.CMN_CONFIGS["cmn_upsampler_1k"], "cmn_upsampler_small", height=20, width=36, frames_per_chunk=2)
+    _run_stream(c, [2, 1])
+
+
+def test_decoder_configuration_small():
+    # spatial (2,2,2), temporal (1,2,2), out_ch = 3 (scalar stores), widths (256,128,64,64)
+    c = wl.scaled_cmn(wl.CMN_CONFIGS["cmn_decoder_crop"], "cmn_decoder_small", height=6, width=10, frames_per_chunk=1)
+    _run_stream(c, [1, 1])
+
+
+def test_upsampler_full_1k_chunk():
+    # BASELINE.json's 1K grid: LR latent 68 x 120, chunk of 3 latent frames -> 136 x 240 (the launch configuration
+    # bench.py times); two chunks so that the second one runs on real memories
+    c = wl.CMN_CONFIGS["cmn_upsampler_1k"]
+    st = _run_stream(c, [3, 3])
+    print("cmn_upsampler_1k parity:", st)
+
+
+def test_argument_errors():
+    import paper_2606_09150_b200 as uf
+    with pytest.raises(uf.UFError) as e:
+        uf.uf_cmn_create(16, 16, (48,), 1, (1,), (1,), 8, 8, 1)
+    assert e.value.code == uf.binding.UF_ERR_UNSUPPORTED
+    c = wl.CMN_CONFIGS["cmn_tiny"]
+    net = uf.uf_cmn_create(c.in_ch, c.out_ch, c.stage_channels, c.n_blocks, c.spatial_factors, c.temporal_factors,
+                           c.height, c.width, 2, 0)
+    try:
+        import torch
+        z = torch.zeros((2, c.height, c.width, c.in_ch), dtype=torch.bfloat16, device="cuda")
+        out = torch.zeros((4, c.height * 2, c.width * 2, c.out_ch), dtype=torch.bfloat16, device="cuda")
+        with pytest.raises(uf.UFError) as e:
+            uf.uf_cmn_step(net, z, 2, out)                 # parameters never set
+        assert e.value.code == uf.binding.UF_ERR_STATE
+        with pytest.raises(uf.UFError) as e:
+            uf.uf_cmn_set_param(net, "nope", np.zeros(4, np.uint16))
+        assert e.value.code == uf.binding.UF_ERR_INVALID_ARG
+        with pytest.raises(uf.UFError) as e:
+            uf.uf_cmn_set_param(net, "s0.b0.skip", np.zeros((64, 64, 1, 1), np.uint16), np.zeros(64, np.float32))
+        assert e.value.code == uf.binding.UF_ERR_INVALID_ARG
+    finally:
+        uf.uf_cmn_destroy(net)
