@@ -576,6 +576,117 @@ def run_reference(args, w):
 
 
 # --------------------------------------------------------------------------------------------------
+# causal memory network streaming step (include/uf_cmn.h)
+CMN_METRIC = "effective TFLOP/s of the causal memory network streaming step (ms/chunk in ms_per_step)"
+
+
+def cmn_cpu_oracle(cw, budget_frames: int = 1):
+    """the oracle's streaming step timed on host cores on a bounded crop of the workload (same network, same
+    weights, a 20 x 36 grid, one frame): a reported baseline, TFLOP/s by the definition's FLOP count"""
+    from oracle import uf_causal_mem as cm
+    crop = wl.scaled_cmn(cw, cw.name + "_crop20x36", height=20, width=36, frames_per_chunk=budget_frames)
+    cfg = cm.CmnConfig(crop.in_ch, crop.out_ch, tuple(crop.stage_channels), crop.n_blocks,
+                       tuple(crop.spatial_factors), tuple(crop.temporal_factors))
+    wt = {k: v.astype(np.float64) for k, v in wl.cmn_weights(crop).items()}
+    z = wl.bf16_bits_to_f32(wl.cmn_frames(crop, 0)).astype(np.float64)
+    st = cm.CausalMemStream(cfg, wt)
+    t0 = time.perf_counter()
+    st.step(z)
+    dt = time.perf_counter() - t0
+    fl = cm.flop_count(cfg, crop.height, crop.width, budget_frames)
+    return {"value": fl / dt / 1e12, "unit": UNIT, "cores": len(os.sched_getaffinity(0)), "kind": "oracle",
+            "blas_threads": blas_threads(), "seconds": dt,
+            "sample": f"oracle/uf_causal_mem.py CausalMemStream.step (NumPy fp64) on {budget_frames} frame(s) of a "
+                      f"{crop.height} x {crop.width} crop of workload {cw.name} ({fl / 1e9:.1f} GFLOP)"}
+
+
+def measure_cmn(cw, device, steps, warmup, with_e2e=True, with_cpu=True):
+    """device-resident steps of uf_cmn_step over a rotating set of chunks (+ e2e with pinned host frames in and the
+    output back per step); the whole step is launches of ONE kernel template, so the roofline object is the step's"""
+    import torch
+    import paper_2606_09150_b200 as uf
+    dev = torch.device("cuda", device)
+    torch.cuda.set_device(dev)
+    stream = torch.cuda.current_stream(dev)
+    F = cw.frames_per_chunk
+    rs, ts = int(np.prod(cw.spatial_factors)), int(np.prod(cw.temporal_factors))
+    net = uf.uf_cmn_create(cw.in_ch, cw.out_ch, cw.stage_channels, cw.n_blocks, cw.spatial_factors,
+                           cw.temporal_factors, cw.height, cw.width, F, device)
+    try:
+        wt = wl.cmn_weights(cw)
+        for i in range(uf.uf_cmn_n_params(net)):
+            name, shape, has_bias = uf.uf_cmn_param_info(net, i)
+            w = np.ascontiguousarray(wl.f32_to_bf16_bits(wt[name]).reshape(shape))
+            uf.uf_cmn_set_param(net, name, w, np.ascontiguousarray(wt[name + ".b"]) if has_bias else None)
+        n_rot = 4
+        host = [torch.from_numpy(wl.cmn_frames(cw, c).view(np.int16)).pin_memory() for c in range(n_rot)]
+        z_dev = [h.to(dev).view(torch.bfloat16) for h in host]
+        out_shape = (F * ts, cw.height * rs, cw.width * rs, cw.out_ch)
+        out = torch.empty(out_shape, dtype=torch.bfloat16, device=dev)
+        out_host = torch.empty(out_shape, dtype=torch.bfloat16).pin_memory()
+        z_stage = torch.empty_like(z_dev[0])
+        uf.uf_cmn_reset(net, stream)
+
+        def run(n, e2e):
+            for i in range(n):
+                if e2e:
+                    z_stage.view(torch.int16).copy_(host[i % n_rot], non_blocking=True)
+                    uf.uf_cmn_step(net, z_stage, F, out, stream)
+                    out_host.copy_(out, non_blocking=True)
+                else:
+                    uf.uf_cmn_step(net, z_dev[i % n_rot], F, out, stream)
+
+        def timed(n, e2e):
+            run(warmup, e2e)
+            torch.cuda.synchronize(dev)
+            barrier()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            l0 = uf.uf_cmn_launches(net)
+            e0.record(stream)
+            run(n, e2e)
+            e1.record(stream)
+            torch.cuda.synchronize(dev)
+            barrier()
+            return e0.elapsed_time(e1), uf.uf_cmn_launches(net) - l0
+
+        with ClockSampler(device) as cs:
+            total_ms, launches = timed(steps, False)
+        flop = uf.uf_cmn_flops(net, F)
+        m = {"total_ms": total_ms, "steps": steps, "flop": flop, "launches": launches, "clocks": cs.summary(),
+             "device_bytes": uf.uf_cmn_device_bytes(net), "n_layers": uf.uf_cmn_n_layers(net),
+             "h2d": int(host[0].numel() * 2), "d2h": int(out.numel() * 2)}
+        if with_e2e:
+            m["e2e_ms"], _ = timed(steps, True)
+        if with_cpu:
+            m["cpu"] = cmn_cpu_oracle(cw)
+        return m
+    finally:
+        uf.uf_cmn_destroy(net)
+
+
+def cmn_entry(cw, m, peaks):
+    steps = m["steps"]
+    t = m["flop"] * steps / (m["total_ms"] * 1e-3) / 1e12
+    e = {"workload": f"{cw.name} (PAPER.md:345-347 network: widths {list(cw.stage_channels)}, {cw.n_blocks} blocks/stage, "
+                     f"spatial {list(cw.spatial_factors)}, temporal {list(cw.temporal_factors)}; input {cw.frames_per_chunk} x "
+                     f"{cw.height} x {cw.width} x {cw.in_ch} per chunk)",
+         "metric": CMN_METRIC, "steps": steps, "ms_per_step": m["total_ms"] / steps, "value": t, "unit": UNIT,
+         "tflop_per_step": m["flop"] / 1e12, "gpu_launches": m["launches"], "layers_per_step": m["n_layers"],
+         "ctx_device_bytes": m["device_bytes"], "clocks": m["clocks"],
+         "roofline": {"kernel": "uf_cmn_conv_kernel (every layer of the step is a launch of it)", "bound": "tensor",
+                      "achieved": t, "peak": peaks["bf16_burst"], "unit": UNIT, "frac": t / peaks["bf16_burst"],
+                      "traffic": None, "peak_source": peaks["source"] + ", bf16 burst",
+                      "algorithmic_flop_per_step": m["flop"],
+                      "note": "FLOP by the definition (real channel counts); time = the whole step incl. launch gaps"}}
+    if "e2e_ms" in m:
+        e["e2e"] = {"value": m["flop"] * steps / (m["e2e_ms"] * 1e-3) / 1e12, "unit": UNIT,
+                    "ms_per_step": m["e2e_ms"] / steps, "h2d_bytes_per_step": m["h2d"], "d2h_bytes_per_step": m["d2h"]}
+    if "cpu" in m:
+        e["cpu_baseline"] = m["cpu"]
+    return e
+
+
+# --------------------------------------------------------------------------------------------------
 def measure_workload(w, device, steps, warmup, with_e2e=True, stream_repeats=5, fused=False):
     """device-resident steps (+ attention events), per-call breakdown, optional e2e leg, optional rolling stream"""
     ids = range(w.n_stream_chunks) if w.n_stream_chunks else range(w.capacity_chunks + 1)
@@ -633,18 +744,62 @@ def also_entry(w, m, peaks):
     return e
 
 
+def cmn_main(args):
+    """--workload cmn_*: the causal memory network step as its own line (used for its ncu captures)"""
+    import torch
+    cw = wl.CMN_CONFIGS[args.workload]
+    if args.impl == "reference":
+        if int(os.environ.get("RANK", "0")) == 0:
+            cb = cmn_cpu_oracle(cw)
+            print(json.dumps({"impl": "reference", "metric": CMN_METRIC, "value": cb["value"], "unit": UNIT,
+                              "n_gpus": args.gpus, "steps": 1, "warmup": 0, "ms_per_step": 1e3 * cb["seconds"],
+                              "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+                              "data": "synthetic", "config": {"workload": cw.name}, "cpu_baseline": cb,
+                              "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0,
+                                      "d2h_bytes_per_step": 0}, "gpu_launches": 0}), flush=True)
+        return
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    rank, world, local = dist_setup(args.gpus)
+    device = local if world > 1 else 0
+    peaks = load_peaks()
+    m = measure_cmn(cw, device, args.steps, max(3, args.warmup), with_cpu=(rank == 0 and not args.no_cpu_baseline))
+    e = cmn_entry(cw, m, peaks)
+    dev = torch.device("cuda", device)
+    total_ms, units = aggregate_over_ranks(m["total_ms"], float(m["flop"]) * args.steps, dev)
+    line = {"metric": CMN_METRIC, "value": units / (total_ms * 1e-3) / 1e12, "unit": UNIT, "n_gpus": world,
+            "steps": args.steps, "warmup": max(3, args.warmup), "ms_per_step": total_ms / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+            "config": {"workload": e["workload"], "step": "uf_cmn_step (every layer a tcgen05 implicit-GEMM launch)",
+                       "tflop_per_step": e["tflop_per_step"], "l2": "activations of a step exceed L2 only at the "
+                       "decoder sizes; inputs rotate over 4 chunks", "parallelism": "replicas only" if world > 1 else "single GPU"},
+            "e2e": e.get("e2e"), "gpu_launches": e["gpu_launches"], "clocks": e["clocks"], "roofline": e["roofline"]}
+    if "cpu_baseline" in e:
+        line["cpu_baseline"] = e["cpu_baseline"]
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+        dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=5)
-    ap.add_argument("--workload", default="1k", choices=["1k", "2k", "wide", "1k_stream", "1k_paper", "2k_paper"])
+    ap.add_argument("--workload", default="1k", choices=["1k", "2k", "wide", "1k_stream", "1k_paper", "2k_paper",
+                                                         "cmn_upsampler_1k", "cmn_decoder_crop"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-also", action="store_true", help="skip the secondary workloads (2k, wide, 1k_stream, paper-mask variants)")
-    ap.add_argument("--also", default="2k,1k_stream,wide,1k_paper,2k_paper,1k_fused,2k_fused",
+    ap.add_argument("--also", default="2k,1k_stream,wide,1k_paper,2k_paper,1k_fused,2k_fused,cmn_upsampler_1k,cmn_decoder_crop",
                     help="comma list of secondary workloads (x_fused = workload x through uf_qkv_rope_append)")
     args = ap.parse_args()
+    if args.workload.startswith("cmn_"):
+        cmn_main(args)
+        return
     w = wl.CONFIGS[args.workload]
     if args.impl == "reference":
         run_reference(args, wl.CONFIGS["1k"] if w.tile else w)
@@ -700,6 +855,11 @@ def main():
     if rank == 0 and n_ranks == 1 and not args.no_also and args.workload == "1k":
         line["also"] = {}
         for name in [x for x in args.also.split(",") if x]:
+            if name.startswith("cmn_"):
+                cw = wl.CMN_CONFIGS[name]
+                line["also"][name] = cmn_entry(cw, measure_cmn(cw, device, max(3, args.steps // 2), 3,
+                                                               with_cpu=not args.no_cpu_baseline), peaks)
+                continue
             fused = name.endswith("_fused")
             w2 = wl.CONFIGS[name[:-6] if fused else name]
             steps2 = max(3, args.steps // 2)
