@@ -47,7 +47,7 @@ struct ConvParams {
   int cchunks[kMaxSrc];             // 64-channel slices of each source
   int fshift[kMaxSrc];              // frame coordinate of output frame f in the source buffer = f + fshift
   int F, H, W;                      // frames of this launch, conv grid (= source grid)
-  int tiles_x, tiles_y;             // CTA tiles per frame: 8 rows x 16*MT columns
+  int tiles_x, tiles_y;             // 128-pixel tiles per frame: 8 rows x 16 columns each
   int n_ntiles, N;                  // N tiles, GEMM columns per tile (multiple of 16, <= 256)
   int nA, nB;                       // ring depths
   int n_acc;                        // accumulator buffers in TMEM (1 or 2)
@@ -105,24 +105,38 @@ uf_cmn_conv_kernel(const __grid_constant__ CUtensorMap tm_a0, const __grid_const
   tc_fence_after();
   const uint32_t tmem = *tmem_ptr_smem;
 
+  // Work = cells (N tile nt, pixel tile mi), nt outer; this CTA owns the contiguous range [cell_lo, cell_hi) of a
+  // balanced split and walks it in groups of up to MT pixel tiles that share nt (and so every weight tile).
   const int tiles_per_frame = p.tiles_x * p.tiles_y;
-  const int n_tiles = p.F * tiles_per_frame * p.n_ntiles;
+  const int m_tiles = p.F * tiles_per_frame;
+  const int n_cells = m_tiles * p.n_ntiles;
+  const int cq = n_cells / (int)gridDim.x, cr = n_cells % (int)gridDim.x;
+  const int cell_lo = (int)blockIdx.x * cq + min((int)blockIdx.x, cr);
+  const int cell_hi = cell_lo + cq + ((int)blockIdx.x < cr ? 1 : 0);
   const uint32_t acc_stride = (p.n_acc == 2) ? 256u : 0u;
 
-  // tile id -> (N tile, x tile, y tile, frame); the N tile runs fastest so that neighbouring CTAs share A in L2
-#define UF_TILE_DECODE(t)                                     \
-  const int nt = (t) % p.n_ntiles;                            \
-  const int pt = (t) / p.n_ntiles;                            \
-  const int f = pt / tiles_per_frame;                         \
-  const int rem = pt - f * tiles_per_frame;                   \
+#define UF_GROUP_LOOP_BEGIN                                                                 \
+  for (int cell = cell_lo; cell < cell_hi;) {                                               \
+    const int nt = cell / m_tiles;                                                          \
+    const int m0 = cell - nt * m_tiles;                                                     \
+    const int cnt = min(MT, min(cell_hi - cell, m_tiles - m0));
+#define UF_GROUP_LOOP_END cell += cnt; }
+  // pixel tile mi -> frame, first row, first column
+#define UF_MTILE_DECODE(mi)                                   \
+  const int f = (mi) / tiles_per_frame;                       \
+  const int rem = (mi) - f * tiles_per_frame;                 \
   const int y0 = (rem / p.tiles_x) * 8;                       \
-  const int x0 = (rem % p.tiles_x) * (16 * MT);
+  const int x0 = (rem % p.tiles_x) * 16;
+
+  // programmatic dependent launch: everything above (barriers, TMEM, bias) overlapped the previous layer's tail;
+  // from here on this grid reads what that layer wrote and overwrites buffers it may still read
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 
   if (warp == 0) {
     // ================================ TMA producer ================================
     uint32_t as = 0, aph = 0, bs = 0, bph = 0;
-    for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
-      UF_TILE_DECODE(t)
+    UF_GROUP_LOOP_BEGIN
       int kstep = 0;
       for (int s = 0; s < p.n_src; ++s) {
         const CUtensorMap* ta = s == 0 ? &tm_a0 : &tm_a1;
@@ -132,11 +146,12 @@ uf_cmn_conv_kernel(const __grid_constant__ CUtensorMap tm_a0, const __grid_const
           for (int dxi = 0; dxi < ntx; ++dxi) {
             mbar_wait(bA_EMPTY + 8 * as, aph ^ 1);
             if (elect_one()) {
-              mbar_expect_tx(bA_FULL + 8 * as, MT * a_bytes);
-#pragma unroll
-              for (int mt = 0; mt < MT; ++mt)
+              mbar_expect_tx(bA_FULL + 8 * as, cnt * a_bytes);
+              for (int mt = 0; mt < cnt; ++mt) {
+                UF_MTILE_DECODE(m0 + mt)
                 tma_load_4d(base + as * a_stage_bytes + mt * kATileBytes, ta, bA_FULL + 8 * as, cc * 64,
-                            x0 + mt * 16 + dxi - (ntx == 3 ? 1 : 0), y0 - (nty == 3 ? 1 : 0), f + p.fshift[s]);
+                            x0 + dxi - (ntx == 3 ? 1 : 0), y0 - (nty == 3 ? 1 : 0), f + p.fshift[s]);
+              }
             }
             if (++as == (uint32_t)p.nA) { as = 0; aph ^= 1; }
             for (int dyi = 0; dyi < nty; ++dyi) {
@@ -151,13 +166,14 @@ uf_cmn_conv_kernel(const __grid_constant__ CUtensorMap tm_a0, const __grid_const
           }
         }
       }
-    }
+    UF_GROUP_LOOP_END
   } else if (warp == 1) {
     // ================================ MMA issuer ==================================
     // instruction descriptor kind::f16: D fp32, A/B bf16 K-major, M = 128, N = p.N
     const uint32_t idesc = (1u << 4) | (1u << 7) | (1u << 10) | (((uint32_t)p.N >> 3) << 17) | ((128u >> 4) << 24);
     uint32_t as = 0, aph = 0, bs = 0, bph = 0, ab = 0, abph = 0;
-    for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+    UF_GROUP_LOOP_BEGIN
+      (void)nt;
       mbar_wait(bACC_EMPTY + 8 * ab, abph ^ 1);          // the epilogue has drained this accumulator buffer
       tc_fence_after();
       const uint32_t d_base = tmem + ab * acc_stride;
@@ -175,6 +191,7 @@ uf_cmn_conv_kernel(const __grid_constant__ CUtensorMap tm_a0, const __grid_const
                 const uint32_t b_lo = desc_lo(base + off_b + bs * b_stage_bytes);
 #pragma unroll
                 for (int mt = 0; mt < MT; ++mt) {
+                  if (mt >= cnt) break;
                   const uint32_t a_lo = a_lo0 + ((mt * kATileBytes + dyi * 2048) >> 4);
 #pragma unroll
                   for (int k = 0; k < 4; ++k)             // 64 channels = 4 MMAs of K = 16 (32 B along the row)
@@ -192,7 +209,7 @@ uf_cmn_conv_kernel(const __grid_constant__ CUtensorMap tm_a0, const __grid_const
       }
       if (elect_one()) tc_commit(bACC_FULL + 8 * ab);
       if (p.n_acc == 2) { if (++ab == 2) { ab = 0; abph ^= 1; } } else abph ^= 1;
-    }
+    UF_GROUP_LOOP_END
   } else {
     // ================================== epilogue ==================================
     const int q = warp & 3;                              // TMEM lane quarter this warp may access
@@ -200,14 +217,13 @@ uf_cmn_conv_kernel(const __grid_constant__ CUtensorMap tm_a0, const __grid_const
     const int yy = row >> 4, xx = row & 15;
     const uint32_t lane_addr = (uint32_t)(q * 32) << 16;
     uint32_t ab = 0, abph = 0;
-    for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
-      UF_TILE_DECODE(t)
+    UF_GROUP_LOOP_BEGIN
       mbar_wait(bACC_FULL + 8 * ab, abph);
       tc_fence_after();
-      const int y = y0 + yy;
 #pragma unroll 1
-      for (int mt = 0; mt < MT; ++mt) {
-        const int x = x0 + mt * 16 + xx;
+      for (int mt = 0; mt < cnt; ++mt) {
+        UF_MTILE_DECODE(m0 + mt)
+        const int y = y0 + yy, x = x0 + xx;
         const bool valid = (y < p.H) && (x < p.W);
         const uint32_t t_base = tmem + lane_addr + ab * acc_stride + mt * p.N;
 #pragma unroll 1
@@ -249,9 +265,11 @@ uf_cmn_conv_kernel(const __grid_constant__ CUtensorMap tm_a0, const __grid_const
       __syncwarp();
       if (lane == 0) mbar_arrive(bACC_EMPTY + 8 * ab);
       if (p.n_acc == 2) { if (++ab == 2) { ab = 0; abph ^= 1; } } else abph ^= 1;
-    }
+    UF_GROUP_LOOP_END
   }
-#undef UF_TILE_DECODE
+#undef UF_GROUP_LOOP_BEGIN
+#undef UF_GROUP_LOOP_END
+#undef UF_MTILE_DECODE
 
   tc_fence_before();
   __syncthreads();
@@ -338,7 +356,13 @@ struct Layer {
   int H = 0, W = 0, fmul = 1;         // conv grid, frames per input frame
   __nv_bfloat16* w = nullptr;         // device [n_total][K]
   float* bias = nullptr;              // device [n_total]
-  CUtensorMap tm_a[kMaxSrc], tm_b;
+  CUtensorMap tm_a[kMaxSrc];
+  // the N tile is chosen per step from up to two options (n_total split into k or 2k tiles), each with its own
+  // weight tensor map
+  int n_opt = 1, opt_ntile[2] = {0, 0};
+  CUtensorMap tm_b[2];
+  int opt = 0;                        // option of the current plan
+  int plan_frames = -1;               // frames the current plan was made for
   int nA = 2, nB = 4, n_acc = 1;
   size_t smem = 0;
   int64_t flops_per_frame = 0;        // of one INPUT frame of the network
@@ -386,21 +410,50 @@ int add_buf(uf_cmn* n, int H, int W, int C, int fmul, int has_mem) {
   return (int)n->bufs.size() - 1;
 }
 
-// ring depths and M tiles per CTA for a layer, within 227 KB of shared memory
-void plan_layer(Layer& L) {
-  L.n_ntiles = (L.n_total + 255) / 256;
-  while (L.n_total % (16 * L.n_ntiles)) ++L.n_ntiles;      // N tiles are equal and multiples of 16 columns
-  L.n_tile = L.n_total / L.n_ntiles;
-  // M tiles per CTA: as many as fit in TMEM (MT * N <= 512) and shared memory, so that every weight tile is
-  // reused MT times (L2 -> SM traffic is the bound otherwise)
+// N tile, pixel tiles per group (MT) and ring depths of a layer for `frames` frames on `sms` SMs.
+// Cost of an option = cells of the busiest CTA x columns per cell x a measured cost per column (B200, r2c launch
+// list): an M = 128 SS MMA reads 4 KB of A and 32 N bytes of B from shared memory per N/2 tensor cycles, i.e.
+// 96 B/clk at N = 256 but 128 B/clk (the shared-memory port limit) at N = 128 and 192 B/clk at N = 64, next to the
+// TMA writes; measured per unit of work: N = 128 costs 1.45 x, N <= 64 2.5 x what N = 256 costs.  So narrower tiles
+// only pay where they remove a whole round of CTAs.
+double col_cost(int n_tile) { return n_tile > 128 ? 1.0 : n_tile > 64 ? 1.45 : 2.5; }
+
+void plan_layer(Layer& L, int frames, int sms) {
+  const int m_tiles = frames * ((L.H + 7) / 8) * ((L.W + 15) / 16);
+  double best = 1e300;
+  for (int o = 0; o < L.n_opt; ++o) {
+    const int nt = L.opt_ntile[o], n_ntiles = L.n_total / nt;
+    const int cells = m_tiles * n_ntiles;
+    const int grid = cells < sms ? cells : sms;
+    const int per_cta = (cells + grid - 1) / grid;
+    const double cost = per_cta * (double)nt * col_cost(nt);
+    if (cost < best) { best = cost; L.opt = o; }
+  }
+  L.n_tile = L.opt_ntile[L.opt];
+  L.n_ntiles = L.n_total / L.n_tile;
   L.MT = L.n_tile > 128 ? 2 : 4;
   L.n_acc = (L.MT * L.n_tile <= 256) ? 2 : 1;
   L.nA = 2;
   const size_t budget = 227 * 1024 - 1024 - kMaxBias * 4 - 256;
-  size_t a = (size_t)L.nA * L.MT * kATileBytes;
-  int nb = (int)((budget - a) / ((size_t)L.n_tile * 128));
+  const size_t a = (size_t)L.nA * L.MT * kATileBytes;
+  const int nb = (int)((budget - a) / ((size_t)L.n_tile * 128));
   L.nB = nb > 6 ? 6 : nb;
   L.smem = a + (size_t)L.nB * L.n_tile * 128 + kMaxBias * 4 + 256 + 1024;
+  L.plan_frames = frames;
+}
+
+// the N-tile options of a layer: n_total in the fewest equal tiles of <= 256 columns, and twice as many
+void tile_options(Layer& L) {
+  int k = (L.n_total + 255) / 256;
+  while (L.n_total % (16 * k)) ++k;
+  L.opt_ntile[0] = L.n_total / k;
+  L.n_opt = 1;
+  if (L.opt_ntile[0] % 32 == 0 && L.opt_ntile[0] / 2 >= 64) {
+    // halves must not cut a PixelShuffle / channel-to-time group of c_grp columns in an epilogue chunk: both are
+    // multiples of 16, which is all the epilogue needs
+    L.opt_ntile[1] = L.opt_ntile[0] / 2;
+    L.n_opt = 2;
+  }
 }
 
 template <int MT>
@@ -411,8 +464,15 @@ cudaError_t launch_conv(const Layer& L, const ConvParams& p, int grid, cudaStrea
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
-  uf_cmn_conv_kernel<MT><<<grid, kConvThreads, L.smem, s>>>(L.tm_a[0], L.tm_a[L.n_src > 1 ? 1 : 0], L.tm_b, p);
-  return cudaGetLastError();
+  // programmatic dependent launch: the next layer's prologue (barrier init, TMEM allocation, bias load) may start
+  // while this layer's last CTAs finish; the kernel waits (griddepcontrol.wait) before it touches activations
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3(kConvThreads); cfg.dynamicSmemBytes = L.smem; cfg.stream = s;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr; cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, uf_cmn_conv_kernel<MT>, L.tm_a[0], L.tm_a[L.n_src > 1 ? 1 : 0], L.tm_b[L.opt], p);
 }
 
 void build_graph(uf_cmn* n) {
@@ -504,7 +564,7 @@ void build_graph(uf_cmn* n) {
     L.K = k;
     L.n_total = (L.cout + 15) / 16 * 16;
     if (L.c_grp == 0) { L.c_grp = L.n_total; L.c_real = L.cout; } else L.c_real = L.c_grp;
-    plan_layer(L);
+    tile_options(L);
     int64_t macs = 0;
     for (int s = 0; s < L.n_src; ++s) macs += (int64_t)L.ntap[s] * L.cin[s] * L.cout;
     // pixels of this layer per input frame of the network
@@ -575,8 +635,9 @@ int32_t uf_cmn_create(const uf_cmn_config* cfg, uf_cmn** out) {
     if (e == cudaSuccess) e = cudaMemset(L.bias, 0, (size_t)L.n_total * sizeof(float));
     if (e != cudaSuccess) return bail(UF_ERR_CUDA, std::string("cudaMalloc(weights): ") + cudaGetErrorString(e));
     n->dev_bytes += (int64_t)wb + L.n_total * 4;
-    if (!encode_w_map(&L.tm_b, L.w, L.n_total, L.K, L.n_tile))
-      return bail(UF_ERR_CUDA, "cuTensorMapEncodeTiled failed for the weights of " + L.name);
+    for (int o = 0; o < L.n_opt; ++o)
+      if (!encode_w_map(&L.tm_b[o], L.w, L.n_total, L.K, L.opt_ntile[o]))
+        return bail(UF_ERR_CUDA, "cuTensorMapEncodeTiled failed for the weights of " + L.name);
     for (int s = 0; s < L.n_src; ++s) {
       if (L.src_buf[s] < 0) continue;                       // the caller's z: encoded per step
       const Buf& b = n->bufs[L.src_buf[s]];
@@ -712,6 +773,7 @@ int32_t uf_cmn_step(uf_cmn* n, const void* z, int32_t n_frames, void* out, void*
     n->z_ptr = z; n->z_frames = n_frames;
   }
   for (Layer& L : n->layers) {
+    if (L.plan_frames != n_frames * L.fmul) plan_layer(L, n_frames * L.fmul, n->sm_count);
     ConvParams p;
     memset(&p, 0, sizeof(p));
     p.n_src = L.n_src;
@@ -722,7 +784,7 @@ int32_t uf_cmn_step(uf_cmn* n, const void* z, int32_t n_frames, void* out, void*
       p.fshift[i] = has_mem - L.mem[i];
     }
     p.F = n_frames * L.fmul; p.H = L.H; p.W = L.W;
-    p.tiles_x = (L.W + 16 * L.MT - 1) / (16 * L.MT);
+    p.tiles_x = (L.W + 15) / 16;
     p.tiles_y = (L.H + 7) / 8;
     p.n_ntiles = L.n_ntiles; p.N = L.n_tile; p.nA = L.nA; p.nB = L.nB; p.n_acc = L.n_acc;
     p.bias = L.bias; p.n_total = L.n_total; p.relu = L.relu;
@@ -733,8 +795,8 @@ int32_t uf_cmn_step(uf_cmn* n, const void* z, int32_t n_frames, void* out, void*
     } else {
       p.out = static_cast<__nv_bfloat16*>(out); p.out_fbase = 0; p.Hout = n->out_H; p.Wout = n->out_W; p.Cbuf = c.out_ch;
     }
-    const int n_tiles = p.F * p.tiles_x * p.tiles_y * p.n_ntiles;
-    const int grid = n_tiles < n->sm_count ? n_tiles : n->sm_count;
+    const int n_cells = p.F * p.tiles_x * p.tiles_y * p.n_ntiles;
+    const int grid = n_cells < n->sm_count ? n_cells : n->sm_count;
     cudaError_t e = L.MT == 2 ? launch_conv<2>(L, p, grid, s) : launch_conv<4>(L, p, grid, s);
     if (e != cudaSuccess) return cfail(n, UF_ERR_CUDA, "uf_cmn_conv_kernel (" + L.name + "): " + cudaGetErrorString(e));
     ++n->launches;
