@@ -14,8 +14,13 @@
 //   taps dx are separate loads (a shift by one pixel is not swizzle-aligned).
 // B operand: the layer's weights packed at uf_cmn_set_param time as [N][K] bf16 (K order = the loop order below),
 //   2-D TMA boxes of 64 (K) x N.
-// A CTA works on MT horizontally adjacent pixel tiles at once so that every weight tile is loaded once per MT
-//   tiles: the L2 -> SM path (about 42 B/clk/SM) is what bounds a 128 x N tile with K = 64 per step otherwise.
+// CTA PAIRS (cta_group::2): the two CTAs of a cluster form one 256-pixel MMA tile (each CTA's own 128-pixel tile as
+//   its half of A) and each loads only HALF of every weight tile (N/2 rows): an M = 128 single-CTA MMA reads
+//   4 KB (A) + 32 N bytes (B) of shared memory per N/2 cycles — 128 B/clk at N = 128, the port limit, next to the TMA
+//   writes — and ingests the whole weight tile per SM; in a pair it is 4 KB + 16 N bytes.  The leader CTA issues all
+//   MMAs, TMA loads of both CTAs signal the leader's barriers, tcgen05.commit frees stages in both.
+// A pair works on MT such double tiles at once so that every weight tile is loaded once per MT tiles: the L2 -> SM
+//   path (about 42 B/clk/SM) is what bounds a tile with K = 64 per step otherwise.
 // Warps: 0 = TMA producer, 1 = MMA issuer (+ TMEM allocation), 2..5 = epilogue (TMEM -> registers -> + bias,
 //   ReLU, bf16 -> global, with the PixelShuffle / channel-to-time scatter folded into the store address).
 //   Accumulators are double-buffered in TMEM when MT * N <= 256 columns.
@@ -64,7 +69,7 @@ struct ConvParams {
 };
 
 template <int MT>
-__global__ void __launch_bounds__(kConvThreads, 1)
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kConvThreads, 1)
 uf_cmn_conv_kernel(const __grid_constant__ CUtensorMap tm_a0, const __grid_constant__ CUtensorMap tm_a1,
                    const __grid_constant__ CUtensorMap tm_b, const ConvParams p) {
   extern __shared__ unsigned char smem_raw[];
@@ -74,7 +79,9 @@ uf_cmn_conv_kernel(const __grid_constant__ CUtensorMap tm_a0, const __grid_const
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
   const uint32_t a_stage_bytes = MT * kATileBytes;
-  const uint32_t b_stage_bytes = (uint32_t)p.N * 128u;
+  const uint32_t b_stage_bytes = (uint32_t)(p.N / 2) * 128u;     // this CTA's half of the weight tile
+  const uint32_t rank = cluster_ctarank();                        // 0 = leader of the pair
+  const int pair = (int)(blockIdx.x >> 1), n_pairs = (int)(gridDim.x >> 1);
   const uint32_t off_b = p.nA * a_stage_bytes;
   const uint32_t off_bias = off_b + p.nB * b_stage_bytes;
   const uint32_t off_bar = off_bias + kMaxBias * 4;
@@ -90,36 +97,39 @@ uf_cmn_conv_kernel(const __grid_constant__ CUtensorMap tm_a0, const __grid_const
     asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_a1));
     asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_b));
     for (int i = 0; i < 2 * p.nA + 2 * p.nB + 2; ++i) mbar_init(bars + 8 * i, 1);
-    mbar_init(bACC_EMPTY, 4);
-    mbar_init(bACC_EMPTY + 8, 4);
+    mbar_init(bACC_EMPTY, 8);                          // the 4 epilogue warps of BOTH CTAs arrive on the leader's
+    mbar_init(bACC_EMPTY + 8, 8);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     fence_proxy_async();
   }
   if (warp == 1) {
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32((const void*)tmem_ptr_smem)) : "memory");
-    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32((const void*)tmem_ptr_smem)) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
   }
   for (int i = threadIdx.x; i < p.n_total; i += kConvThreads) bias_s[i] = p.bias[i];
   tc_fence_before();
   __syncthreads();
+  cluster_sync();                                      // the peer's barriers exist before anything signals them
   tc_fence_after();
   const uint32_t tmem = *tmem_ptr_smem;
 
-  // Work = cells (N tile nt, pixel tile mi), nt outer; this CTA owns the contiguous range [cell_lo, cell_hi) of a
-  // balanced split and walks it in groups of up to MT pixel tiles that share nt (and so every weight tile).
+  // Work = cells (N tile nt, double tile di = pixel tiles 2 di and 2 di + 1, one per CTA of the pair), nt outer; a pair
+  // owns the contiguous range [cell_lo, cell_hi) of a balanced split and walks it in groups of up to MT double
+  // tiles that share nt (and so every weight tile).  A pixel tile past the end (odd count) is all zero-fill.
   const int tiles_per_frame = p.tiles_x * p.tiles_y;
   const int m_tiles = p.F * tiles_per_frame;
-  const int n_cells = m_tiles * p.n_ntiles;
-  const int cq = n_cells / (int)gridDim.x, cr = n_cells % (int)gridDim.x;
-  const int cell_lo = (int)blockIdx.x * cq + min((int)blockIdx.x, cr);
-  const int cell_hi = cell_lo + cq + ((int)blockIdx.x < cr ? 1 : 0);
+  const int d_tiles = (m_tiles + 1) / 2;
+  const int n_cells = d_tiles * p.n_ntiles;
+  const int cq = n_cells / n_pairs, cr = n_cells % n_pairs;
+  const int cell_lo = pair * cq + min(pair, cr);
+  const int cell_hi = cell_lo + cq + (pair < cr ? 1 : 0);
   const uint32_t acc_stride = (p.n_acc == 2) ? 256u : 0u;
 
 #define UF_GROUP_LOOP_BEGIN                                                                 \
   for (int cell = cell_lo; cell < cell_hi;) {                                               \
-    const int nt = cell / m_tiles;                                                          \
-    const int m0 = cell - nt * m_tiles;                                                     \
-    const int cnt = min(MT, min(cell_hi - cell, m_tiles - m0));
+    const int nt = cell / d_tiles;                                                          \
+    const int m0 = cell - nt * d_tiles;                                                     \
+    const int cnt = min(MT, min(cell_hi - cell, d_tiles - m0));
 #define UF_GROUP_LOOP_END cell += cnt; }
   // pixel tile mi -> frame, first row, first column
 #define UF_MTILE_DECODE(mi)                                   \
@@ -146,19 +156,21 @@ uf_cmn_conv_kernel(const __grid_constant__ CUtensorMap tm_a0, const __grid_const
           for (int dxi = 0; dxi < ntx; ++dxi) {
             mbar_wait(bA_EMPTY + 8 * as, aph ^ 1);
             if (elect_one()) {
-              mbar_expect_tx(bA_FULL + 8 * as, cnt * a_bytes);
+              if (rank == 0) mbar_expect_tx(bA_FULL + 8 * as, 2 * cnt * a_bytes);      // both CTAs' bytes
               for (int mt = 0; mt < cnt; ++mt) {
-                UF_MTILE_DECODE(m0 + mt)
-                tma_load_4d(base + as * a_stage_bytes + mt * kATileBytes, ta, bA_FULL + 8 * as, cc * 64,
-                            x0 + dxi - (ntx == 3 ? 1 : 0), y0 - (nty == 3 ? 1 : 0), f + p.fshift[s]);
+                UF_MTILE_DECODE(2 * (m0 + mt) + (int)rank)                                // past the end: frame out of range
+                tma_load_4d_2sm(base + as * a_stage_bytes + mt * kATileBytes, ta, bA_FULL + 8 * as, cc * 64,
+                                x0 + dxi - (ntx == 3 ? 1 : 0), y0 - (nty == 3 ? 1 : 0),
+                                f < p.F ? f + p.fshift[s] : 0x100000);
               }
             }
             if (++as == (uint32_t)p.nA) { as = 0; aph ^= 1; }
             for (int dyi = 0; dyi < nty; ++dyi) {
               mbar_wait(bB_EMPTY + 8 * bs, bph ^ 1);
               if (elect_one()) {
-                mbar_expect_tx(bB_FULL + 8 * bs, b_stage_bytes);
-                tma_load_2d(base + off_b + bs * b_stage_bytes, &tm_b, bB_FULL + 8 * bs, kstep * 64, nt * p.N);
+                if (rank == 0) mbar_expect_tx(bB_FULL + 8 * bs, 2 * b_stage_bytes);
+                tma_load_2d_2sm(base + off_b + bs * b_stage_bytes, &tm_b, bB_FULL + 8 * bs, kstep * 64,
+                                nt * p.N + (int)rank * (p.N / 2));
               }
               ++kstep;
               if (++bs == (uint32_t)p.nB) { bs = 0; bph ^= 1; }
@@ -168,9 +180,10 @@ uf_cmn_conv_kernel(const __grid_constant__ CUtensorMap tm_a0, const __grid_const
       }
     UF_GROUP_LOOP_END
   } else if (warp == 1) {
-    // ================================ MMA issuer ==================================
-    // instruction descriptor kind::f16: D fp32, A/B bf16 K-major, M = 128, N = p.N
-    const uint32_t idesc = (1u << 4) | (1u << 7) | (1u << 10) | (((uint32_t)p.N >> 3) << 17) | ((128u >> 4) << 24);
+    // ================================ MMA issuer (leader CTA only) ================
+    // instruction descriptor kind::f16: D fp32, A/B bf16 K-major, M = 256 over the pair, N = p.N
+    const uint32_t idesc = (1u << 4) | (1u << 7) | (1u << 10) | (((uint32_t)p.N >> 3) << 17) | ((256u >> 4) << 24);
+    if (rank == 0) {
     uint32_t as = 0, aph = 0, bs = 0, bph = 0, ab = 0, abph = 0;
     UF_GROUP_LOOP_BEGIN
       (void)nt;
@@ -195,21 +208,22 @@ uf_cmn_conv_kernel(const __grid_constant__ CUtensorMap tm_a0, const __grid_const
                   const uint32_t a_lo = a_lo0 + ((mt * kATileBytes + dyi * 2048) >> 4);
 #pragma unroll
                   for (int k = 0; k < 4; ++k)             // 64 channels = 4 MMAs of K = 16 (32 B along the row)
-                    mma_ss(d_base + mt * p.N, a_lo + k * 2, b_lo + k * 2, idesc, (first && k == 0) ? 0u : 1u);
+                    mma_ss_2sm(d_base + mt * p.N, a_lo + k * 2, b_lo + k * 2, idesc, (first && k == 0) ? 0u : 1u);
                 }
-                tc_commit(bB_EMPTY + 8 * bs);
+                tc_commit_2sm(bB_EMPTY + 8 * bs);
               }
               first = false;
               if (++bs == (uint32_t)p.nB) { bs = 0; bph ^= 1; }
             }
-            if (elect_one()) tc_commit(bA_EMPTY + 8 * as);
+            if (elect_one()) tc_commit_2sm(bA_EMPTY + 8 * as);
             if (++as == (uint32_t)p.nA) { as = 0; aph ^= 1; }
           }
         }
       }
-      if (elect_one()) tc_commit(bACC_FULL + 8 * ab);
+      if (elect_one()) tc_commit_2sm(bACC_FULL + 8 * ab);
       if (p.n_acc == 2) { if (++ab == 2) { ab = 0; abph ^= 1; } } else abph ^= 1;
     UF_GROUP_LOOP_END
+    }
   } else {
     // ================================== epilogue ==================================
     const int q = warp & 3;                              // TMEM lane quarter this warp may access
@@ -222,9 +236,9 @@ uf_cmn_conv_kernel(const __grid_constant__ CUtensorMap tm_a0, const __grid_const
       tc_fence_after();
 #pragma unroll 1
       for (int mt = 0; mt < cnt; ++mt) {
-        UF_MTILE_DECODE(m0 + mt)
+        UF_MTILE_DECODE(2 * (m0 + mt) + (int)rank)
         const int y = y0 + yy, x = x0 + xx;
-        const bool valid = (y < p.H) && (x < p.W);
+        const bool valid = (f < p.F) && (y < p.H) && (x < p.W);
         const uint32_t t_base = tmem + lane_addr + ab * acc_stride + mt * p.N;
 #pragma unroll 1
         for (int c0 = 0; c0 < p.N; c0 += 16) {
@@ -263,7 +277,7 @@ uf_cmn_conv_kernel(const __grid_constant__ CUtensorMap tm_a0, const __grid_const
       }
       tc_fence_before();
       __syncwarp();
-      if (lane == 0) mbar_arrive(bACC_EMPTY + 8 * ab);
+      if (lane == 0) mbar_arrive_leader(bACC_EMPTY + 8 * ab);
       if (p.n_acc == 2) { if (++ab == 2) { ab = 0; abph ^= 1; } } else abph ^= 1;
     UF_GROUP_LOOP_END
   }
@@ -273,8 +287,9 @@ uf_cmn_conv_kernel(const __grid_constant__ CUtensorMap tm_a0, const __grid_const
 
   tc_fence_before();
   __syncthreads();
+  cluster_sync();                                      // neither CTA frees TMEM or exits while the other may still use it
   if (warp == 1) {
-    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem) : "memory");
+    asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, 512;" ::"r"(tmem) : "memory");
   }
 }
 
@@ -411,22 +426,22 @@ int add_buf(uf_cmn* n, int H, int W, int C, int fmul, int has_mem) {
 }
 
 // N tile, pixel tiles per group (MT) and ring depths of a layer for `frames` frames on `sms` SMs.
-// Cost of an option = cells of the busiest CTA x columns per cell x a measured cost per column (B200, r2c launch
-// list): an M = 128 SS MMA reads 4 KB of A and 32 N bytes of B from shared memory per N/2 tensor cycles, i.e.
-// 96 B/clk at N = 256 but 128 B/clk (the shared-memory port limit) at N = 128 and 192 B/clk at N = 64, next to the
-// TMA writes; measured per unit of work: N = 128 costs 1.45 x, N <= 64 2.5 x what N = 256 costs.  So narrower tiles
-// only pay where they remove a whole round of CTAs.
-double col_cost(int n_tile) { return n_tile > 128 ? 1.0 : n_tile > 64 ? 1.45 : 2.5; }
+// Cost of an option = cells of the busiest CTA pair x columns per cell x a relative cost per column: per MMA a CTA
+// of a pair reads 4 KB of A and 16 N bytes of B from shared memory per N/2 tensor cycles, i.e. 64 B/clk at N = 256,
+// 96 at N = 128, 160 at N = 64 (above the 128 B/clk port), next to the TMA writes.  Narrower tiles only pay where
+// they remove a whole round of CTA pairs.
+double col_cost(int n_tile) { return n_tile > 128 ? 1.0 : n_tile > 64 ? 1.15 : 1.6; }
 
 void plan_layer(Layer& L, int frames, int sms) {
   const int m_tiles = frames * ((L.H + 7) / 8) * ((L.W + 15) / 16);
+  const int d_tiles = (m_tiles + 1) / 2, pairs = sms / 2;
   double best = 1e300;
   for (int o = 0; o < L.n_opt; ++o) {
     const int nt = L.opt_ntile[o], n_ntiles = L.n_total / nt;
-    const int cells = m_tiles * n_ntiles;
-    const int grid = cells < sms ? cells : sms;
-    const int per_cta = (cells + grid - 1) / grid;
-    const double cost = per_cta * (double)nt * col_cost(nt);
+    const int cells = d_tiles * n_ntiles;
+    const int grid = cells < pairs ? cells : pairs;
+    const int per_pair = (cells + grid - 1) / grid;
+    const double cost = per_pair * (double)nt * col_cost(nt);
     if (cost < best) { best = cost; L.opt = o; }
   }
   L.n_tile = L.opt_ntile[L.opt];
@@ -436,9 +451,9 @@ void plan_layer(Layer& L, int frames, int sms) {
   L.nA = 2;
   const size_t budget = 227 * 1024 - 1024 - kMaxBias * 4 - 256;
   const size_t a = (size_t)L.nA * L.MT * kATileBytes;
-  const int nb = (int)((budget - a) / ((size_t)L.n_tile * 128));
-  L.nB = nb > 6 ? 6 : nb;
-  L.smem = a + (size_t)L.nB * L.n_tile * 128 + kMaxBias * 4 + 256 + 1024;
+  const int nb = (int)((budget - a) / ((size_t)(L.n_tile / 2) * 128));
+  L.nB = nb > 8 ? 8 : nb;
+  L.smem = a + (size_t)L.nB * (L.n_tile / 2) * 128 + kMaxBias * 4 + 256 + 1024;
   L.plan_frames = frames;
 }
 
@@ -636,7 +651,7 @@ int32_t uf_cmn_create(const uf_cmn_config* cfg, uf_cmn** out) {
     if (e != cudaSuccess) return bail(UF_ERR_CUDA, std::string("cudaMalloc(weights): ") + cudaGetErrorString(e));
     n->dev_bytes += (int64_t)wb + L.n_total * 4;
     for (int o = 0; o < L.n_opt; ++o)
-      if (!encode_w_map(&L.tm_b[o], L.w, L.n_total, L.K, L.opt_ntile[o]))
+      if (!encode_w_map(&L.tm_b[o], L.w, L.n_total, L.K, L.opt_ntile[o] / 2))      // a CTA loads half a tile
         return bail(UF_ERR_CUDA, "cuTensorMapEncodeTiled failed for the weights of " + L.name);
     for (int s = 0; s < L.n_src; ++s) {
       if (L.src_buf[s] < 0) continue;                       // the caller's z: encoded per step
@@ -795,8 +810,9 @@ int32_t uf_cmn_step(uf_cmn* n, const void* z, int32_t n_frames, void* out, void*
     } else {
       p.out = static_cast<__nv_bfloat16*>(out); p.out_fbase = 0; p.Hout = n->out_H; p.Wout = n->out_W; p.Cbuf = c.out_ch;
     }
-    const int n_cells = p.F * p.tiles_x * p.tiles_y * p.n_ntiles;
-    const int grid = n_cells < n->sm_count ? n_cells : n->sm_count;
+    const int n_cells = ((p.F * p.tiles_x * p.tiles_y + 1) / 2) * p.n_ntiles;      // (N tile, double pixel tile)
+    const int pairs = n_cells < n->sm_count / 2 ? n_cells : n->sm_count / 2;
+    const int grid = 2 * pairs;
     cudaError_t e = L.MT == 2 ? launch_conv<2>(L, p, grid, s) : launch_conv<4>(L, p, grid, s);
     if (e != cudaSuccess) return cfail(n, UF_ERR_CUDA, "uf_cmn_conv_kernel (" + L.name + "): " + cudaGetErrorString(e));
     ++n->launches;
