@@ -65,6 +65,8 @@ def ncu_attn_dram_bytes(workload: str):
         return None, "no capture committed"
 
 
+ATTN_IMPL = 0          # --attn-impl: which tcgen05 attention kernel uf_sparse_attn_fwd runs (uf_set_attn_impl)
+
 METRIC = "effective TFLOP/s on kept blocks, sparse causal chunk attention step (ms/chunk in ms_per_step)"
 UNIT = "TFLOP/s"
 
@@ -219,9 +221,12 @@ class HotPath:
         self.fused = fused          # NEXT-2: raw Q, K, V in; QK-norm + RoPE + append + pooling in one kernel
         self.H, self.d = w.n_heads, w.head_dim
         self.n = w.n_tiles * w.block if self.paper else w.chunk_tokens      # rows the library sees per chunk
+        self.attn_impl = ATTN_IMPL
         self.ctx = uf.uf_ctx_create(w.n_heads, w.head_dim, w.block, self.n, w.capacity_chunks,
                                     0 if self.paper else w.sink_blocks, w.k_min, device)
         self.stream = torch.cuda.current_stream(self.dev)
+        if self.attn_impl:
+            uf.uf_set_attn_impl(self.ctx, self.attn_impl)
         if self.paper:
             uf.uf_ctx_set_tiling(self.ctx, w.frames_per_chunk, w.grid_h, w.grid_w, *w.tile, w.window)
         self.ts, self.hs = self.H * self.d, self.d
@@ -793,10 +798,14 @@ def main():
                                                          "cmn_upsampler_1k", "cmn_decoder_crop"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--attn-impl", type=int, default=0, choices=[0, 2],
+                    help="uf_set_attn_impl: 0 = the default tcgen05 attention kernel, 2 = the other tcgen05 variant")
     ap.add_argument("--no-also", action="store_true", help="skip the secondary workloads (2k, wide, 1k_stream, paper-mask variants)")
     ap.add_argument("--also", default="2k,1k_stream,wide,1k_paper,2k_paper,1k_fused,2k_fused,cmn_upsampler_1k,cmn_decoder_crop",
                     help="comma list of secondary workloads (x_fused = workload x through uf_qkv_rope_append)")
     args = ap.parse_args()
+    global ATTN_IMPL
+    ATTN_IMPL = args.attn_impl
     if args.workload.startswith("cmn_"):
         cmn_main(args)
         return

@@ -474,8 +474,8 @@ int32_t uf_sparse_attn_fwd(uf_ctx* c, const void* q, void* o, float* lse, int32_
   if (!(softmax_scale >= 0.0f) || std::isinf(softmax_scale)) return fail(c, UF_ERR_INVALID_ARG, "uf_sparse_attn_fwd: bad softmax_scale");
   float scale = softmax_scale == 0.0f ? (float)(1.0 / std::sqrt((double)c->cfg.head_dim)) : softmax_scale;
   UF_CUDA(c, cudaSetDevice(c->cfg.device));
-  const bool fast = (c->cfg.block == 128 && c->cfg.head_dim == 128 && c->attn_impl == 0 && c->tm_ok);
-  if (!fast && c->attn_impl == 0)
+  const bool fast = (c->cfg.block == 128 && c->cfg.head_dim == 128 && c->attn_impl != 1 && c->tm_ok);
+  if (!fast && c->attn_impl != 1)
     return fail(c, UF_ERR_UNSUPPORTED,
                 "uf_sparse_attn_fwd: the tcgen05 kernel needs block == 128 and head_dim == 128; other shapes only run "
                 "on the (slow) CUDA-core kernel after uf_set_attn_impl(ctx, 1)");
@@ -581,7 +581,7 @@ int32_t uf_next_window(uf_ctx* c, const uf_window_policy* p, int32_t* window_chu
 }
 
 int32_t uf_set_attn_impl(uf_ctx* c, int32_t impl) {
-  if (!c || impl < 0 || impl > 1) return UF_ERR_INVALID_ARG;
+  if (!c || impl < 0 || impl > 2) return UF_ERR_INVALID_ARG;
   c->attn_impl = impl;
   return UF_OK;
 }

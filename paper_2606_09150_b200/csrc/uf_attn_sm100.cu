@@ -42,6 +42,7 @@
 // mode (uf_select_blocks_paper) there is no SINK and no implicit CUR: every kept block, the query
 // block's own included, is in the lists, with its valid-row count.
 #include "uf_internal.h"
+#include "uf_sm100_ptx.h"
 
 namespace {
 
@@ -764,6 +765,406 @@ uf_attn_sm100_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_cons
   }
 }
 
+// =====================================================================================================
+// CTA-pair variant (cta_group::2): ONE 128-row query tile per CTA, the two CTAs of a cluster take query blocks
+// (2p, 2p+1) of an item and act as one 256-row MMA tile.
+//   * every K tile is split between the pair by key (CTA r holds keys [64 r, 64 r + 64)), every V tile by column
+//     (CTA r holds columns [64 r, 64 r + 64) of all 128 keys): each SM ingests 32 KB per key block for its tile, as
+//     the two-tiles-per-CTA kernel does, and reads half as much operand data from shared memory per MMA;
+//   * S is TRIPLE-BUFFERED in TMEM (S_0 [0,128), S_1 [128,256), S_2 [256,384), O [384,512)): S(n+3) = Q K(n+3)^T is
+//     issued right after O += P(n) V(n), so softmax(n+1) and softmax(n+2) find their S ready and the tensor pipe
+//     never waits for the softmax of the block it just fed: no softmax -> PV -> QK chain any more.  P(n) aliases
+//     S(n mod 3).  (Two buffers were measured first: the loop P_FULL(n) -> PV(n), QK(n+2) -> S_FULL(n+2) carries the
+//     cross-CTA barrier latencies, about 1000 cycles per turn, and two steps of slack do not cover it: 1610 cycles
+//     per block; three do.)
+//   * both CTAs walk the pair's merged list; a block only the other tile attends is a zero-fill step (P = 0).
+//   * a raise of the reference max decided after block n is applied at the START of step n+1 to m and l, and to O at
+//     the END of step n+1 (O += P(n) V is still in flight at its start; P(n+1) is already relative to the new m and
+//     O += P(n+1) V is issued only after this step's P_FULL arrive).
+// Barriers: TMA loads of both CTAs complete on the LEADER's Q/K/V_FULL; tcgen05.commit multicasts S_FULL, PV_DONE,
+// O_FULL and the ring's EMPTY barriers to both CTAs; the softmax warps of both CTAs arrive on the leader's P_FULL.
+constexpr int kNK2 = 6;                  // K ring stages (half tiles)
+constexpr int kNV2 = 4;                  // V ring stages (half tiles)
+constexpr int kHalfTile = kTile / 2;     // this CTA's half of a K or V tile
+constexpr int kOff2Q = 0;
+constexpr int kOff2K = kOff2Q + kTile;
+constexpr int kOff2V = kOff2K + kNK2 * kHalfTile;
+constexpr int kOff2Bar = kOff2V + kNV2 * kHalfTile;
+enum Bar2 {
+  B2_Q_FULL = 0, B2_Q_EMPTY,
+  B2_K_FULL0 = 2, B2_K_EMPTY0 = B2_K_FULL0 + kNK2,
+  B2_V_FULL0 = B2_K_EMPTY0 + kNK2, B2_V_EMPTY0 = B2_V_FULL0 + kNV2,
+  B2_S_FULL0 = B2_V_EMPTY0 + kNV2, B2_P_FULL0 = B2_S_FULL0 + 3, B2_PV_DONE0 = B2_P_FULL0 + 3, B2_O_FULL = B2_PV_DONE0 + 2, kNumBars2
+};
+constexpr int kOff2TmemPtr = kOff2Bar + kNumBars2 * 8;
+constexpr int kOff2Xc = kOff2TmemPtr + 16;                    // row-pair exchange: [half][row][parity] bytes
+constexpr int kSmemBytes2 = kOff2Xc + 2 * 128 * 2 + 1024;
+constexpr uint32_t kIdescQK2 = (1u << 4) | (1u << 7) | (1u << 10) | ((128u >> 3) << 17) | ((256u >> 4) << 24);
+constexpr uint32_t kIdescPV2 = kIdescQK2 | (1u << 16);
+
+template <bool kSafe>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
+uf_attn_pair_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_o,
+                    const __grid_constant__ CUtensorMap tm_k, const __grid_constant__ CUtensorMap tm_v,
+                    const AttnParams a) {
+  if (kSafe && *a.panic_last != a.seq) return;         // nothing was flagged (both CTAs of a pair see the same value)
+  extern __shared__ unsigned char smem_raw[];
+  const uint32_t raw = smem_u32(smem_raw);
+  const uint32_t base = (raw + 1023u) & ~1023u;
+  unsigned char* base_ptr = smem_raw + (base - raw);
+  const uint32_t bars = base + kOff2Bar;
+  volatile uint32_t* tmem_ptr_smem = reinterpret_cast<volatile uint32_t*>(base_ptr + kOff2TmemPtr);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int rank = (int)ufptx::cluster_ctarank();      // 0 = leader: issues every MMA of the pair
+  const int pair = (int)(blockIdx.x >> 1), n_pairs = (int)(gridDim.x >> 1);
+  const int n_items = a.H * a.np_cur;
+
+  if (warp == 8 && lane == 0) {
+    asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_q));
+    asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_o));
+    asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_k));
+    asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_v));
+  }
+  if (warp == 9 && lane == 0) {
+    for (int i = 0; i < kNumBars2; ++i)
+      mbar_init(bars + i * 8, (i >= B2_P_FULL0 && i < B2_P_FULL0 + 3) ? 2 * kPArrivals : 1u);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    fence_proxy_async();
+  }
+  if (warp == 10) {
+    asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32((const void*)tmem_ptr_smem)) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+  }
+  tc_fence_before();
+  __syncthreads();
+  ufptx::cluster_sync();                               // the peer's barriers exist before anything signals them
+  tc_fence_after();
+  const uint32_t tmem = *tmem_ptr_smem;
+
+#define UF_ITEM_LOOP_BEGIN                                                                      \
+  for (int it = pair; it < n_items; it += n_pairs) {                                            \
+    if (kSafe && a.panic_item[it] != a.seq) continue;                                           \
+    const int h = it / a.np_cur, p = it % a.np_cur;                                             \
+    const int64_t pi = (int64_t)h * a.NP + p;                                                   \
+    const int n_u = __shfl_sync(0xffffffffu, a.pair_cnt[pi], 0);                                \
+    const int32_t* ulist = a.sel_pair + pi * 2 * a.kcap;                                        \
+    const int full_mask = (2 * p + 1 < a.nqb) ? 3 : 1;
+#define UF_ITEM_LOOP_END }
+
+  if (warp >= 8) {
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 80;");
+    if (warp == 8) {
+      // ================================ TMA producer (both CTAs) =====================
+      uint32_t ks = 0, kph = 0, vs = 0, vph = 0, qph = 0;
+      auto load_kv = [&](int phys, int h) {
+        {
+          const uint32_t bf = bars + (B2_K_FULL0 + ks) * 8, dst = base + kOff2K + ks * kHalfTile;
+          mbar_wait(bars + (B2_K_EMPTY0 + ks) * 8, kph ^ 1);
+          if (elect_one()) {
+            if (rank == 0) mbar_expect_tx(bf, 2 * kHalfTile);            // both CTAs' halves land on the leader's barrier
+            const int row = phys * 128 + rank * 64;                     // this CTA's 64 keys
+            ufptx::tma_load_3d_2sm(dst, &tm_k, bf, 0, row, h);
+            ufptx::tma_load_3d_2sm(dst + kHalfTile / 2, &tm_k, bf, 64, row, h);
+          }
+          if (++ks == kNK2) { ks = 0; kph ^= 1; }
+        }
+        {
+          const uint32_t bf = bars + (B2_V_FULL0 + vs) * 8, dst = base + kOff2V + vs * kHalfTile;
+          mbar_wait(bars + (B2_V_EMPTY0 + vs) * 8, vph ^ 1);
+          if (elect_one()) {
+            if (rank == 0) mbar_expect_tx(bf, 2 * kHalfTile);
+            ufptx::tma_load_3d_2sm(dst, &tm_v, bf, rank * 64, phys * 128, h);   // this CTA's 64 columns of all 128 keys
+          }
+          if (++vs == kNV2) { vs = 0; vph ^= 1; }
+        }
+      };
+      UF_ITEM_LOOP_BEGIN
+        (void)full_mask;
+        int32_t nxt = (lane < n_u) ? __ldg(ulist + lane) : 0;
+        {
+          const uint32_t bq = bars + B2_Q_FULL * 8;
+          mbar_wait(bars + B2_Q_EMPTY * 8, qph ^ 1);
+          qph ^= 1;
+          const int row0 = (2 * p + rank) * 128;                        // past the last token (no such tile): zero-filled
+          if (elect_one()) {
+            if (rank == 0) mbar_expect_tx(bq, 2 * kTile);
+            ufptx::tma_load_3d_2sm(base + kOff2Q, &tm_q, bq, 0, row0, h);
+            ufptx::tma_load_3d_2sm(base + kOff2Q + kHalf, &tm_q, bq, 64, row0, h);
+          }
+        }
+        for (int st0 = 0; st0 < n_u; st0 += 32) {
+          const int32_t mine = nxt;
+          if (st0 + 32 + lane < n_u) nxt = __ldg(ulist + st0 + 32 + lane);
+          const int cnt = min(32, n_u - st0);
+          for (int j = 0; j < cnt; ++j) load_kv(uf_entry_phys(__shfl_sync(0xffffffffu, mine, j)), h);
+        }
+        for (int j = 0; j < a.n_sink; ++j) load_kv(j, h);
+        for (int j = 0; j < a.n_cur; ++j) load_kv(a.cur_phys0 + j, h);
+      UF_ITEM_LOOP_END
+    } else if (warp == 9 && rank == 0) {
+      // ================================ MMA issuer (leader CTA) ======================
+      // S(j) = Q K(j)^T for j = 0, 1, 2 up front; then per block n: O += P(n) V(n), S(n+3) = Q K(n+3)^T into buffer n mod 3.
+      const uint32_t q_lo = desc_lo(base + kOff2Q, 16);
+      const uint32_t k_lo_base = desc_lo(base + kOff2K, 16);
+      const uint32_t v_lo_base = desc_lo(base + kOff2V, kHalf);
+      uint32_t ks = 0, kph = 0, vs = 0, vph = 0, qph = 0, pph = 0;      // pph: one parity bit per S / P buffer
+      uint32_t pv_count = 0;                                            // O += P V launches so far
+      auto issue_qk = [&](int buf) {
+        mbar_wait(bars + (B2_K_FULL0 + ks) * 8, kph);
+        tc_fence_after();
+        if (elect_one()) {
+          const uint32_t k_lo = k_lo_base + ks * (kHalfTile >> 4);
+#pragma unroll
+          for (int k = 0; k < 8; ++k)
+            // 16 elements = 32 B along K; the second 64-column box is 16 KB further in the Q tile (128 rows), 8 KB in
+            // this CTA's K half (64 rows)
+            ufptx::mma_ss_2sm(tmem + buf * 128, q_lo + (((k & 3) * 32 + (k >> 2) * kHalf) >> 4),
+                              k_lo + (((k & 3) * 32 + (k >> 2) * (kHalfTile / 2)) >> 4), kIdescQK2, k == 0 ? 0u : 1u);
+          ufptx::tc_commit_2sm(bars + (B2_S_FULL0 + buf) * 8);
+          ufptx::tc_commit_2sm(bars + (B2_K_EMPTY0 + ks) * 8);
+        }
+        if (++ks == kNK2) { ks = 0; kph ^= 1; }
+      };
+      UF_ITEM_LOOP_BEGIN
+        (void)ulist; (void)full_mask;
+        const int n_steps = n_u + a.n_sink + a.n_cur;
+        mbar_wait(bars + B2_Q_FULL * 8, qph);
+        qph ^= 1;
+        for (int j = 0; j < 3 && j < n_steps; ++j) issue_qk(j);
+        for (int n = 0, buf = 0; n < n_steps; ++n, buf = (buf == 2 ? 0 : buf + 1)) {
+          mbar_wait(bars + (B2_P_FULL0 + buf) * 8, (pph >> buf) & 1u);
+          pph ^= 1u << buf;
+          mbar_wait(bars + (B2_V_FULL0 + vs) * 8, vph);
+          tc_fence_after();
+          if (elect_one()) {
+            // B = this CTA's V half: 128 keys x 64 columns, MN-major: 16 keys = 2048 B per K step
+            const uint32_t v_lo = v_lo_base + vs * (kHalfTile >> 4);
+            const uint32_t p_tmem = tmem + buf * 128;
+#pragma unroll
+            for (int k = 0; k < 8; ++k)
+              ufptx::mma_ts_2sm(tmem + 384, p_tmem + (k >> 2) * 64 + (k & 3) * 8, v_lo + k * (2048 >> 4), kDescHi, kIdescPV2,
+                                (n == 0 && k == 0) ? 0u : 1u);
+            ufptx::tc_commit_2sm(bars + (B2_V_EMPTY0 + vs) * 8);
+            ufptx::tc_commit_2sm(bars + (B2_PV_DONE0 + (pv_count & 1u)) * 8);
+          }
+          ++pv_count;
+          if (++vs == kNV2) { vs = 0; vph ^= 1; }
+          if (n + 3 < n_steps) issue_qk(buf);
+        }
+        if (elect_one()) ufptx::tc_commit_2sm(bars + B2_O_FULL * 8);
+      UF_ITEM_LOOP_END
+    }
+  } else {
+    // ================================== softmax + epilogue (both CTAs) ======================
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 208;");
+    const int wq = warp & 3;                           // TMEM lane quarter
+    const int half = warp >> 2;                        // which 64 keys of a block / 64 columns of O
+    const int row = wq * 32 + lane;
+    const uint32_t lane_addr = (uint32_t)(wq * 32) << 16;
+    const uint32_t col0 = (uint32_t)half * 64;
+    const float sl2 = a.sl2;
+    const uint64_t sl22 = pack2(sl2, sl2);
+    volatile uint8_t* xc = reinterpret_cast<volatile uint8_t*>(base_ptr + kOff2Xc);     // [half][row][parity]
+    volatile uint8_t* x_own = xc + (half * 128 + row) * 2;
+    volatile uint8_t* x_oth = xc + ((half ^ 1) * 128 + row) * 2;
+    const uint32_t o_tmem = tmem + lane_addr + 384 + col0;
+    uint32_t sph = 0, oph = 0;                         // sph: one parity bit per S buffer
+    uint32_t pv_seen = 0;                              // O += P V launches of this CTA pair before the current step
+
+    UF_ITEM_LOOP_BEGIN
+      const bool tile_exists = (full_mask >> rank) & 1;
+      float m = -INFINITY, l = 0.f;
+      int d_own = 0, par = 0, n = 0, buf = 0;
+      bool first = true;
+
+      // multiply this thread's half of the O row by f; O must be quiescent: every O += P V issued so far is complete
+      // (PV_DONE of the previous step) and the next one waits for this step's P_FULL
+      // The tensor pipe may lag the softmax by up to two blocks, so O += P V number g signals PV_DONE[g & 1]: of that
+      // barrier's phases the one before ((g - 2): complete, S_FULL of this step was committed after it) and the
+      // one waited for are the only candidates, and the parity wait cannot alias.
+      auto rescale_o = [&](float f) {
+        const uint32_t g = pv_seen - 1;
+        mbar_wait(bars + (B2_PV_DONE0 + (g & 1u)) * 8, (g >> 1) & 1u);
+        tc_fence_after();
+#pragma unroll
+        for (int cc = 0; cc < 64; cc += 32) {
+          uint32_t ov[32];
+          UF_TMEM_LD32(o_tmem + cc, ov, 0);
+          UF_TMEM_WAIT_LD32(ov);
+#pragma unroll
+          for (int c = 0; c < 32; ++c) ov[c] = __float_as_uint(__uint_as_float(ov[c]) * f);
+          UF_TMEM_ST32(o_tmem + cc, ov, 0);
+        }
+      };
+
+      auto softmax_step = [&](const bool attend, const int nvalid) {
+        const uint32_t s_tmem = tmem + lane_addr + buf * 128 + col0;       // this thread's 64 S columns
+        const int left = nvalid - (int)col0;
+        mbar_wait(bars + (B2_S_FULL0 + buf) * 8, (sph >> buf) & 1u);
+        sph ^= 1u << buf;
+        tc_fence_after();
+        // the two threads of a row step together (S_FULL no longer implies that the partner finished the last step)
+        asm volatile("bar.sync %0, 64;" ::"r"(2 + wq) : "memory");
+        uint32_t sa[32], sb[32], pk[16];
+        float f_o = 1.0f;                              // pending factor for O (applied at the end of the step)
+        if (!kSafe && !first) {
+          const int D = max(d_own, (int)x_oth[par ^ 1]);
+          if (D > 0) {
+            f_o = __int_as_float((127 - D) << 23);     // 2^-D
+            l *= f_o;
+            m += (float)D;
+          }
+        }
+        int Dnew = 0;
+        if (attend) {
+          if (kSafe || first) {
+            float mx0 = -INFINITY, mx1 = -INFINITY;
+#pragma unroll
+            for (int c = 0; c < 2; ++c) {
+              UF_TMEM_LD32(s_tmem + c * 32, sa, 0);
+              UF_TMEM_WAIT_LD32(sa);
+#pragma unroll
+              for (int u = 0; u < 32; u += 2) {
+                const float v0 = (c * 32 + u < left) ? __uint_as_float(sa[u]) : -INFINITY;
+                const float v1 = (c * 32 + u + 1 < left) ? __uint_as_float(sa[u + 1]) : -INFINITY;
+                if (u & 2) mx1 = max3(mx1, v0, v1); else mx0 = max3(mx0, v0, v1);
+              }
+            }
+            const uint32_t mine = bf16_bits_up(fmaxf(mx0, mx1));
+            *reinterpret_cast<volatile uint16_t*>(x_own) = (uint16_t)mine;
+            asm volatile("bar.sync %0, 64;" ::"r"(2 + wq) : "memory");
+            const uint32_t theirs = *reinterpret_cast<volatile uint16_t*>(x_oth);
+            const float rowmax = fmaxf(__uint_as_float(mine << 16), __uint_as_float(theirs << 16));
+            asm volatile("bar.sync %0, 64;" ::"r"(2 + wq) : "memory");
+            const float m_new = fmaxf(m, rowmax * sl2);
+            if (first) {
+              m = m_new;
+              first = false;
+            } else if ((m_new - m) > kRescaleThreshold) {          // kSafe only
+              f_o = ex2(m - m_new);
+              m = m_new;
+              l *= f_o;
+            }
+          }
+          const uint64_t nm2 = pack2(-m, -m);
+          uint64_t acc0 = pack2(0.f, 0.f), acc1 = acc0;
+          UF_TMEM_LD32(s_tmem + 0, sa, 0);
+          UF_TMEM_WAIT_LD32(sa);
+          UF_TMEM_LD32(s_tmem + 32, sb, 0);
+          exp_chunk(sa, pk, half * 2 + 0, left, sl22, nm2, acc0, acc1);
+          UF_TMEM_ST16(s_tmem + 0, pk);
+          UF_TMEM_WAIT_LD32(sb);
+          exp_chunk(sb, pk, half * 2 + 1, left - 32, sl22, nm2, acc0, acc1);
+          UF_TMEM_ST16(s_tmem + 16, pk);
+          float a0, a1, b0, b1;
+          unpack2(acc0, a0, a1);
+          unpack2(acc1, b0, b1);
+          const float lsum = (a0 + a1) + (b0 + b1);
+          l += lsum;
+          if (!kSafe && !(lsum <= 256.0f)) {
+            if (lsum < kPanicSum) {
+              Dnew = (int)((__float_as_uint(lsum) >> 23) & 0xffu) - 126;
+            } else {
+              a.panic_item[it] = a.seq;
+              *a.panic_last = a.seq;
+              Dnew = 101;
+            }
+          }
+        } else {
+          // a block only the other tile of the pair attends: P = 0
+#pragma unroll
+          for (int c = 0; c < 16; ++c) pk[c] = 0u;
+          UF_TMEM_ST16(s_tmem + 0, pk);
+          UF_TMEM_ST16(s_tmem + 16, pk);
+        }
+        if (!kSafe) {
+          x_own[par] = (uint8_t)Dnew;
+          d_own = Dnew;
+        }
+        par ^= 1;
+        // O still holds the blocks before this one relative to the old m
+        if (__any_sync(0xffffffffu, f_o != 1.0f) && n > 0) rescale_o(f_o);
+        tmem_wait_st();
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) ufptx::mbar_arrive_leader(bars + (B2_P_FULL0 + buf) * 8);
+        ++n;
+        buf = (buf == 2) ? 0 : buf + 1;
+        ++pv_seen;
+      };
+
+      {
+        int32_t mine = 0;
+        for (int st = 0; st < n_u; ++st) {
+          if ((st & 31) == 0) mine = (st + lane < n_u) ? __ldg(ulist + st + lane) : 0;
+          const int32_t e = __shfl_sync(0xffffffffu, mine, st & 31);
+          softmax_step(((uf_entry_mask(e) >> rank) & 1) != 0, uf_entry_nvalid(e));
+        }
+        for (int j = 0; j < a.n_sink + a.n_cur; ++j) {
+          const int nvalid = (j < a.n_sink) ? min(128, a.sink_ntok - j * 128) : min(128, a.ntok - (j - a.n_sink) * 128);
+          softmax_step(tile_exists, nvalid);
+        }
+      }
+
+      // ---- epilogue: O / l -> bf16 -> swizzled staging (the Q buffer) -> TMA store ----
+      {
+        unsigned char* stage = base_ptr + kOff2Q;
+        mbar_wait(bars + B2_O_FULL * 8, oph);          // every MMA of the item is complete: Q is free too
+        oph ^= 1;
+        tc_fence_after();
+        volatile float* xl = reinterpret_cast<volatile float*>(stage);
+        xl[half * 128 + row] = l;
+        asm volatile("bar.sync 1, 256;" ::: "memory");
+        const float l_tot = l + xl[(half ^ 1) * 128 + row];
+        asm volatile("bar.sync 1, 256;" ::: "memory");
+        const float inv = 1.0f / l_tot;
+#pragma unroll
+        for (int cc = 0; cc < 64; cc += 32) {
+          uint32_t ov[32];
+          UF_TMEM_LD32(o_tmem + cc, ov, 0);
+          UF_TMEM_WAIT_LD32(ov);
+          unsigned char* half_base = stage + half * kHalf + row * 128;
+#pragma unroll
+          for (int j = 0; j < 4; ++j) {
+            uint4 w;
+            w.x = pack_bf16x2(__uint_as_float(ov[8 * j + 0]) * inv, __uint_as_float(ov[8 * j + 1]) * inv);
+            w.y = pack_bf16x2(__uint_as_float(ov[8 * j + 2]) * inv, __uint_as_float(ov[8 * j + 3]) * inv);
+            w.z = pack_bf16x2(__uint_as_float(ov[8 * j + 4]) * inv, __uint_as_float(ov[8 * j + 5]) * inv);
+            w.w = pack_bf16x2(__uint_as_float(ov[8 * j + 6]) * inv, __uint_as_float(ov[8 * j + 7]) * inv);
+            const int chunk = (cc >> 3) + j;
+            *reinterpret_cast<uint4*>(half_base + ((chunk ^ (row & 7)) << 4)) = w;
+          }
+        }
+        tc_fence_before();
+        fence_proxy_async();
+        asm volatile("bar.sync 1, 256;" ::: "memory");
+        const int row0 = (2 * p + rank) * 128;
+        if (warp == 0 && lane == 0) {
+          if (tile_exists) {
+            const uint32_t src = base + kOff2Q;
+            tma_store_3d(&tm_o, src, 0, row0, h);
+            tma_store_3d(&tm_o, src + kHalf, 64, row0, h);
+            tma_store_commit_and_wait_read();
+          }
+          mbar_arrive(bars + B2_Q_EMPTY * 8);
+        }
+        if (tile_exists && half == 0 && a.lse != nullptr && row0 + row < a.ntok)
+          a.lse[(int64_t)h * a.ntok + row0 + row] = (m + log2f(l_tot)) * 0.6931471805599453f;
+      }
+    UF_ITEM_LOOP_END
+    if (warp == 0 && lane == 0) tma_store_wait_all();
+  }
+#undef UF_ITEM_LOOP_BEGIN
+#undef UF_ITEM_LOOP_END
+
+  tc_fence_before();
+  __syncthreads();
+  ufptx::cluster_sync();                               // neither CTA frees TMEM or exits while the other may still use it
+  if (warp == 10) {
+    asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, 512;" ::"r"(tmem) : "memory");
+  }
+}
+
 typedef CUresult (*PFN_encodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                     const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                     CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -781,12 +1182,13 @@ PFN_encodeTiled get_encode_fn() {
 }
 
 // bf16 tensor [rows, H, 128] with element strides (row_stride, head_stride, 1); box = 64 x 128 x 1
-bool encode_map(CUtensorMap* m, const void* ptr, uint64_t rows, uint64_t H, uint64_t row_stride, uint64_t head_stride) {
+bool encode_map(CUtensorMap* m, const void* ptr, uint64_t rows, uint64_t H, uint64_t row_stride, uint64_t head_stride,
+                uint32_t box_rows = 128) {
   PFN_encodeTiled fn = get_encode_fn();
   if (!fn) return false;
   const cuuint64_t dims[3] = {128, rows, H};
   const cuuint64_t strides[2] = {row_stride * 2, head_stride * 2};
-  const cuuint32_t box[3] = {64, 128, 1};
+  const cuuint32_t box[3] = {64, box_rows, 1};
   const cuuint32_t estr[3] = {1, 1, 1};
   return fn(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(ptr), dims, strides, box, estr,
             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
@@ -812,6 +1214,7 @@ const CUtensorMap* cached_map(uf_ctx* c, const void* ptr, int rows, int H, int64
 int uf_sm100_make_cache_maps(uf_ctx* c) {
   const uint64_t rows = (uint64_t)c->P * 128;
   if (!encode_map(&c->tm_k, c->kc, rows, c->cfg.n_heads, 128, rows * 128) ||
+      !encode_map(&c->tm_k_half, c->kc, rows, c->cfg.n_heads, 128, rows * 128, 64) ||
       !encode_map(&c->tm_v, c->vc, rows, c->cfg.n_heads, 128, rows * 128)) {
     c->err = "cuTensorMapEncodeTiled failed for the K/V cache";
     return UF_ERR_CUDA;
@@ -819,6 +1222,10 @@ int uf_sm100_make_cache_maps(uf_ctx* c) {
   cudaError_t e = cudaFuncSetAttribute(uf_attn_sm100_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
   if (e == cudaSuccess)
     e = cudaFuncSetAttribute(uf_attn_sm100_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+  if (e == cudaSuccess)
+    e = cudaFuncSetAttribute(uf_attn_pair_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes2);
+  if (e == cudaSuccess)
+    e = cudaFuncSetAttribute(uf_attn_pair_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes2);
   if (e != cudaSuccess) {
     c->err = std::string("cudaFuncSetAttribute(smem): ") + cudaGetErrorString(e);
     return UF_ERR_CUDA;
@@ -849,8 +1256,15 @@ int uf_launch_attn_sm100(uf_ctx* c, const UfView& v, const __nv_bfloat16* q, __n
   if (++c->attn_seq <= 0) c->attn_seq = 1;
   a.panic_item = c->panic_item; a.panic_last = c->panic_last; a.seq = c->attn_seq;
   // fast kernel, then the safe kernel for the items it flagged (returns at once when there are none)
-  uf_attn_sm100_kernel<false><<<grid, kThreads, kSmemBytes, s>>>(tm_q, tm_o, c->tm_k, c->tm_v, a);
-  uf_attn_sm100_kernel<true><<<grid, kThreads, kSmemBytes, s>>>(tm_q, tm_o, c->tm_k, c->tm_v, a);
+  if (c->attn_impl == 2) {
+    // CTA pairs: one query tile per CTA, the pair shares every K / V tile (uf_attn_pair_kernel)
+    const int pairs = n_items < c->sm_count / 2 ? n_items : c->sm_count / 2;
+    uf_attn_pair_kernel<false><<<2 * pairs, kThreads, kSmemBytes2, s>>>(tm_q, tm_o, c->tm_k_half, c->tm_v, a);
+    uf_attn_pair_kernel<true><<<2 * pairs, kThreads, kSmemBytes2, s>>>(tm_q, tm_o, c->tm_k_half, c->tm_v, a);
+  } else {
+    uf_attn_sm100_kernel<false><<<grid, kThreads, kSmemBytes, s>>>(tm_q, tm_o, c->tm_k, c->tm_v, a);
+    uf_attn_sm100_kernel<true><<<grid, kThreads, kSmemBytes, s>>>(tm_q, tm_o, c->tm_k, c->tm_v, a);
+  }
   c->launches += 2;
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) {

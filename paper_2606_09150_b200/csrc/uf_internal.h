@@ -147,6 +147,7 @@ struct uf_ctx {
   int64_t launches = 0;
   int sm_count = 0;
   CUtensorMap tm_k, tm_v;         // K / V cache maps for the sm100 kernel (valid when B == d == 128)
+  CUtensorMap tm_k_half;          // K cache map with 64-row boxes (the CTA-pair kernel loads half a K tile per CTA)
   bool tm_ok = false;
   // Q / O tensor maps of recent callers, keyed by (pointer, rows, strides): a model calls with the same few
   // buffers for every layer and chunk, so cuTensorMapEncodeTiled runs once per buffer, not twice per call

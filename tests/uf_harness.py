@@ -3,6 +3,7 @@ and through the fp64 oracle, and compare.  Test infrastructure only (imports `or
 from __future__ import annotations
 
 import math
+import os
 
 import numpy as np
 
@@ -77,6 +78,8 @@ class CudaStream:
             o = torch.full((n, H, d), float("nan"), dtype=torch.bfloat16, device=self.dev)
         lse = torch.full((H, n), float("nan"), dtype=torch.float32, device=self.dev) if want_lse else None
         # shapes other than B = d = 128 have no tcgen05 kernel: the caller has to opt in to the CUDA-core kernel
+        if impl == 0:
+            impl = int(os.environ.get("UF_TEST_ATTN_IMPL", "0"))      # run the suite on another tcgen05 kernel variant
         uf.uf_set_attn_impl(self.ctx, impl if (w.block == 128 and w.head_dim == 128) else 1)
         if fused_qkv:
             # attention takes one token stride for Q and O: O's [n, 2, H, d] slice has stride 2*H*d, so Q is
