@@ -446,7 +446,16 @@ void plan_layer(Layer& L, int frames, int sms) {
   }
   L.n_tile = L.opt_ntile[L.opt];
   L.n_ntiles = L.n_total / L.n_tile;
-  L.MT = L.n_tile > 128 ? 2 : 4;
+  // Groups small enough for two accumulator buffers (MT * N <= 256 TMEM columns) let the epilogue of a group run under
+  // the next group's main loop.  Exception (measured, r2e launch lists): when ALL cells of the busiest pair fit one
+  // single-buffered group (MT * N <= 512), that one group — every weight tile loaded once — beats several small ones.
+  {
+    const int cells = ((m_tiles + 1) / 2) * L.n_ntiles;
+    const int grid = cells < sms / 2 ? cells : sms / 2;
+    const int per_pair = (cells + grid - 1) / grid;
+    const int mt_single = L.n_tile > 128 ? 2 : 4, mt_double = L.n_tile > 128 ? 1 : L.n_tile > 64 ? 2 : 4;
+    L.MT = per_pair <= mt_single ? mt_single : mt_double;
+  }
   L.n_acc = (L.MT * L.n_tile <= 256) ? 2 : 1;
   L.nA = 2;
   const size_t budget = 227 * 1024 - 1024 - kMaxBias * 4 - 256;
@@ -813,7 +822,8 @@ int32_t uf_cmn_step(uf_cmn* n, const void* z, int32_t n_frames, void* out, void*
     const int n_cells = ((p.F * p.tiles_x * p.tiles_y + 1) / 2) * p.n_ntiles;      // (N tile, double pixel tile)
     const int pairs = n_cells < n->sm_count / 2 ? n_cells : n->sm_count / 2;
     const int grid = 2 * pairs;
-    cudaError_t e = L.MT == 2 ? launch_conv<2>(L, p, grid, s) : launch_conv<4>(L, p, grid, s);
+    cudaError_t e = L.MT == 1 ? launch_conv<1>(L, p, grid, s)
+                  : L.MT == 2 ? launch_conv<2>(L, p, grid, s) : launch_conv<4>(L, p, grid, s);
     if (e != cudaSuccess) return cfail(n, UF_ERR_CUDA, "uf_cmn_conv_kernel (" + L.name + "): " + cudaGetErrorString(e));
     ++n->launches;
   }
