@@ -421,8 +421,8 @@ def call_breakdown(hp: HotPath, steps: int, hbm_gbs: float):
                    "frac_of_hbm_peak": app_bytes / app / 1e6 / hbm_gbs},
         "select": {"ms": sel, "algorithmic_bytes": sel_bytes, "achieved_gbs": sel_bytes / sel / 1e6,
                    "frac_of_hbm_peak": sel_bytes / sel / 1e6 / hbm_gbs,
-                   "note": ("2 kernels: fp64 score + exact top-k, pair merge (Q pooled by the fused append)" if hp.fused else
-                            "3 kernels: pool Q (HBM-bound), fp64 score + exact threshold-search top-k (latency/ALU-bound), pair merge")},
+                   "note": ("1 kernel: fp64 score + exact top-k + pair merge (Q pooled by the fused append)" if hp.fused else
+                            "2 kernels: pool Q (HBM-bound); fp64 score + exact threshold-search top-k + pair merge (latency/ALU-bound)")},
         "attention": {"ms": att},
         "hbm_peak_gbs": hbm_gbs,
     }

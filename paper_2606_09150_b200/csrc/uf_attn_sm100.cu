@@ -1236,13 +1236,19 @@ int uf_sm100_make_cache_maps(uf_ctx* c) {
 
 int uf_launch_attn_sm100(uf_ctx* c, const UfView& v, const __nv_bfloat16* q, __nv_bfloat16* o, float* lse,
                          int64_t tok_stride, int64_t head_stride, float scale, cudaStream_t s) {
+  // each map is copied before the next lookup: a miss may recycle the very cache entry the previous hit returned
   const CUtensorMap* pq = cached_map(c, q, v.cur_ntok, v.H, tok_stride, head_stride);
-  const CUtensorMap* po = cached_map(c, o, v.cur_ntok, v.H, tok_stride, head_stride);
-  if (!pq || !po) {
-    c->err = "cuTensorMapEncodeTiled failed for Q/O (check strides and alignment)";
+  if (!pq) {
+    c->err = "cuTensorMapEncodeTiled failed for Q (check strides and alignment)";
     return UF_ERR_INVALID_ARG;
   }
-  const CUtensorMap tm_q = *pq, tm_o = *po;
+  const CUtensorMap tm_q = *pq;
+  const CUtensorMap* po = cached_map(c, o, v.cur_ntok, v.H, tok_stride, head_stride);
+  if (!po) {
+    c->err = "cuTensorMapEncodeTiled failed for O (check strides and alignment)";
+    return UF_ERR_INVALID_ARG;
+  }
+  const CUtensorMap tm_o = *po;
   AttnParams a;
   a.sel_pair = c->sel_pair; a.pair_cnt = c->pair_cnt; a.lse = lse;
   a.H = v.H; a.NP = (v.BPC + 1) / 2; a.kcap = c->kcap;

@@ -62,6 +62,11 @@ __device__ __forceinline__ unsigned long long sortable(double x) {
   return (u & 0x8000000000000000ull) ? ~u : (u | 0x8000000000000000ull);
 }
 
+__device__ __forceinline__ void uf_merge_pair(const UfView& v, uint32_t* bma, uint32_t* bmb, int nw, int h, int p, int nqb,
+                                              int k_eff, int kcap, const int32_t* __restrict__ sel_rank,
+                                              const int32_t* __restrict__ sel_cnt, int32_t* __restrict__ sel_pair,
+                                              int32_t* __restrict__ pair_cnt, int lane);
+
 // ---- a3 + a4: scores and top-k.  grid (ceil(nqb / kQG), H) ------------------------------------------
 // kQG query blocks are scored per CTA (each pooled-K load is re-used kQG times).
 // dynamic smem: double qs[kQG][D]; unsigned long long key[kQG][n_cand]
@@ -74,8 +79,11 @@ __global__ void __launch_bounds__(kScoreThreads)
 uf_score_topk_kernel(UfView v, const double* __restrict__ qbar, const double* __restrict__ kpool,
                      int nqb, int k_eff, int32_t* __restrict__ sel_q, int32_t* __restrict__ sel_rank, int kcap,
                      int32_t* __restrict__ sel_cnt, int32_t* __restrict__ idx_out, int32_t* __restrict__ cnt_out,
-                     int out_stride, unsigned long long* __restrict__ usage) {
+                     int out_stride, unsigned long long* __restrict__ usage,
+                     int32_t* __restrict__ sel_pair, int32_t* __restrict__ pair_cnt,
+                     unsigned long long* __restrict__ usage_next) {
   __shared__ unsigned int usage_s[UF_MAXC];            // kept blocks per listed chunk, this CTA (NEXT-3 statistic)
+  if (blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x < UF_MAXC) usage_next[threadIdx.x] = 0ull;   // the next selection's
   if (threadIdx.x < UF_MAXC) usage_s[threadIdx.x] = 0u;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   double* qs = reinterpret_cast<double*>(smem_raw);                                  // [kQG][D]
@@ -202,6 +210,16 @@ uf_score_topk_kernel(UfView v, const double* __restrict__ qbar, const double* __
   }
   __syncthreads();
   if (tid < v.n_prior && usage_s[tid]) atomicAdd(&usage[tid], (unsigned long long)usage_s[tid]);
+  // Merge the lists of the query-block pairs this CTA just selected (kQG even, i0 a multiple of kQG: both blocks of
+  // a pair are here; their sel_rank rows were written by this CTA before the barrier above) into the union lists
+  // the tcgen05 attention kernels walk: no separate launch.  The key array is dead: its memory holds the bitmaps.
+  if (sel_pair != nullptr && kQG >= 2) {
+    const int nw = (nc + 31) / 32;
+    uint32_t* bm = reinterpret_cast<uint32_t*>(key);
+    for (int pp = wid; 2 * pp < ng; pp += kScoreThreads / 32)
+      uf_merge_pair(v, bm + (size_t)pp * 2 * nw, bm + (size_t)pp * 2 * nw + nw, nw, h, i0 / 2 + pp, nqb, k_eff, kcap,
+                    sel_rank, kPaper ? sel_cnt : nullptr, sel_pair, pair_cnt, lane);
+  }
 }
 
 // ---- merge the lists of query blocks (2p, 2p+1) into one union list with tile masks -----------------
@@ -212,23 +230,13 @@ uf_score_topk_kernel(UfView v, const double* __restrict__ qbar, const double* __
 // tensor pipe has the other tile's MMAs (two single-tile steps of the same tile in a row would serialise).
 // An entry's position is its rank within its class (word popcounts + a warp scan); its payload (physical
 // block, valid rows) is recomputed from the candidate index.  dynamic smem: uint32 [warps][2][ceil(n_cand / 32)]
-constexpr int kMergeWarps = 4;
-__global__ void __launch_bounds__(kMergeWarps * 32)
-uf_pair_merge_kernel(UfView v, const int32_t* __restrict__ sel_rank, const int32_t* __restrict__ sel_cnt,
-                     int32_t* __restrict__ sel_pair, int32_t* __restrict__ pair_cnt, int nqb, int k_eff, int kcap,
-                     unsigned long long* __restrict__ usage_next) {
-  extern __shared__ uint32_t bm_raw[];
-  if (blockIdx.x == 0 && threadIdx.x < UF_MAXC) usage_next[threadIdx.x] = 0ull;   // the next selection's counters
+// One warp merges the lists of query blocks (2p, 2p + 1) of head h; bma / bmb: nw words of shared memory each.
+__device__ __forceinline__ void uf_merge_pair(const UfView& v, uint32_t* bma, uint32_t* bmb, int nw, int h, int p, int nqb,
+                                              int k_eff, int kcap, const int32_t* __restrict__ sel_rank,
+                                              const int32_t* __restrict__ sel_cnt, int32_t* __restrict__ sel_pair,
+                                              int32_t* __restrict__ pair_cnt, int lane) {
   const int NP = (v.BPC + 1) / 2;
-  const int np_cur = (nqb + 1) / 2;
-  const int nw = (v.n_cand + 31) / 32;
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int x = blockIdx.x * kMergeWarps + warp;
-  if (x >= v.H * np_cur) return;
-  const int h = x / np_cur, p = x % np_cur;
-  uint32_t* bma = bm_raw + (size_t)warp * 2 * nw;
-  uint32_t* bmb = bma + nw;
-  for (int w = lane; w < 2 * nw; w += 32) bma[w] = 0u;
+  for (int w = lane; w < nw; w += 32) { bma[w] = 0u; bmb[w] = 0u; }
   __syncwarp();
   const int32_t* ra = sel_rank + ((int64_t)h * v.BPC + 2 * p) * kcap;
   const int32_t* rb = ra + kcap;
@@ -290,6 +298,21 @@ uf_pair_merge_kernel(UfView v, const int32_t* __restrict__ sel_rank, const int32
   if (lane == 0) pair_cnt[(int64_t)h * NP + p] = n3 + n1 + n2;
 }
 
+// the stand-alone form (only when the score kernel runs one query block per CTA and cannot merge pairs itself)
+constexpr int kMergeWarps = 4;
+__global__ void __launch_bounds__(kMergeWarps * 32)
+uf_pair_merge_kernel(UfView v, const int32_t* __restrict__ sel_rank, const int32_t* __restrict__ sel_cnt,
+                     int32_t* __restrict__ sel_pair, int32_t* __restrict__ pair_cnt, int nqb, int k_eff, int kcap) {
+  extern __shared__ uint32_t bm_raw[];
+  const int np_cur = (nqb + 1) / 2;
+  const int nw = (v.n_cand + 31) / 32;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int x = blockIdx.x * kMergeWarps + warp;
+  if (x >= v.H * np_cur) return;
+  uint32_t* bma = bm_raw + (size_t)warp * 2 * nw;
+  uf_merge_pair(v, bma, bma + nw, nw, x / np_cur, x % np_cur, nqb, k_eff, kcap, sel_rank, sel_cnt, sel_pair, pair_cnt, lane);
+}
+
 }  // namespace
 
 cudaError_t uf_launch_select(uf_ctx* c, const UfView& v, const __nv_bfloat16* q, int64_t tok_stride,
@@ -326,6 +349,8 @@ cudaError_t uf_launch_select(uf_ctx* c, const UfView& v, const __nv_bfloat16* q,
   const size_t smem = smem_for(qg);
   if (smem > 200 * 1024) return cudaErrorInvalidConfiguration;     // > ~25k candidates: not supported
   dim3 gs(uf_ceil_div(nqb, qg), v.H);
+  const bool want_pairs = (v.B == 128 && v.d == 128);      // the tcgen05 attention kernels walk per-pair union lists
+  const bool fuse_merge = want_pairs && qg >= 2;           // built by the score kernel itself
   const bool deep_prefetch = (int64_t)gs.x * gs.y <= 2 * (int64_t)c->sm_count;
 #define UF_SCORE_LAUNCH3(DD, QG, PP, PF)                                                                     \
   {                                                                                                          \
@@ -339,7 +364,7 @@ cudaError_t uf_launch_select(uf_ctx* c, const UfView& v, const __nv_bfloat16* q,
     }                                                                                                        \
     uf_score_topk_kernel<DD, QG, PP, PF><<<gs, kScoreThreads, smem, s>>>(                                    \
         v, c->qbar, c->kpool, nqb, k_eff, c->sel_q, c->sel_rank, c->kcap, c->sel_cnt, idx_out, cnt_out,      \
-        out_stride, usage_cur);                                                                              \
+        out_stride, usage_cur, fuse_merge ? c->sel_pair : nullptr, c->pair_cnt, usage_next);                 \
   }
   /* few CTAs per SM: latency-bound, prefetch deep (16 loads ahead, 122 registers); many: keep the occupancy */
 #define UF_SCORE_LAUNCH2(DD, QG, PP)                                                                         \
@@ -375,15 +400,13 @@ cudaError_t uf_launch_select(uf_ctx* c, const UfView& v, const __nv_bfloat16* q,
   c->launches += 1;
   e = cudaGetLastError();
   if (e != cudaSuccess) return e;
-  if (v.B == 128 && v.d == 128) {
+  if (want_pairs && !fuse_merge) {
     const int np_cur = (nqb + 1) / 2;
     const size_t msmem = (size_t)kMergeWarps * 2 * uf_ceil_div(v.n_cand, 32) * sizeof(uint32_t);
     uf_pair_merge_kernel<<<uf_ceil_div(v.H * np_cur, kMergeWarps), kMergeWarps * 32, msmem, s>>>(
-        v, c->sel_rank, paper ? c->sel_cnt : nullptr, c->sel_pair, c->pair_cnt, nqb, k_eff, c->kcap, usage_next);
+        v, c->sel_rank, paper ? c->sel_cnt : nullptr, c->sel_pair, c->pair_cnt, nqb, k_eff, c->kcap);
     c->launches += 1;
     e = cudaGetLastError();
-  } else {
-    e = cudaMemsetAsync(usage_next, 0, UF_MAXC * sizeof(unsigned long long), s);
   }
   return e;
 }

@@ -478,3 +478,39 @@ def test_sm100_kernel_matches_generic_kernel_medium():
         assert diff.max() <= 2e-2 and diff.mean() <= 2e-3, (diff.max(), diff.mean())
     finally:
         cu.close()
+
+
+def test_tensor_map_cache_eviction_between_q_and_o_lookups():
+    """The ctx caches the Q / O tensor maps of recent callers (8 entries, recycled round-robin).  A call whose Q hits the
+    entry that its O, missing, is about to recycle must still read Q: with 4 buffer pairs the cache is full and the
+    next slot is the first Q's, so (q0, new O) is exactly that case (it once loaded Q through O's map)."""
+    import torch
+    w = wl.scaled(wl.CONFIGS["1k"], "tmcache", n_heads=2, frames_per_chunk=1, grid_h=16, grid_w=20, capacity_chunks=2)
+    cu = hz.CudaStream(w)
+    try:
+        for c in range(2):
+            Qb, Kb, Vb = wl.make_chunk(w, c)
+            got = cu.step(Qb, Kb, Vb, topk_percent=50)                  # leaves a valid selection in the ctx
+        n, H, d = Qb.shape
+        uf, ref = cu.uf, torch.from_numpy(got["O"]).to(cu.dev)
+        uf.uf_ctx_reset(cu.ctx, cu.stream)                              # a fresh cache of maps needs a fresh ctx: new one
+    finally:
+        cu.close()
+    cu = hz.CudaStream(w)
+    try:
+        for c in range(2):
+            Qb, Kb, Vb = wl.make_chunk(w, c)
+            k, v = cu.to_dev(Kb), cu.to_dev(Vb)
+            uf.uf_kv_append(cu.ctx, k, v, n, H * d, d, 0, cu.stream)
+        qs = [cu.to_dev(Qb) for _ in range(4)]
+        os_ = [torch.full((n, H, d), float("nan"), dtype=torch.bfloat16, device=cu.dev) for _ in range(5)]
+        uf.uf_select_blocks(cu.ctx, qs[0], n, H * d, d, -1, 50, None, None, cu.stream)
+        for i in range(4):                                              # fills the 8 entries: q0 o0 q1 o1 q2 o2 q3 o3
+            uf.uf_sparse_attn_fwd(cu.ctx, qs[i], os_[i], None, n, H * d, d, 0.0, cu.stream)
+        uf.uf_sparse_attn_fwd(cu.ctx, qs[0], os_[4], None, n, H * d, d, 0.0, cu.stream)   # q0 hits slot 0, o4 recycles it
+        torch.cuda.synchronize()
+        for i in range(5):
+            assert not torch.isnan(os_[i].float()).any(), f"call {i}: NaN / unwritten rows"
+            assert torch.equal(os_[i].float(), ref), f"call {i} differs from the first result"
+    finally:
+        cu.close()
