@@ -32,7 +32,7 @@ import uf_workloads as wl  # noqa: E402
 
 PROFILE_TRAFFIC = os.path.join(ROOT, "profiles", "attn_dram_traffic.txt")
 KERNEL_SOURCES = ["include/uf.h"] + ["paper_2606_09150_b200/csrc/" + f for f in (
-    "uf_internal.h", "uf_api.cu", "uf_append.cu", "uf_fused_append.cu", "uf_select.cu", "uf_attn_generic.cu", "uf_attn_sm100.cu")]
+    "uf_internal.h", "uf_sm100_ptx.h", "uf_api.cu", "uf_append.cu", "uf_fused_append.cu", "uf_select.cu", "uf_attn_generic.cu", "uf_attn_sm100.cu")]
 
 
 def kernel_source_hash() -> str:

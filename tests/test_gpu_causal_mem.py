@@ -104,6 +104,14 @@ def test_upsampler_full_1k_chunk():
     print("cmn_upsampler_1k parity:", st)
 
 
+def test_decoder_crop_full_size():
+    # P:347 on one 68 x 120 latent frame -> 4 frames of 544 x 960 x 3: the second launch configuration bench.py times
+    # (64-channel layers on 272 x 480 x 2 frames, N = 64 tiles, 3-channel scalar stores)
+    c = wl.CMN_CONFIGS["cmn_decoder_crop"]
+    st = _run_stream(c, [1])
+    print("cmn_decoder_crop parity:", st)
+
+
 def test_argument_errors():
     import paper_2606_09150_b200 as uf
     with pytest.raises(uf.UFError) as e:
