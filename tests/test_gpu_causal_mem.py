@@ -104,6 +104,27 @@ def test_upsampler_full_1k_chunk():
     print("cmn_upsampler_1k parity:", st)
 
 
+@pytest.mark.parametrize("seed", range(6))
+def test_randomised_networks(seed):
+    """Seeded random small networks: widths 64 / 128 / 192 / 256 (N = 192 tiles, three 64-channel slices), 1-3 stages,
+    spatial factors 1-3, temporal factors 1-3, 1-2 blocks per stage, in_ch 8 / 16 / 24, out_ch 1-40 (GEMM columns padded
+    to 16, scalar and vector stores), grids from smaller than one tile to several ragged tiles, ragged chunk lengths."""
+    rng = np.random.default_rng(500 + seed)
+    n_stages = int(rng.integers(1, 4))
+    widths, rs, ts = [], [], []
+    for _ in range(n_stages):
+        r = int(rng.choice([1, 1, 2, 3]))
+        c = int(rng.choice([64, 128, 192, 256] if r == 1 else [64, 128, 256] if r == 2 else [64]))   # C r^2 <= 1024
+        widths.append(c); rs.append(r); ts.append(int(rng.choice([1, 1, 2, 3])))
+    if rng.random() < 0.5:
+        widths.append(int(rng.choice([64, 128])))
+    c = wl.CmnWorkload(f"cmn_rand{seed}", int(rng.choice([8, 16, 24])), int(rng.integers(1, 41)), tuple(widths),
+                       int(rng.integers(1, 3)), tuple(rs), tuple(ts), int(rng.integers(3, 20)), int(rng.integers(3, 40)), 2)
+    chunks = [int(x) for x in rng.integers(1, 4, size=int(rng.integers(1, 4)))]
+    print(c, chunks)
+    _run_stream(c, chunks, frames_max=3)
+
+
 def test_decoder_crop_full_size():
     # P:347 on one 68 x 120 latent frame -> 4 frames of 544 x 960 x 3: the second launch configuration bench.py times
     # (64-channel layers on 272 x 480 x 2 frames, N = 64 tiles, 3-channel scalar stores)
