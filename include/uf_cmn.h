@@ -69,7 +69,8 @@ int32_t uf_cmn_param_info(const uf_cmn* n, int32_t index, char* name, int32_t na
                           int32_t* has_bias);
 int32_t uf_cmn_set_param(uf_cmn* n, const char* name, const void* w_host, const float* bias_host);
 
-/* Start a new video stream: every block memory becomes zero (Alg. 2 line 23).  Asynchronous on `stream`.          */
+/* Start a new video stream: every block memory becomes zero (Alg. 2 line 23).  Host bookkeeping only (the next step
+ * reads an all-zero frame kept in every memory buffer); `stream` is unused.                                          */
 int32_t uf_cmn_reset(uf_cmn* n, void* stream);
 
 /* One streaming step (Alg. 2 lines 24-41 for n_frames consecutive frames).

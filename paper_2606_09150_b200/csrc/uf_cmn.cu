@@ -50,7 +50,9 @@ struct ConvParams {
   int n_src;
   int ntx[kMaxSrc], nty[kMaxSrc];   // taps of each source along x / y (3 or 1)
   int cchunks[kMaxSrc];             // 64-channel slices of each source
-  int fshift[kMaxSrc];              // frame coordinate of output frame f in the source buffer = f + fshift
+  int fbase[kMaxSrc];               // frame slot of output frame f in the source buffer = fbase + f ...
+  int mem[kMaxSrc];                 // ... or, for a memory source, fbase + f - 1, and f0_slot for f == 0
+  int f0_slot[kMaxSrc];
   int F, H, W;                      // frames of this launch, conv grid (= source grid)
   int tiles_x, tiles_y;             // 128-pixel tiles per frame: 8 rows x 16 columns each
   int n_ntiles, N;                  // N tiles, GEMM columns per tile (multiple of 16, <= 256)
@@ -161,7 +163,7 @@ uf_cmn_conv_kernel(const __grid_constant__ CUtensorMap tm_a0, const __grid_const
                 UF_MTILE_DECODE(2 * (m0 + mt) + (int)rank)                                // past the end: frame out of range
                 tma_load_4d_2sm(base + as * a_stage_bytes + mt * kATileBytes, ta, bA_FULL + 8 * as, cc * 64,
                                 x0 + dxi - (ntx == 3 ? 1 : 0), y0 - (nty == 3 ? 1 : 0),
-                                f < p.F ? f + p.fshift[s] : 0x100000);
+                                f >= p.F ? 0x100000 : !p.mem[s] ? p.fbase[s] + f : f ? p.fbase[s] + f - 1 : p.f0_slot[s]);
               }
             }
             if (++as == (uint32_t)p.nA) { as = 0; aph ^= 1; }
@@ -341,8 +343,15 @@ struct Buf {
   __nv_bfloat16* p = nullptr;
   int H = 0, W = 0, C = 0;
   int fmul = 1;              // frames per input frame at this point of the network
-  int has_mem = 0;           // slot 0 holds the last frame of the previous step (a block input, R-41)
-  int slots = 0;             // frame slots allocated = frames_max * fmul + has_mem
+  // A block input keeps its own past (R-41): slot 0 is all zeros (the memory at the start of a stream), then two
+  // regions of frames_max * fmul slots that successive steps fill in turn; the memory of a step is the slot the
+  // previous step wrote its last frame to.  No copies: "memory" is the same tensor map at another frame coordinate.
+  int has_mem = 0;
+  int slots = 0;             // frame slots allocated: frames_max * fmul, or 1 + 2 * that
+  int region = 0;            // region the NEXT step writes (has_mem only)
+  int mem_slot = 0;          // slot of the current memory frame (0 = zeros)
+  int last_base = 0;         // first slot the last step wrote
+  int base(int frames_max) const { return has_mem ? 1 + region * frames_max * fmul : 0; }
   size_t frame_elems() const { return (size_t)H * W * C; }
 };
 
@@ -420,7 +429,7 @@ int stage_out_width(const uf_cmn_config& c, int s) {
 int add_buf(uf_cmn* n, int H, int W, int C, int fmul, int has_mem) {
   Buf b;
   b.H = H; b.W = W; b.C = C; b.fmul = fmul; b.has_mem = has_mem;
-  b.slots = n->cfg.frames_max * fmul + has_mem;
+  b.slots = has_mem ? 1 + 2 * n->cfg.frames_max * fmul : n->cfg.frames_max * fmul;
   n->bufs.push_back(b);
   return (int)n->bufs.size() - 1;
 }
@@ -774,12 +783,9 @@ int32_t uf_cmn_set_param(uf_cmn* n, const char* name, const void* w_host, const 
 
 int32_t uf_cmn_reset(uf_cmn* n, void* stream) {
   if (!n) return UF_ERR_INVALID_ARG;
-  cudaStream_t s = static_cast<cudaStream_t>(stream);
-  for (Buf& b : n->bufs)
-    if (b.has_mem) {
-      cudaError_t e = cudaMemsetAsync(b.p, 0, b.frame_elems() * sizeof(__nv_bfloat16), s);
-      if (e != cudaSuccess) return cfail(n, UF_ERR_CUDA, std::string("cudaMemsetAsync: ") + cudaGetErrorString(e));
-    }
+  (void)stream;
+  // host state only: slot 0 of every block input is zero for good, and the next step takes it as its memory
+  for (Buf& b : n->bufs) { b.mem_slot = 0; b.region = 0; }
   return UF_OK;
 }
 
@@ -804,8 +810,10 @@ int32_t uf_cmn_step(uf_cmn* n, const void* z, int32_t n_frames, void* out, void*
     for (int i = 0; i < L.n_src; ++i) {
       p.ntx[i] = p.nty[i] = L.ntap[i] == 9 ? 3 : 1;
       p.cchunks[i] = (L.cin[i] + 63) / 64;
-      const int has_mem = L.src_buf[i] >= 0 ? n->bufs[L.src_buf[i]].has_mem : 0;
-      p.fshift[i] = has_mem - L.mem[i];
+      const Buf* sb = L.src_buf[i] >= 0 ? &n->bufs[L.src_buf[i]] : nullptr;
+      p.fbase[i] = sb ? sb->base(c.frames_max) : 0;
+      p.mem[i] = L.mem[i];
+      p.f0_slot[i] = sb ? sb->mem_slot : 0;
     }
     p.F = n_frames * L.fmul; p.H = L.H; p.W = L.W;
     p.tiles_x = (L.W + 15) / 16;
@@ -815,7 +823,7 @@ int32_t uf_cmn_step(uf_cmn* n, const void* z, int32_t n_frames, void* out, void*
     p.mode = L.mode; p.r = L.r; p.fs = L.fs; p.c_grp = L.c_grp; p.c_real = L.c_real;
     if (L.out_buf >= 0) {
       const Buf& b = n->bufs[L.out_buf];
-      p.out = b.p; p.out_fbase = b.has_mem; p.Hout = b.H; p.Wout = b.W; p.Cbuf = b.C;
+      p.out = b.p; p.out_fbase = b.base(c.frames_max); p.Hout = b.H; p.Wout = b.W; p.Cbuf = b.C;
     } else {
       p.out = static_cast<__nv_bfloat16*>(out); p.out_fbase = 0; p.Hout = n->out_H; p.Wout = n->out_W; p.Cbuf = c.out_ch;
     }
@@ -828,14 +836,14 @@ int32_t uf_cmn_step(uf_cmn* n, const void* z, int32_t n_frames, void* out, void*
     ++n->launches;
   }
   n->last_frames = n_frames;
-  // the last frame of every block input becomes the memory of the next step (R-41)
-  for (Buf& b : n->bufs)
+  // the last frame of every block input is the memory of the next step (R-41): remember where it is, switch regions
+  for (Buf& b : n->bufs) {
+    b.last_base = b.base(c.frames_max);
     if (b.has_mem) {
-      const size_t fe = b.frame_elems();
-      cudaError_t e = cudaMemcpyAsync(b.p, b.p + fe * (size_t)(n_frames * b.fmul), fe * sizeof(__nv_bfloat16),
-                                      cudaMemcpyDeviceToDevice, s);
-      if (e != cudaSuccess) return cfail(n, UF_ERR_CUDA, std::string("cudaMemcpyAsync(memory): ") + cudaGetErrorString(e));
+      b.mem_slot = b.last_base + n_frames * b.fmul - 1;
+      b.region ^= 1;
     }
+  }
   return UF_OK;
 }
 
@@ -845,7 +853,8 @@ int32_t uf_cmn_get_memory(uf_cmn* n, int32_t stage, int32_t block, void* out_hos
     return cfail(n, UF_ERR_INVALID_ARG, "uf_cmn_get_memory: no such block");
   const Buf& b = n->bufs[n->mem_buf[(size_t)stage * n->cfg.n_blocks + block]];
   cudaStream_t s = static_cast<cudaStream_t>(stream);
-  cudaError_t e = cudaMemcpyAsync(out_host, b.p, b.frame_elems() * sizeof(__nv_bfloat16), cudaMemcpyDeviceToHost, s);
+  cudaError_t e = cudaMemcpyAsync(out_host, b.p + b.frame_elems() * (size_t)b.mem_slot, b.frame_elems() * sizeof(__nv_bfloat16),
+                                  cudaMemcpyDeviceToHost, s);
   if (e == cudaSuccess) e = cudaStreamSynchronize(s);
   if (e != cudaSuccess) return cfail(n, UF_ERR_CUDA, std::string("uf_cmn_get_memory: ") + cudaGetErrorString(e));
   if (shape_out) { shape_out[0] = b.H; shape_out[1] = b.W; shape_out[2] = b.C; }
@@ -860,7 +869,7 @@ int32_t uf_cmn_get_activation(uf_cmn* n, int32_t layer, void* out_host, int32_t 
   const Buf& b = n->bufs[n->layers[layer].out_buf];
   const int F = n->last_frames * b.fmul;
   cudaStream_t s = static_cast<cudaStream_t>(stream);
-  cudaError_t e = cudaMemcpyAsync(out_host, b.p + b.frame_elems() * (size_t)b.has_mem,
+  cudaError_t e = cudaMemcpyAsync(out_host, b.p + b.frame_elems() * (size_t)b.last_base,
                                   b.frame_elems() * (size_t)F * sizeof(__nv_bfloat16), cudaMemcpyDeviceToHost, s);
   if (e == cudaSuccess) e = cudaStreamSynchronize(s);
   if (e != cudaSuccess) return cfail(n, UF_ERR_CUDA, std::string("uf_cmn_get_activation: ") + cudaGetErrorString(e));
