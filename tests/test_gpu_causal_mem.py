@@ -12,7 +12,7 @@ import uf_harness as hz
 pytestmark = pytest.mark.gpu
 
 
-def _run_stream(c, chunks, frames_max=None, layerwise=True):
+def _run_stream(c, chunks, frames_max=None, layerwise=True, check_memory=True):
     """stream of sum(chunks) frames cut into the given chunk lengths.  Per chunk: (1) every layer of the step against
     the oracle's layer function on the same inputs (one-ulp bound, uf_harness.cmn_layer_check); (2) the network
     output against the oracle's variant A over the whole stream (rounding-noise bound, uf_harness.compare_cmn);
@@ -34,12 +34,13 @@ def _run_stream(c, chunks, frames_max=None, layerwise=True):
                                                               f"[{c.name} chunk {i}]")
             stats.append(st)
             f0 += n
-        # memory of every block == the block's input at the last frame (R-41), from the streaming oracle
-        so = cm.CausalMemStream(cfg, wt)
-        so.step(z)
-        for s in range(cfg.n_stages):
-            for b in range(cfg.n_blocks):
-                hz.compare_cmn(cu.memory(s, b)[None], so.mem[f"s{s}.b{b}."], nl, f"[{c.name} memory s{s}.b{b}]")
+        if check_memory:
+            # memory of every block == the block's input at the last frame (R-41), from the streaming oracle (variant B)
+            so = cm.CausalMemStream(cfg, wt)
+            so.step(z)
+            for s in range(cfg.n_stages):
+                for b in range(cfg.n_blocks):
+                    hz.compare_cmn(cu.memory(s, b)[None], so.mem[f"s{s}.b{b}."], nl, f"[{c.name} memory s{s}.b{b}]")
         assert cu.uf.uf_cmn_launches(cu.net) == len(chunks) * nl
         assert cu.uf.uf_cmn_flops(cu.net, 1) == cm.flop_count(cfg, c.height, c.width, 1)
         return stats
@@ -98,9 +99,10 @@ def test_decoder_configuration_small():
 
 def test_upsampler_full_1k_chunk():
     # BASELINE.json's 1K grid: LR latent 68 x 120, chunk of 3 latent frames -> 136 x 240 (the launch configuration
-    # bench.py times); two chunks so that the second one runs on real memories
+    # bench.py times); a second chunk runs on real memories (its first Conv1 of every block is checked layer-wise
+    # against the oracle fed with the GPU's own previous frame, so the streaming oracle is not run a third time here)
     c = wl.CMN_CONFIGS["cmn_upsampler_1k"]
-    st = _run_stream(c, [3, 3])
+    st = _run_stream(c, [3, 1], check_memory=False)
     print("cmn_upsampler_1k parity:", st)
 
 
@@ -129,7 +131,7 @@ def test_decoder_crop_full_size():
     # P:347 on one 68 x 120 latent frame -> 4 frames of 544 x 960 x 3: the second launch configuration bench.py times
     # (64-channel layers on 272 x 480 x 2 frames, N = 64 tiles, 3-channel scalar stores)
     c = wl.CMN_CONFIGS["cmn_decoder_crop"]
-    st = _run_stream(c, [1])
+    st = _run_stream(c, [1], check_memory=False)
     print("cmn_decoder_crop parity:", st)
 
 
