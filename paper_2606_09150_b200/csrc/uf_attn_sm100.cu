@@ -797,13 +797,23 @@ enum Bar2 {
   B2_S_FULL0 = B2_V_EMPTY0 + kNV2, B2_P_FULL0 = B2_S_FULL0 + 3, B2_PV_DONE0 = B2_P_FULL0 + 3, B2_O_FULL = B2_PV_DONE0 + 2, kNumBars2
 };
 constexpr int kOff2TmemPtr = kOff2Bar + kNumBars2 * 8;
-constexpr int kOff2Xc = kOff2TmemPtr + 16;                    // row-pair exchange: [half][row][parity] bytes
-constexpr int kSmemBytes2 = kOff2Xc + 2 * 128 * 2 + 1024;
+constexpr int kOff2Xc = kOff2TmemPtr + 16;                    // row-pair exchange: [group][half][row][parity] bytes
+constexpr int kOff2M0 = kOff2Xc + 2 * 2 * 128 * 2;            // two softmax groups: reference max of the item's rows (float)
+constexpr int kOff2Rc = kOff2M0 + 128 * 4;                    // ... binades it was raised by so far (int)
+constexpr int kOff2Cnt = kOff2Rc + 128 * 4;                   // ... steps whose start decision is published
+constexpr int kSmemBytes2 = kOff2Cnt + 16 + 1024;
 constexpr uint32_t kIdescQK2 = (1u << 4) | (1u << 7) | (1u << 10) | ((128u >> 3) << 17) | ((256u >> 4) << 24);
 constexpr uint32_t kIdescPV2 = kIdescQK2 | (1u << 16);
 
-template <bool kSafe>
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
+// kGroups = 2 (fast kernel only): TWO groups of 8 softmax warps take the key blocks of the tile in turn (group g the
+// blocks with global step number gs = g mod 2), so that the TMEM round trips, barrier waits and dependency stalls of
+// one group's step run under the arithmetic of the other's (the arithmetic alone needs ~1000-1080 cycles per block
+// and 8 warps cannot overlap the ~320 cycles around it).  Both groups use ONE reference max per row, m = m0 + r
+// (m0 set by the group that gets the first attended block, r = binades raised so far, both in shared memory): a step
+// publishes its decision (a raise of r) before it computes, and the next step, the other group's, starts only after
+// that, so every P is relative to the m that O will have when its O += P V is issued.
+template <bool kSafe, int kGroups>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__((8 * kGroups + 4) * 32, 1)
 uf_attn_pair_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_o,
                     const __grid_constant__ CUtensorMap tm_k, const __grid_constant__ CUtensorMap tm_v,
                     const AttnParams a) {
@@ -818,20 +828,23 @@ uf_attn_pair_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
   const int rank = (int)ufptx::cluster_ctarank();      // 0 = leader: issues every MMA of the pair
   const int pair = (int)(blockIdx.x >> 1), n_pairs = (int)(gridDim.x >> 1);
   const int n_items = a.H * a.np_cur;
+  static_assert(kGroups == 1 || !kSafe, "the exact-max kernel runs one softmax group");
+  constexpr int kW0 = 8 * kGroups;                     // first non-softmax warp: producer, MMA issuer, TMEM allocator
+  if (threadIdx.x == 0) *reinterpret_cast<volatile uint32_t*>(base_ptr + kOff2Cnt) = 0u;
 
-  if (warp == 8 && lane == 0) {
+  if (warp == kW0 && lane == 0) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_q));
     asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_o));
     asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_k));
     asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_v));
   }
-  if (warp == 9 && lane == 0) {
+  if (warp == kW0 + 1 && lane == 0) {
     for (int i = 0; i < kNumBars2; ++i)
       mbar_init(bars + i * 8, (i >= B2_P_FULL0 && i < B2_P_FULL0 + 3) ? 2 * kPArrivals : 1u);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     fence_proxy_async();
   }
-  if (warp == 10) {
+  if (warp == kW0 + 2) {
     asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32((const void*)tmem_ptr_smem)) : "memory");
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
   }
@@ -851,9 +864,10 @@ uf_attn_pair_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
     const int full_mask = (2 * p + 1 < a.nqb) ? 3 : 1;
 #define UF_ITEM_LOOP_END }
 
-  if (warp >= 8) {
-    asm volatile("setmaxnreg.dec.sync.aligned.u32 80;");
-    if (warp == 8) {
+  if (warp >= kW0) {
+    if (kGroups == 1) asm volatile("setmaxnreg.dec.sync.aligned.u32 80;");
+    else asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
+    if (warp == kW0) {
       // ================================ TMA producer (both CTAs) =====================
       uint32_t ks = 0, kph = 0, vs = 0, vph = 0, qph = 0;
       auto load_kv = [&](int phys, int h) {
@@ -901,7 +915,7 @@ uf_attn_pair_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
         for (int j = 0; j < a.n_sink; ++j) load_kv(j, h);
         for (int j = 0; j < a.n_cur; ++j) load_kv(a.cur_phys0 + j, h);
       UF_ITEM_LOOP_END
-    } else if (warp == 9 && rank == 0) {
+    } else if (warp == kW0 + 1 && rank == 0) {
       // ================================ MMA issuer (leader CTA) ======================
       // S(j) = Q K(j)^T for j = 0, 1, 2 up front; then per block n: O += P(n) V(n), S(n+3) = Q K(n+3)^T into buffer n mod 3.
       const uint32_t q_lo = desc_lo(base + kOff2Q, 16);
@@ -954,6 +968,221 @@ uf_attn_pair_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
         if (elect_one()) ufptx::tc_commit_2sm(bars + B2_O_FULL * 8);
       UF_ITEM_LOOP_END
     }
+  } else if (kGroups == 2) {
+    // ============================ softmax + epilogue, two groups of 8 warps (both CTAs) ======================
+    // 640 threads x 96 registers at launch; 16 x 32 x 104 + 4 x 32 x 40 fits that pool (112 would not: the request
+    // would never be granted)
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 104;");
+    const int grp = warp >> 3;                         // group: takes the steps with global number gs = grp (mod 2)
+    const int wq = warp & 3;                           // TMEM lane quarter
+    const int half = (warp >> 2) & 1;                  // which 64 keys of a block
+    const int row = wq * 32 + lane;
+    const uint32_t lane_addr = (uint32_t)(wq * 32) << 16;
+    const uint32_t col0 = (uint32_t)half * 64;
+    const float sl2 = a.sl2;
+    const uint64_t sl22 = pack2(sl2, sl2);
+    volatile uint8_t* xc = reinterpret_cast<volatile uint8_t*>(base_ptr + kOff2Xc);     // [group][half][row][parity]
+    volatile uint8_t* x_own = xc + ((grp * 2 + half) * 128 + row) * 2;
+    volatile uint8_t* x_oth = xc + ((grp * 2 + (half ^ 1)) * 128 + row) * 2;
+    volatile float* m0_s = reinterpret_cast<volatile float*>(base_ptr + kOff2M0);       // [row]
+    volatile int* rc_s = reinterpret_cast<volatile int*>(base_ptr + kOff2Rc);           // [row]
+    volatile uint32_t* cnt_s = reinterpret_cast<volatile uint32_t*>(base_ptr + kOff2Cnt);
+    const uint32_t o_tmem = tmem + lane_addr + 384 + col0;                              // this thread's 64 O columns (rescale)
+    uint32_t oph = 0, sph = 0;                         // sph: one parity bit per S buffer, toggled at EVERY step
+    uint32_t gs = 0;                                   // global step number (all items, all steps, both groups count)
+    auto pow2neg = [](int k) { return __int_as_float((127 - min(k, 126)) << 23); };     // 2^-k
+
+    UF_ITEM_LOOP_BEGIN
+      const bool tile_exists = (full_mask >> rank) & 1;
+      float m0 = 0.f, l = 0.f;                         // the row's reference max is m0 + r
+      int r_loc = 0;                                   // r this thread's l (and last P) is relative to
+      int d_own = 0, par = 0, n = 0;
+      uint32_t buf = 0;                                // S / P buffer of the step: n mod 3 (the MMA warp restarts at 0 per item)
+      bool seen_first = false;                         // a block this tile attends has been processed (by either group)
+      bool have_m = false;                             // this thread has taken part since: m0, r_loc, l are valid
+
+      // one key block.  mine: this group's turn.  Every thread of both groups walks all steps (gs, seen_first).
+      auto step = [&](const bool attend, const int nvalid) {
+        const bool mine = ((gs & 1u) == (uint32_t)grp);
+        if (mine) {
+          const uint32_t s_tmem = tmem + lane_addr + buf * 128 + col0;      // this thread's 64 S columns
+          const int left = nvalid - (int)col0;
+          mbar_wait(bars + (B2_S_FULL0 + buf) * 8, (sph >> buf) & 1u);
+          tc_fence_after();
+          // the previous step (the other group's) has published its decision
+          while (*cnt_s < gs) { }
+          asm volatile("bar.sync %0, 64;" ::"r"(2 + grp * 4 + wq) : "memory");          // row partners step together
+          uint32_t sa[32], pk[16];
+          int D_eff = 0;
+          const bool exact = attend && !seen_first;
+          if (attend && seen_first) {
+            // adopt the row's current m; raise it if this group's previous step asked for more
+            const int r_cur = rc_s[row];
+            const bool joined = have_m;      // else: first block this thread computes in the item (its partner's too)
+            if (!joined) { m0 = m0_s[row]; r_loc = r_cur; l = 0.f; have_m = true; d_own = 0; }
+            const int want = r_loc + (joined ? max(d_own, (int)x_oth[par ^ 1]) : 0);   // relative to this group's last step
+            const int r_new = max(r_cur, want);
+            D_eff = r_new - r_cur;
+            l *= pow2neg(r_new - r_loc);
+            r_loc = r_new;
+          }
+          asm volatile("bar.sync %0, 64;" ::"r"(2 + grp * 4 + wq) : "memory");          // both threads of the row have read r
+          if (D_eff > 0 && half == 0) rc_s[row] = r_loc;
+          if (exact) {
+            // first attended block of the item: exact row max before the exponentials
+            float mx0 = -INFINITY, mx1 = -INFINITY;
+#pragma unroll
+            for (int c = 0; c < 2; ++c) {
+              UF_TMEM_LD32(s_tmem + c * 32, sa, 0);
+              UF_TMEM_WAIT_LD32(sa);
+#pragma unroll
+              for (int u = 0; u < 32; u += 2) {
+                const float v0 = (c * 32 + u < left) ? __uint_as_float(sa[u]) : -INFINITY;
+                const float v1 = (c * 32 + u + 1 < left) ? __uint_as_float(sa[u + 1]) : -INFINITY;
+                if (u & 2) mx1 = max3(mx1, v0, v1); else mx0 = max3(mx0, v0, v1);
+              }
+            }
+            const uint32_t mine_b = bf16_bits_up(fmaxf(mx0, mx1));
+            *reinterpret_cast<volatile uint16_t*>(x_own) = (uint16_t)mine_b;
+            asm volatile("bar.sync %0, 64;" ::"r"(2 + grp * 4 + wq) : "memory");
+            const uint32_t theirs = *reinterpret_cast<volatile uint16_t*>(x_oth);
+            asm volatile("bar.sync %0, 64;" ::"r"(2 + grp * 4 + wq) : "memory");
+            m0 = fmaxf(__uint_as_float(mine_b << 16), __uint_as_float(theirs << 16)) * sl2;
+            r_loc = 0; l = 0.f; have_m = true; d_own = 0;
+            x_own[0] = 0; x_own[1] = 0;                 // the exchange slots held the bf16 max: no raise pending
+            if (half == 0) { m0_s[row] = m0; rc_s[row] = 0; }
+          }
+          // publish: everything this step decided is in shared memory before the next step may start
+          __threadfence_block();
+          asm volatile("bar.sync %0, 256;" ::"r"(10 + grp) : "memory");
+          if ((warp & 7) == 0 && lane == 0) *cnt_s = gs + 1u;
+          int Dnew = 0;
+          if (attend) {
+            const float m = m0 + (float)r_loc;
+            const uint64_t nm2 = pack2(-m, -m);
+            uint64_t acc0 = pack2(0.f, 0.f), acc1 = acc0;
+            UF_TMEM_LD32(s_tmem + 0, sa, 0);
+            UF_TMEM_WAIT_LD32(sa);
+            exp_chunk(sa, pk, half * 2 + 0, left, sl22, nm2, acc0, acc1);
+            UF_TMEM_ST16(s_tmem + 0, pk);
+            UF_TMEM_LD32(s_tmem + 32, sa, 0);
+            UF_TMEM_WAIT_LD32(sa);
+            exp_chunk(sa, pk, half * 2 + 1, left - 32, sl22, nm2, acc0, acc1);
+            UF_TMEM_ST16(s_tmem + 16, pk);
+            float a0, a1, b0, b1;
+            unpack2(acc0, a0, a1);
+            unpack2(acc1, b0, b1);
+            const float lsum = (a0 + a1) + (b0 + b1);
+            l += lsum;
+            if (!(lsum <= 256.0f)) {
+              if (lsum < kPanicSum) {
+                Dnew = (int)((__float_as_uint(lsum) >> 23) & 0xffu) - 126;
+              } else {
+                a.panic_item[it] = a.seq;
+                *a.panic_last = a.seq;
+                Dnew = 101;
+              }
+            }
+          } else {
+            // a block only the other tile of the pair attends: P = 0
+#pragma unroll
+            for (int c = 0; c < 16; ++c) pk[c] = 0u;
+            UF_TMEM_ST16(s_tmem + 0, pk);
+            UF_TMEM_ST16(s_tmem + 16, pk);
+          }
+          x_own[par] = (uint8_t)Dnew;
+          d_own = Dnew;
+          par ^= 1;
+          // O still holds the blocks before this one relative to the m before this step's raise: every O += P V issued
+          // so far must be complete (the previous step's, number gs - 1, was the last), the next waits for our P_FULL
+          if (__any_sync(0xffffffffu, D_eff > 0) && n > 0) {
+            const uint32_t g = gs - 1u;
+            mbar_wait(bars + (B2_PV_DONE0 + (g & 1u)) * 8, (g >> 1) & 1u);
+            tc_fence_after();
+            const float f = pow2neg(D_eff);
+#pragma unroll
+            for (int cc = 0; cc < 64; cc += 32) {
+              UF_TMEM_LD32(o_tmem + cc, sa, 0);
+              UF_TMEM_WAIT_LD32(sa);
+#pragma unroll
+              for (int c = 0; c < 32; ++c) sa[c] = __float_as_uint(__uint_as_float(sa[c]) * f);
+              UF_TMEM_ST32(o_tmem + cc, sa, 0);
+            }
+          }
+          tmem_wait_st();
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) ufptx::mbar_arrive_leader(bars + (B2_P_FULL0 + buf) * 8);
+        }
+        if (attend) seen_first = true;
+        sph ^= 1u << buf;
+        buf = (buf == 2u) ? 0u : buf + 1u;
+        ++gs;
+        ++n;
+      };
+
+      {
+        int32_t mine_e = 0;
+        for (int st = 0; st < n_u; ++st) {
+          if ((st & 31) == 0) mine_e = (st + lane < n_u) ? __ldg(ulist + st + lane) : 0;
+          const int32_t e = __shfl_sync(0xffffffffu, mine_e, st & 31);
+          step(((uf_entry_mask(e) >> rank) & 1) != 0, uf_entry_nvalid(e));
+        }
+        for (int j = 0; j < a.n_sink + a.n_cur; ++j) {
+          const int nvalid = (j < a.n_sink) ? min(128, a.sink_ntok - j * 128) : min(128, a.ntok - (j - a.n_sink) * 128);
+          step(tile_exists, nvalid);
+        }
+      }
+
+      // ---- epilogue: O / l -> bf16 -> swizzled staging (the Q buffer) -> TMA store; the 16 warps split O 4 ways ----
+      {
+        unsigned char* stage = base_ptr + kOff2Q;
+        mbar_wait(bars + B2_O_FULL * 8, oph);          // every MMA of the item is complete: Q is free too
+        oph ^= 1;
+        tc_fence_after();
+        asm volatile("bar.sync 1, 512;" ::: "memory");                     // every step's decision is in shared memory
+        const int r_fin = have_m ? rc_s[row] : 0;
+        volatile float* xl = reinterpret_cast<volatile float*>(stage);
+        xl[(grp * 2 + half) * 128 + row] = have_m ? l * pow2neg(r_fin - r_loc) : 0.f;
+        asm volatile("bar.sync 1, 512;" ::: "memory");
+        const float l_tot = (xl[row] + xl[128 + row]) + (xl[256 + row] + xl[384 + row]);
+        const float m_fin = m0_s[row] + (float)rc_s[row];
+        asm volatile("bar.sync 1, 512;" ::: "memory");                     // all read before the staging writes
+        const float inv = 1.0f / l_tot;
+        {
+          uint32_t ov[32];
+          UF_TMEM_LD32(tmem + lane_addr + 384 + col0 + grp * 32, ov, 0);   // columns [64 half + 32 grp, + 32)
+          UF_TMEM_WAIT_LD32(ov);
+          unsigned char* half_base = stage + half * kHalf + row * 128;
+#pragma unroll
+          for (int j = 0; j < 4; ++j) {
+            uint4 w;
+            w.x = pack_bf16x2(__uint_as_float(ov[8 * j + 0]) * inv, __uint_as_float(ov[8 * j + 1]) * inv);
+            w.y = pack_bf16x2(__uint_as_float(ov[8 * j + 2]) * inv, __uint_as_float(ov[8 * j + 3]) * inv);
+            w.z = pack_bf16x2(__uint_as_float(ov[8 * j + 4]) * inv, __uint_as_float(ov[8 * j + 5]) * inv);
+            w.w = pack_bf16x2(__uint_as_float(ov[8 * j + 6]) * inv, __uint_as_float(ov[8 * j + 7]) * inv);
+            const int chunk = grp * 4 + j;
+            *reinterpret_cast<uint4*>(half_base + ((chunk ^ (row & 7)) << 4)) = w;
+          }
+        }
+        tc_fence_before();
+        fence_proxy_async();
+        asm volatile("bar.sync 1, 512;" ::: "memory");
+        const int row0 = (2 * p + rank) * 128;
+        if (warp == 0 && lane == 0) {
+          if (tile_exists) {
+            const uint32_t src = base + kOff2Q;
+            tma_store_3d(&tm_o, src, 0, row0, h);
+            tma_store_3d(&tm_o, src + kHalf, 64, row0, h);
+            tma_store_commit_and_wait_read();
+          }
+          mbar_arrive(bars + B2_Q_EMPTY * 8);
+        }
+        if (tile_exists && grp == 0 && half == 0 && a.lse != nullptr && row0 + row < a.ntok)
+          a.lse[(int64_t)h * a.ntok + row0 + row] = (m_fin + log2f(l_tot)) * 0.6931471805599453f;
+      }
+    UF_ITEM_LOOP_END
+    if (warp == 0 && lane == 0) tma_store_wait_all();
   } else {
     // ================================== softmax + epilogue (both CTAs) ======================
     asm volatile("setmaxnreg.inc.sync.aligned.u32 208;");
@@ -1160,7 +1389,7 @@ uf_attn_pair_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
   tc_fence_before();
   __syncthreads();
   ufptx::cluster_sync();                               // neither CTA frees TMEM or exits while the other may still use it
-  if (warp == 10) {
+  if (warp == kW0 + 2) {
     asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, 512;" ::"r"(tmem) : "memory");
   }
 }
@@ -1223,9 +1452,11 @@ int uf_sm100_make_cache_maps(uf_ctx* c) {
   if (e == cudaSuccess)
     e = cudaFuncSetAttribute(uf_attn_sm100_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
   if (e == cudaSuccess)
-    e = cudaFuncSetAttribute(uf_attn_pair_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes2);
+    e = cudaFuncSetAttribute(uf_attn_pair_kernel<false, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes2);
   if (e == cudaSuccess)
-    e = cudaFuncSetAttribute(uf_attn_pair_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes2);
+    e = cudaFuncSetAttribute(uf_attn_pair_kernel<false, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes2);
+  if (e == cudaSuccess)
+    e = cudaFuncSetAttribute(uf_attn_pair_kernel<true, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes2);
   if (e != cudaSuccess) {
     c->err = std::string("cudaFuncSetAttribute(smem): ") + cudaGetErrorString(e);
     return UF_ERR_CUDA;
@@ -1262,11 +1493,16 @@ int uf_launch_attn_sm100(uf_ctx* c, const UfView& v, const __nv_bfloat16* q, __n
   if (++c->attn_seq <= 0) c->attn_seq = 1;
   a.panic_item = c->panic_item; a.panic_last = c->panic_last; a.seq = c->attn_seq;
   // fast kernel, then the safe kernel for the items it flagged (returns at once when there are none)
-  if (c->attn_impl == 2) {
+  if (c->attn_impl == 3) {
+    // CTA pairs with two softmax groups per CTA (640 threads); flagged items are redone by the one-group exact-max kernel
+    const int pairs = n_items < c->sm_count / 2 ? n_items : c->sm_count / 2;
+    uf_attn_pair_kernel<false, 2><<<2 * pairs, 20 * 32, kSmemBytes2, s>>>(tm_q, tm_o, c->tm_k_half, c->tm_v, a);
+    uf_attn_pair_kernel<true, 1><<<2 * pairs, kThreads, kSmemBytes2, s>>>(tm_q, tm_o, c->tm_k_half, c->tm_v, a);
+  } else if (c->attn_impl == 2) {
     // CTA pairs: one query tile per CTA, the pair shares every K / V tile (uf_attn_pair_kernel)
     const int pairs = n_items < c->sm_count / 2 ? n_items : c->sm_count / 2;
-    uf_attn_pair_kernel<false><<<2 * pairs, kThreads, kSmemBytes2, s>>>(tm_q, tm_o, c->tm_k_half, c->tm_v, a);
-    uf_attn_pair_kernel<true><<<2 * pairs, kThreads, kSmemBytes2, s>>>(tm_q, tm_o, c->tm_k_half, c->tm_v, a);
+    uf_attn_pair_kernel<false, 1><<<2 * pairs, kThreads, kSmemBytes2, s>>>(tm_q, tm_o, c->tm_k_half, c->tm_v, a);
+    uf_attn_pair_kernel<true, 1><<<2 * pairs, kThreads, kSmemBytes2, s>>>(tm_q, tm_o, c->tm_k_half, c->tm_v, a);
   } else {
     uf_attn_sm100_kernel<false><<<grid, kThreads, kSmemBytes, s>>>(tm_q, tm_o, c->tm_k, c->tm_v, a);
     uf_attn_sm100_kernel<true><<<grid, kThreads, kSmemBytes, s>>>(tm_q, tm_o, c->tm_k, c->tm_v, a);
