@@ -798,7 +798,7 @@ def main():
                                                          "cmn_upsampler_1k", "cmn_decoder_crop"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--attn-impl", type=int, default=0, choices=[0, 2, 3],
+    ap.add_argument("--attn-impl", type=int, default=0, choices=[0, 2],
                     help="uf_set_attn_impl: 0 = the default tcgen05 attention kernel, 2 = the other tcgen05 variant")
     ap.add_argument("--no-also", action="store_true", help="skip the secondary workloads (2k, wide, 1k_stream, paper-mask variants)")
     ap.add_argument("--also", default="2k,1k_stream,wide,1k_paper,2k_paper,1k_fused,2k_fused,cmn_upsampler_1k,cmn_decoder_crop",

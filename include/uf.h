@@ -272,8 +272,8 @@ int32_t uf_get_select_usage(uf_ctx* ctx, int64_t* kept_per_chunk, int32_t* chunk
 /* impl: 0 = tcgen05 kernel only (default; shapes it does not cover -> UF_ERR_UNSUPPORTED),
  *       1 = the generic CUDA-core attention kernel (any supported shape; slow),
  *       2 = the CTA-pair tcgen05 kernel (cta_group::2 MMAs over two CTAs, one query tile per CTA, each CTA loads half of
- *           every K / V tile, triple-buffered S; same shapes and results as 0 within the tolerance; measured slower on
- *           B200, kept selectable: DESIGN.md 5.1). */
+ *           every K / V tile, triple-buffered S, two softmax warp groups per CTA taking the key blocks in turn; same
+ *           shapes and results as 0 within the tolerance; measured 3-5 % slower on B200, kept selectable: DESIGN.md 5.1). */
 int32_t uf_set_attn_impl(uf_ctx* ctx, int32_t impl);
 
 /* Observability (host outputs).

@@ -581,7 +581,7 @@ int32_t uf_next_window(uf_ctx* c, const uf_window_policy* p, int32_t* window_chu
 }
 
 int32_t uf_set_attn_impl(uf_ctx* c, int32_t impl) {
-  if (!c || impl < 0 || impl > 3) return UF_ERR_INVALID_ARG;
+  if (!c || impl < 0 || impl > 2) return UF_ERR_INVALID_ARG;
   c->attn_impl = impl;
   return UF_OK;
 }

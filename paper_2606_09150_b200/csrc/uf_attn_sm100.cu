@@ -794,7 +794,8 @@ enum Bar2 {
   B2_Q_FULL = 0, B2_Q_EMPTY,
   B2_K_FULL0 = 2, B2_K_EMPTY0 = B2_K_FULL0 + kNK2,
   B2_V_FULL0 = B2_K_EMPTY0 + kNK2, B2_V_EMPTY0 = B2_V_FULL0 + kNV2,
-  B2_S_FULL0 = B2_V_EMPTY0 + kNV2, B2_P_FULL0 = B2_S_FULL0 + 3, B2_PV_DONE0 = B2_P_FULL0 + 3, B2_O_FULL = B2_PV_DONE0 + 2, kNumBars2
+  B2_S_FULL0 = B2_V_EMPTY0 + kNV2, B2_P_FULL0 = B2_S_FULL0 + 3, B2_PV_DONE0 = B2_P_FULL0 + 3, B2_O_FULL = B2_PV_DONE0 + 2,
+  B2_DEC0, kNumBars2 = B2_DEC0 + 2           // DEC[gs & 1]: step gs of a two-group kernel has published its decision
 };
 constexpr int kOff2TmemPtr = kOff2Bar + kNumBars2 * 8;
 constexpr int kOff2Xc = kOff2TmemPtr + 16;                    // row-pair exchange: [group][half][row][parity] bytes
@@ -1009,8 +1010,9 @@ uf_attn_pair_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
           const int left = nvalid - (int)col0;
           mbar_wait(bars + (B2_S_FULL0 + buf) * 8, (sph >> buf) & 1u);
           tc_fence_after();
-          // the previous step (the other group's) has published its decision
-          while (*cnt_s < gs) { }
+          // the previous step (the other group's) has published its decision (its successor on the same barrier, step
+          // gs + 1, waits for this step's: no aliasing)
+          if (gs > 0u) mbar_wait(bars + (B2_DEC0 + ((gs - 1u) & 1u)) * 8, ((gs - 1u) >> 1) & 1u);
           asm volatile("bar.sync %0, 64;" ::"r"(2 + grp * 4 + wq) : "memory");          // row partners step together
           uint32_t sa[32], pk[16];
           int D_eff = 0;
@@ -1055,7 +1057,7 @@ uf_attn_pair_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_const
           // publish: everything this step decided is in shared memory before the next step may start
           __threadfence_block();
           asm volatile("bar.sync %0, 256;" ::"r"(10 + grp) : "memory");
-          if ((warp & 7) == 0 && lane == 0) *cnt_s = gs + 1u;
+          if ((warp & 7) == 0 && lane == 0) mbar_arrive(bars + (B2_DEC0 + (gs & 1u)) * 8);
           int Dnew = 0;
           if (attend) {
             const float m = m0 + (float)r_loc;
@@ -1452,8 +1454,6 @@ int uf_sm100_make_cache_maps(uf_ctx* c) {
   if (e == cudaSuccess)
     e = cudaFuncSetAttribute(uf_attn_sm100_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
   if (e == cudaSuccess)
-    e = cudaFuncSetAttribute(uf_attn_pair_kernel<false, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes2);
-  if (e == cudaSuccess)
     e = cudaFuncSetAttribute(uf_attn_pair_kernel<false, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes2);
   if (e == cudaSuccess)
     e = cudaFuncSetAttribute(uf_attn_pair_kernel<true, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes2);
@@ -1493,15 +1493,11 @@ int uf_launch_attn_sm100(uf_ctx* c, const UfView& v, const __nv_bfloat16* q, __n
   if (++c->attn_seq <= 0) c->attn_seq = 1;
   a.panic_item = c->panic_item; a.panic_last = c->panic_last; a.seq = c->attn_seq;
   // fast kernel, then the safe kernel for the items it flagged (returns at once when there are none)
-  if (c->attn_impl == 3) {
-    // CTA pairs with two softmax groups per CTA (640 threads); flagged items are redone by the one-group exact-max kernel
+  if (c->attn_impl == 2) {
+    // CTA pairs: one query tile per CTA, the pair shares every K / V tile, two softmax groups per CTA (640 threads);
+    // flagged items are redone by the one-group exact-max instantiation
     const int pairs = n_items < c->sm_count / 2 ? n_items : c->sm_count / 2;
     uf_attn_pair_kernel<false, 2><<<2 * pairs, 20 * 32, kSmemBytes2, s>>>(tm_q, tm_o, c->tm_k_half, c->tm_v, a);
-    uf_attn_pair_kernel<true, 1><<<2 * pairs, kThreads, kSmemBytes2, s>>>(tm_q, tm_o, c->tm_k_half, c->tm_v, a);
-  } else if (c->attn_impl == 2) {
-    // CTA pairs: one query tile per CTA, the pair shares every K / V tile (uf_attn_pair_kernel)
-    const int pairs = n_items < c->sm_count / 2 ? n_items : c->sm_count / 2;
-    uf_attn_pair_kernel<false, 1><<<2 * pairs, kThreads, kSmemBytes2, s>>>(tm_q, tm_o, c->tm_k_half, c->tm_v, a);
     uf_attn_pair_kernel<true, 1><<<2 * pairs, kThreads, kSmemBytes2, s>>>(tm_q, tm_o, c->tm_k_half, c->tm_v, a);
   } else {
     uf_attn_sm100_kernel<false><<<grid, kThreads, kSmemBytes, s>>>(tm_q, tm_o, c->tm_k, c->tm_v, a);
