@@ -1,5 +1,6 @@
 """GPU parity of the CTA-pair attention kernel (uf_set_attn_impl(ctx, 2): cta_group::2 MMAs over two CTAs, one query
-tile per CTA, triple-buffered S) against the fp64 oracle, on the cases that exercise what is specific to it: an odd
+tile per CTA, triple-buffered S, two softmax warp groups per CTA taking the key blocks in turn with one shared reference
+max per row) against the fp64 oracle, on the cases that exercise what is specific to it: an odd
 number of query blocks (the second CTA of the last pair has no tile), blocks only one tile of a pair attends
 (zero-fill steps), the deferred raise of the reference max with the tensor pipe up to two blocks behind, the
 exact-max redo kernel, and BASELINE.json configs[1] at full size (every row against the default kernel, sampled
