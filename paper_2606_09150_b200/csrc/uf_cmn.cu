@@ -462,14 +462,18 @@ void plan_layer(Layer& L, int frames, int sms) {
     const int cells = ((m_tiles + 1) / 2) * L.n_ntiles;
     const int grid = cells < sms / 2 ? cells : sms / 2;
     const int per_pair = (cells + grid - 1) / grid;
-    const int mt_single = L.n_tile > 128 ? 2 : 4, mt_double = L.n_tile > 128 ? 1 : L.n_tile > 64 ? 2 : 4;
+    const int mt_single = L.n_tile > 128 ? 2 : 4, mt_double = L.n_tile > 128 ? 1 : L.n_tile > 64 ? 2 : 4;   // (N <= 64 with MT = 2 and a 4-deep A ring: measured slower)
     L.MT = per_pair <= mt_single ? mt_single : mt_double;
   }
   L.n_acc = (L.MT * L.n_tile <= 256) ? 2 : 1;
-  L.nA = 2;
+  // ring depths: an A stage (MT tall tiles) lasts 3 * 4 * MT * N/2 tensor cycles, less than a TMA round trip for the
+  // narrow layers, so the A ring gets up to 4 stages once 6 weight stages (two (slice, dx) groups) are reserved
   const size_t budget = 227 * 1024 - 1024 - kMaxBias * 4 - 256;
-  const size_t a = (size_t)L.nA * L.MT * kATileBytes;
-  const int nb = (int)((budget - a) / ((size_t)(L.n_tile / 2) * 128));
+  const size_t b_stage = (size_t)(L.n_tile / 2) * 128, a_stage = (size_t)L.MT * kATileBytes;
+  int na = (int)((budget - 6 * b_stage) / a_stage);
+  L.nA = na < 2 ? 2 : na > 4 ? 4 : na;
+  const size_t a = (size_t)L.nA * a_stage;
+  const int nb = (int)((budget - a) / b_stage);
   L.nB = nb > 8 ? 8 : nb;
   L.smem = a + (size_t)L.nB * (L.n_tile / 2) * 128 + kMaxBias * 4 + 256 + 1024;
   L.plan_frames = frames;
