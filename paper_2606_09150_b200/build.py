@@ -19,9 +19,9 @@ CSRC = os.path.join(PKG_DIR, "csrc")
 LIB = os.path.join(PKG_DIR, "libuf.so")
 
 SOURCES = ["uf_api.cu", "uf_append.cu", "uf_fused_append.cu", "uf_select.cu", "uf_attn_generic.cu", "uf_attn_sm100.cu",
-           "uf_cmn.cu"]
+           "uf_cmn.cu", "uf_select_static.cu"]
 HEADERS = [os.path.join(CSRC, "uf_internal.h"), os.path.join(CSRC, "uf_sm100_ptx.h"), os.path.join(ROOT, "include", "uf.h"),
-           os.path.join(ROOT, "include", "uf_cmn.h")]
+           os.path.join(ROOT, "include", "uf_cmn.h"), os.path.join(ROOT, "include", "uf_static.h")]
 
 NVCC_FLAGS = [
     "-O3", "-std=c++17",
