@@ -167,7 +167,10 @@ typedef struct uf_tiling {
 int32_t uf_ctx_set_tiling(uf_ctx* ctx, const uf_tiling* tiling);
 
 /* Host query: N_blocks = blocks in the causal mask for the current state (all resident chunks incl. the newest)
- * and the budget k' = min(k, N_blocks), k = topk_count if >= 0 else tau_k(rho_permille / 1000) above. */
+ * and the budget k' = min(k, N_blocks), k = topk_count if >= 0 else tau_k(rho_permille / 1000) above.  k' is the
+ * size of the top-k BEFORE the window: the blocks a row really keeps are top-k' n M_local plus its own block (the
+ * cnt_out of uf_select_blocks_paper), fewer than k' + 1 wherever the window cuts.  The 0.42 of tau_k was read off
+ * Table 21's default row as a pre-window fraction; the executed mask is sparser than that column (R-34). */
 int32_t uf_query_budget_paper(const uf_ctx* ctx, int32_t topk_count, int32_t rho_permille,
                               int32_t* n_blocks, int32_t* k_eff);
 
@@ -206,7 +209,12 @@ int32_t uf_untile_tokens(uf_ctx* ctx, const void* tiled, void* raster,
  *   write    post-RoPE Q -> q_out; post-RoPE K and V -> the cache slot, exactly as uf_kv_append (same eviction policy,
  *            sink copy, zero pad rows); block-mean pooled K and pooled Q -> the ctx.
  * A following uf_select_blocks / uf_select_blocks_paper called with q == q_out (same strides) skips its pooling
- * pass.  Token positions: raster order (t, y, x) over a grid_h x grid_w grid (token n: t = t0 + n / (gh*gw), ...); on a
+ * pass: it is recognised by ADDRESS AND STRIDES ONLY, so the buffer must still hold, bit for bit, what this call
+ * wrote.  A caller that rewrites q_out (or reuses its memory for another Q) between the two calls must switch the
+ * shortcut off with uf_set_pooled_q_reuse(ctx, 0); otherwise the selection is made for the Q this call wrote, not for
+ * the q argument, and no error is raised.
+ * Aliasing: q_out may be q_in itself (same pointer and strides: in place); any other overlap of q_out with q_in,
+ * k_in or v_in is refused (UF_ERR_INVALID_ARG).  Disjoint slices of one fused tensor are fine.  Token positions: raster order (t, y, x) over a grid_h x grid_w grid (token n: t = t0 + n / (gh*gw), ...); on a
  * tiled ctx the tiling's grid and order are used and grid_h / grid_w are ignored.  head_dim must be 128.
  * Errors as uf_kv_append, plus UF_ERR_CAPACITY when a position exceeds max_pos. */
 typedef struct uf_rope_spec {
@@ -225,6 +233,10 @@ int32_t uf_qkv_rope_append(uf_ctx* ctx, const void* q_in, const void* k_in, cons
                            int32_t n_tokens, int64_t in_tok_stride, int64_t in_head_stride,
                            int64_t out_tok_stride, int64_t out_head_stride,
                            const uf_rope_spec* rope, int32_t window_chunks, void* stream);
+
+/* on != 0 (default): a select called with the q_out pointer and strides of the chunk's uf_qkv_rope_append reuses the
+ * pooled Q that call produced.  on == 0: every select pools the q it is given (one more small kernel per call). */
+int32_t uf_set_pooled_q_reuse(uf_ctx* ctx, int32_t on);
 
 /* ---- SR cache window policy --------------------------------------------------------------
  * The paper states the idea three times and gives no rule: P:136 (iii) "dynamically selecting a compact cache window,

@@ -1,6 +1,11 @@
 /* uf_cmn.h — C ABI of the causal memory network streaming step of Ultra Flash:
  * the streaming latent upsampler and the HR decoder of paper section 2.2, Eq. 2,
- * Algorithm 2 variant B, configurations P:345-347.  Same library as uf.h
+ * Algorithm 2, configurations P:345-347: VARIANT A's function (the memory of a block is its INPUT one
+ * frame earlier, line 7 at P:482), evaluated as a stream with the state variant B keeps (one memory per block in the
+ * handle).  It is NOT variant B as printed: lines 31-32 store the block OUTPUT, a recurrence over frames
+ * that is a different function from the second frame on (reading R-41; oracle/uf_causal_mem.py
+ * CausalMemStream(memory="output") is that literal form, and tests/test_causal_mem_pins.py pins the difference).
+ * Weights trained against the literal variant B are not served by this call.  Same library as uf.h
  * (paper_2606_09150_b200/libuf.so); status codes and conventions are those of uf.h.
  *
  * What one uf_cmn_step computes, for the next n_frames input frames z of a video stream:

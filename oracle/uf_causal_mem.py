@@ -23,7 +23,8 @@ Readings (R-41 ... R-46; the paper is silent or at odds with itself)
         sequential (streaming inference) execution modes" the same function.  Taken: m_t^(l) = h_t^(l-1),
         the block's input at the previous frame of the block's own frame rate; the first frame of a stream sees
         zeros.  `forward_parallel` (A) and `CausalMemStream.step` (B) implement it independently and are pinned
-        to agree frame by frame.
+        to agree frame by frame.  The literal variant B (memory = block OUTPUT) is available as
+        `CausalMemStream(..., memory="output")`; it is a different function from the second frame on.
   R-42  Zero padding (spatial size is preserved by every 3x3 convolution); cross-correlation as in every deep
         learning framework: out[y,x,o] = b[o] + sum_{i,dy,dx} w[o,i,dy,dx] * in[y+dy-1, x+dx-1, i].
   R-43  Every convolution has a bias except W_skip (Eq. 2 writes it as a plain projection); no activation other
@@ -199,8 +200,16 @@ class CausalMemStream:
     """State = one memory frame per block (zeros at the start of a stream).  `step` takes the next frames of the
     stream (any number; a chunk) and emits their outputs; frame by frame inside (Alg. 2 line 24)."""
 
-    def __init__(self, cfg: CmnConfig, wt: dict):
-        self.cfg, self.wt = cfg, wt
+    def __init__(self, cfg: CmnConfig, wt: dict, memory: str = "input"):
+        """memory = "input" (default, R-41: what the GPU path and `forward_parallel` compute): a block remembers its
+        INPUT at the previous frame, Alg. 2 variant A line 7 carried into the streaming loop.
+        memory = "output": Alg. 2 variant B exactly as printed: the memory is overwritten
+        with h AFTER the block's ReLU, i.e. the block's OUTPUT.  That is a recurrence over frames (every earlier frame
+        reaches the current one), cannot be evaluated for all frames at once, and is NOT the function variant A
+        defines; it exists here so that the difference between the two readings is a number, not an argument."""
+        if memory not in ("input", "output"):
+            raise ValueError(memory)
+        self.cfg, self.wt, self.memory = cfg, wt, memory
         self.mem: dict[str, np.ndarray | None] = {}
         self.reset()
 
@@ -215,8 +224,11 @@ class CausalMemStream:
             for b in range(b0, self.cfg.n_blocks):
                 p = f"s{s}.b{b}."
                 m = self.mem[p] if self.mem[p] is not None else np.zeros_like(x)
-                self.mem[p] = x                              # R-41: the block's input is the next frame's memory
+                if self.memory == "input":
+                    self.mem[p] = x                          # R-41: the block's input is the next frame's memory
                 x = mem_block(x, m, self.wt, p)
+                if self.memory == "output":
+                    self.mem[p] = x                          # variant B lines 31-32 as printed: m <- h after the ReLU
             outs.append(x)
         return np.concatenate(outs, axis=0)
 

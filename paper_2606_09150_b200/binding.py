@@ -24,7 +24,7 @@ SYMBOLS = [
     "uf_ctx_create", "uf_ctx_destroy", "uf_ctx_reset", "uf_kv_append", "uf_query_topk", "uf_select_blocks",
     "uf_sparse_attn_fwd", "uf_set_attn_impl", "uf_get_slot_map", "uf_get_cache_block", "uf_get_pooled_k",
     "uf_attn_redone_items", "uf_ctx_device_bytes", "uf_ctx_launch_count", "uf_last_error", "uf_version",
-    "uf_next_window", "uf_get_select_usage", "uf_qkv_rope_append",
+    "uf_next_window", "uf_get_select_usage", "uf_qkv_rope_append", "uf_set_pooled_q_reuse",
     "uf_ctx_set_tiling", "uf_query_budget_paper", "uf_select_blocks_paper", "uf_tile_tokens", "uf_untile_tokens",
 ]
 
@@ -96,6 +96,7 @@ def load_library() -> ctypes.CDLL:
     lib.uf_untile_tokens.argtypes = [P, P, P, c_int64, c_int64, c_int64, c_int64, P]
     lib.uf_qkv_rope_append.argtypes = [P, P, P, P, P, c_int32, c_int64, c_int64, c_int64, c_int64,
                                        POINTER(uf_rope_spec), c_int32, P]
+    lib.uf_set_pooled_q_reuse.argtypes = [P, c_int32]
     lib.uf_next_window.argtypes = [P, POINTER(uf_window_policy), POINTER(c_int32), P]
     lib.uf_get_select_usage.argtypes = [P, POINTER(c_int64), POINTER(c_int32), POINTER(c_int32), P]
     lib.uf_version.argtypes = []
@@ -179,6 +180,10 @@ def uf_qkv_rope_append(ctx, q_in, k_in, v_in, q_out, n_tokens: int, in_tok_strid
     _check(ctx, load_library().uf_qkv_rope_append(ctx, _ptr(q_in), _ptr(k_in), _ptr(v_in), _ptr(q_out), n_tokens,
                                                   in_tok_stride, in_head_stride, out_tok_stride, out_head_stride,
                                                   byref(rs), window_chunks, _stream(stream)))
+
+
+def uf_set_pooled_q_reuse(ctx, on: bool) -> None:
+    _check(ctx, load_library().uf_set_pooled_q_reuse(ctx, 1 if on else 0))
 
 
 def uf_next_window(ctx, kind: int, warm_chunks: int = 0, compact_window: int = 1, min_share_permille: int = 0,

@@ -7,6 +7,7 @@
 #include <cstdio>
 #include <cstring>
 #include <new>
+#include <utility>
 
 namespace {
 
@@ -97,6 +98,28 @@ int check_tensor_args(uf_ctx* c, const void* p, int64_t tok_stride, int64_t head
   if (tok_stride < c->cfg.head_dim || head_stride < c->cfg.head_dim || (tok_stride % 8) || (head_stride % 8))
     return fail(c, UF_ERR_INVALID_ARG, std::string(name) + ": strides must be >= head_dim and multiples of 8 elements");
   return UF_OK;
+}
+
+// Do two [n, H, d] bf16 tensors (element strides ts, hs, 1) share an element?  Exact for the layouts a QKV projection
+// leaves behind when both have the same strides and rows / heads do not overlap themselves (slices of [n, 3, H, d] or
+// of [n, H, 3, d]: the byte ranges interleave but no element is shared); conservative (byte ranges) otherwise.
+bool tensors_overlap(const void* a, int64_t a_ts, int64_t a_hs, const void* b, int64_t b_ts, int64_t b_hs, int n, int H,
+                     int d) {
+  auto last = [&](int64_t ts, int64_t hs) { return (int64_t)(n - 1) * ts + (int64_t)(H - 1) * hs + d; };
+  const intptr_t pa = (intptr_t)a, pb = (intptr_t)b;
+  if (pa + 2 * last(a_ts, a_hs) <= pb || pb + 2 * last(b_ts, b_hs) <= pa) return false;      // disjoint byte ranges
+  if (a_ts != b_ts || a_hs != b_hs || ((pb - pa) & 1)) return true;
+  const int64_t ts = a_ts, hs = a_hs, hspan = (int64_t)(H - 1) * hs + d;
+  if (hspan > ts || d > hs) return true;                                                      // self-overlapping layout
+  const int64_t delta = (pb - pa) / 2;
+  const int64_t in_row = ((delta % ts) + ts) % ts;              // b's row start relative to the row of a it falls in
+  for (int64_t x : {in_row, in_row - ts}) {                     // ... and to the next row of a
+    if (x >= hspan || -x >= hspan) continue;                    // the two rows' occupied spans do not meet
+    if (H == 1) return true;
+    const int64_t y = ((x % hs) + hs) % hs;                     // same question one level down: head windows of d
+    if (y < d || hs - y < d) return true;
+  }
+  return false;
 }
 
 void clear_host_state(uf_ctx* c) {
@@ -290,6 +313,18 @@ int32_t uf_qkv_rope_append(uf_ctx* c, const void* q_in, const void* k_in, const 
   if (r) return r;
   if (!rs->cos_tab || !rs->sin_tab || !rs->gq || !rs->gk)
     return fail(c, UF_ERR_INVALID_ARG, "uf_qkv_rope_append: null table / weight pointer");
+  if (n_tokens >= 1) {
+    // q_out may be q_in itself (same pointer, same strides: a row is staged on chip before it is overwritten, and no
+    // other CTA reads it); every other overlap of q_out with an input would let one CTA overwrite rows another CTA
+    // has not read yet
+    const bool same_strides = out_tok_stride == in_tok_stride && out_head_stride == in_head_stride;
+    auto collides = [&](const void* in) {
+      return tensors_overlap(q_out, out_tok_stride, out_head_stride, in, in_tok_stride, in_head_stride, n_tokens,
+                             c->cfg.n_heads, c->cfg.head_dim);
+    };
+    if ((!(q_out == q_in && same_strides) && collides(q_in)) || collides(k_in) || collides(v_in))
+      return fail(c, UF_ERR_INVALID_ARG, "uf_qkv_rope_append: q_out overlaps an input (only q_out == q_in with equal strides is allowed)");
+  }
   if (rs->dim_t < 0 || rs->dim_h < 0 || rs->dim_w < 0 || (rs->dim_t & 1) || (rs->dim_h & 1) || (rs->dim_w & 1) ||
       rs->dim_t + rs->dim_h + rs->dim_w != c->cfg.head_dim)
     return fail(c, UF_ERR_INVALID_ARG, "uf_qkv_rope_append: axis dims must be even and sum to head_dim");
@@ -315,6 +350,12 @@ int32_t uf_qkv_rope_append(uf_ctx* c, const void* q_in, const void* k_in, const 
     c->qbar_chunk = c->next_chunk - 1; c->qbar_ptr = q_out; c->qbar_ts = out_tok_stride; c->qbar_hs = out_head_stride;
   }
   return st;
+}
+
+int32_t uf_set_pooled_q_reuse(uf_ctx* c, int32_t on) {
+  if (!c) return UF_ERR_INVALID_ARG;
+  c->reuse_pooled_q = on != 0;
+  return UF_OK;
 }
 
 int32_t uf_query_topk(const uf_ctx* c, int32_t topk_count, int32_t topk_percent, int32_t* n_cand, int32_t* k_eff) {
@@ -345,7 +386,7 @@ int32_t uf_select_blocks(uf_ctx* c, const void* q, int32_t n_tokens, int64_t tok
   if (r) return fail(c, r, "uf_select_blocks: topk_percent outside 0..100");
   if (k > c->kcap) return fail(c, UF_ERR_CAPACITY, "uf_select_blocks: k exceeds workspace (internal)");
   UF_CUDA(c, cudaSetDevice(c->cfg.device));
-  c->skip_pool_q = (c->qbar_chunk == v.cur_chunk && c->qbar_ptr == q && c->qbar_ts == tok_stride && c->qbar_hs == head_stride);
+  c->skip_pool_q = c->reuse_pooled_q && (c->qbar_chunk == v.cur_chunk && c->qbar_ptr == q && c->qbar_ts == tok_stride && c->qbar_hs == head_stride);
   cudaError_t e = uf_launch_select(c, v, (const __nv_bfloat16*)q, tok_stride, head_stride, k, idx_out, cnt_out,
                                    false, k, (cudaStream_t)stream);
   if (e != cudaSuccess) return fail_cuda(c, e, "uf_select_blocks kernel launch");
@@ -423,7 +464,7 @@ int32_t uf_select_blocks_paper(uf_ctx* c, const void* q, int32_t n_tokens, int64
   if (idx_out && idx_stride < max_row)
     return fail(c, UF_ERR_CAPACITY, "uf_select_blocks_paper: idx_stride < min(k + 1, N_blocks)");
   UF_CUDA(c, cudaSetDevice(c->cfg.device));
-  c->skip_pool_q = (c->qbar_chunk == v.cur_chunk && c->qbar_ptr == q && c->qbar_ts == tok_stride && c->qbar_hs == head_stride);
+  c->skip_pool_q = c->reuse_pooled_q && (c->qbar_chunk == v.cur_chunk && c->qbar_ptr == q && c->qbar_ts == tok_stride && c->qbar_hs == head_stride);
   cudaError_t e = uf_launch_select(c, v, (const __nv_bfloat16*)q, tok_stride, head_stride, k, idx_out, cnt_out,
                                    true, idx_stride, (cudaStream_t)stream);
   if (e != cudaSuccess) return fail_cuda(c, e, "uf_select_blocks_paper kernel launch");

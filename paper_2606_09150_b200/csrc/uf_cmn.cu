@@ -1,5 +1,5 @@
 // uf_cmn.cu — the causal memory network streaming step (include/uf_cmn.h; paper section 2.2, Eq. 2 P:65,
-// Alg. 2 variant B P:512-552): every convolution of the network as an implicit GEMM on the tcgen05 tensor cores.
+// Alg. 2: variant A's function — memory = block input one frame earlier, R-41 — streamed with per-block state): every convolution of the network as an implicit GEMM on the tcgen05 tensor cores.
 //
 // One kernel serves all layers.  GEMM view of a layer: M = output pixels (tiles of 128 = 8 rows x 16 columns of one
 // frame), N = output channels (<= 256 per tile), K = sum over the layer's sources of taps x channels:
@@ -409,6 +409,8 @@ struct uf_cmn {
   const void* z_ptr = nullptr;
   int z_frames = 0;
   int last_frames = 0;                // input frames of the last uf_cmn_step
+  bool smem_attr[3] = {};             // 227 KB dynamic-smem limit already raised on uf_cmn_conv_kernel<1 | 2 | 4> for
+                                      // THIS handle's device (the attribute is per device, so the flag is per handle)
   std::string err;
 };
 
@@ -494,8 +496,7 @@ void tile_options(Layer& L) {
 }
 
 template <int MT>
-cudaError_t launch_conv(const Layer& L, const ConvParams& p, int grid, cudaStream_t s) {
-  static bool attr_set = false;
+cudaError_t launch_conv(const Layer& L, const ConvParams& p, int grid, cudaStream_t s, bool& attr_set) {
   if (!attr_set) {
     cudaError_t e = cudaFuncSetAttribute(uf_cmn_conv_kernel<MT>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     if (e != cudaSuccess) return e;
@@ -688,6 +689,7 @@ int32_t uf_cmn_create(const uf_cmn_config* cfg, uf_cmn** out) {
 
 int32_t uf_cmn_destroy(uf_cmn* n) {
   if (!n) return UF_OK;
+  cudaSetDevice(n->cfg.device);
   for (Buf& b : n->bufs) if (b.p) cudaFree(b.p);
   for (Layer& L : n->layers) { if (L.w) cudaFree(L.w); if (L.bias) cudaFree(L.bias); }
   delete n;
@@ -742,6 +744,8 @@ int32_t uf_cmn_set_param(uf_cmn* n, const char* name, const void* w_host, const 
   for (Param& p : n->params) if (p.name == name) pp = &p;
   if (!pp) return cfail(n, UF_ERR_INVALID_ARG, std::string("uf_cmn_set_param: unknown parameter ") + name);
   if (!pp->has_bias && bias_host) return cfail(n, UF_ERR_INVALID_ARG, std::string(name) + " has no bias (R-43)");
+  { cudaError_t de = cudaSetDevice(n->cfg.device);
+    if (de != cudaSuccess) return cfail(n, UF_ERR_CUDA, std::string("cudaSetDevice: ") + cudaGetErrorString(de)); }
   Layer& L = n->layers[pp->layer];
   const int Co = pp->shape[0], Ci = pp->shape[1], kk = pp->shape[2] * pp->shape[3];
   const uint16_t* w = static_cast<const uint16_t*>(w_host);
@@ -799,6 +803,8 @@ int32_t uf_cmn_step(uf_cmn* n, const void* z, int32_t n_frames, void* out, void*
   if (n_frames < 1 || n_frames > n->cfg.frames_max) return cfail(n, UF_ERR_CAPACITY, "uf_cmn_step: n_frames outside 1..frames_max");
   for (const Param& p : n->params)
     if (!p.set) return cfail(n, UF_ERR_STATE, "uf_cmn_step: parameter " + p.name + " was never set");
+  { cudaError_t de = cudaSetDevice(n->cfg.device);
+    if (de != cudaSuccess) return cfail(n, UF_ERR_CUDA, std::string("cudaSetDevice: ") + cudaGetErrorString(de)); }
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   const uf_cmn_config& c = n->cfg;
   if (n->z_ptr != z || n->z_frames != n_frames) {
@@ -834,8 +840,9 @@ int32_t uf_cmn_step(uf_cmn* n, const void* z, int32_t n_frames, void* out, void*
     const int n_cells = ((p.F * p.tiles_x * p.tiles_y + 1) / 2) * p.n_ntiles;      // (N tile, double pixel tile)
     const int pairs = n_cells < n->sm_count / 2 ? n_cells : n->sm_count / 2;
     const int grid = 2 * pairs;
-    cudaError_t e = L.MT == 1 ? launch_conv<1>(L, p, grid, s)
-                  : L.MT == 2 ? launch_conv<2>(L, p, grid, s) : launch_conv<4>(L, p, grid, s);
+    cudaError_t e = L.MT == 1 ? launch_conv<1>(L, p, grid, s, n->smem_attr[0])
+                  : L.MT == 2 ? launch_conv<2>(L, p, grid, s, n->smem_attr[1])
+                              : launch_conv<4>(L, p, grid, s, n->smem_attr[2]);
     if (e != cudaSuccess) return cfail(n, UF_ERR_CUDA, "uf_cmn_conv_kernel (" + L.name + "): " + cudaGetErrorString(e));
     ++n->launches;
   }
@@ -855,6 +862,8 @@ int32_t uf_cmn_get_memory(uf_cmn* n, int32_t stage, int32_t block, void* out_hos
   if (!n || !out_host) return cfail(n, UF_ERR_INVALID_ARG, "uf_cmn_get_memory: null argument");
   if (stage < 0 || stage >= n->cfg.n_stages || block < 0 || block >= n->cfg.n_blocks)
     return cfail(n, UF_ERR_INVALID_ARG, "uf_cmn_get_memory: no such block");
+  { cudaError_t de = cudaSetDevice(n->cfg.device);
+    if (de != cudaSuccess) return cfail(n, UF_ERR_CUDA, std::string("cudaSetDevice: ") + cudaGetErrorString(de)); }
   const Buf& b = n->bufs[n->mem_buf[(size_t)stage * n->cfg.n_blocks + block]];
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   cudaError_t e = cudaMemcpyAsync(out_host, b.p + b.frame_elems() * (size_t)b.mem_slot, b.frame_elems() * sizeof(__nv_bfloat16),
@@ -870,6 +879,8 @@ int32_t uf_cmn_get_activation(uf_cmn* n, int32_t layer, void* out_host, int32_t 
   if (layer < 0 || layer >= (int32_t)n->layers.size() || n->layers[layer].out_buf < 0)
     return cfail(n, UF_ERR_INVALID_ARG, "uf_cmn_get_activation: no such layer (the last layer writes the caller's out)");
   if (n->last_frames < 1) return cfail(n, UF_ERR_STATE, "uf_cmn_get_activation: no step has run");
+  { cudaError_t de = cudaSetDevice(n->cfg.device);
+    if (de != cudaSuccess) return cfail(n, UF_ERR_CUDA, std::string("cudaSetDevice: ") + cudaGetErrorString(de)); }
   const Buf& b = n->bufs[n->layers[layer].out_buf];
   const int F = n->last_frames * b.fmul;
   cudaStream_t s = static_cast<cudaStream_t>(stream);

@@ -353,13 +353,12 @@ cudaError_t uf_launch_fused_append(uf_ctx* c, const UfView& v, const __nv_bfloat
   else if (v.H == 40 && R == 2 && a.parts == 10) { kern = uf_fused_append_kernel<D, 640, 1, 40, 2, 10>; small = 1; }
   else if (threads <= 256) { kern = uf_fused_append_kernel<D, 256, 3, 0, 0, 0>; small = 2; }
   else { kern = uf_fused_append_kernel<D, 1024, 1, 0, 0, 0>; small = 3; }
-  static size_t attr_set[4][64] = {};
-  int dev = 0;
-  cudaGetDevice(&dev);
-  if (smem > 48 * 1024 && dev < 64 && smem > attr_set[small][dev]) {
+  // the limit is a per-device attribute and a ctx lives on one device: the record is kept in the ctx (a ctx is
+  // not thread-safe, so neither is this)
+  if (smem > 48 * 1024 && smem > c->fused_smem_attr[small]) {
     cudaError_t e0 = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e0 != cudaSuccess) return e0;
-    attr_set[small][dev] = smem;
+    c->fused_smem_attr[small] = smem;
   }
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3((unsigned)(nb * kCluster));

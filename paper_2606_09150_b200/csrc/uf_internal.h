@@ -127,6 +127,7 @@ struct uf_ctx {
   const void* qbar_ptr = nullptr; // ... for this post-RoPE Q buffer and these strides
   int64_t qbar_ts = 0, qbar_hs = 0;
   bool skip_pool_q = false;       // set per select call: qbar is valid for the q passed in
+  bool reuse_pooled_q = true;     // uf_set_pooled_q_reuse: a select may skip its pooling pass (see uf.h)
   int32_t* sel_cnt = nullptr;     // [H][BPC]: entries of every sel_q row (paper-mask mode: rows differ in length)
   UfTiling til = {};              // paper-mask mode when til.enabled
   bool sel_paper = false;         // the stored selection came from uf_select_blocks_paper
@@ -156,6 +157,7 @@ struct uf_ctx {
   TmEntry tm_cache[kTmCache];
   int tm_cache_n = 0, tm_cache_next = 0;
   size_t score_smem_attr[4][3][4] = {};   // dynamic-smem limit already set on uf_score_topk_kernel<d, QG>
+  size_t fused_smem_attr[4] = {};         // ... on the four uf_fused_append_kernel instantiations (this ctx's device)
   std::string err;
 };
 

@@ -320,17 +320,17 @@ cudaError_t uf_launch_select(uf_ctx* c, const UfView& v, const __nv_bfloat16* q,
                              bool paper, int out_stride, cudaStream_t s) {
   const int nqb = uf_ceil_div(v.cur_ntok, v.B);
   const int NP = (v.BPC + 1) / 2;
-  // usage statistic (NEXT-3): this call counts into buffer `seq & 1`; the other buffer is zeroed for the next call
-  // (by the pair-merge kernel when it runs, else by a memset), so no extra launch sits on the hot path
-  c->usage_seq ^= 1;
-  unsigned long long* usage_cur = c->usage + (size_t)c->usage_seq * UF_MAXC;
-  unsigned long long* usage_next = c->usage + (size_t)(c->usage_seq ^ 1) * UF_MAXC;
-  c->usage_n = v.n_prior;
-  for (int i = 0; i < v.n_prior; ++i) c->usage_chunk[i] = v.prior_chunk[i];
+  // usage statistic (NEXT-3): this call counts into the buffer that is NOT current (the previous score kernel zeroed
+  // it) and zeroes the current one for the call after it, so no extra launch sits on the hot path.  The host record
+  // (which buffer is current, which chunks its counters refer to) is committed only once the score kernel has been
+  // enqueued: a call that fails before that leaves the previous selection's statistic intact and the spare buffer zero.
+  const int seq = c->usage_seq ^ 1;
+  unsigned long long* usage_cur = c->usage + (size_t)seq * UF_MAXC;
+  unsigned long long* usage_next = c->usage + (size_t)(seq ^ 1) * UF_MAXC;
   if (k_eff == 0 && !paper) {
-    c->usage_n = 0;
     cudaError_t e0 = cudaMemsetAsync(c->usage, 0, 2 * UF_MAXC * sizeof(unsigned long long), s);
     if (e0 != cudaSuccess) return e0;
+    c->usage_n = 0;                                    // both buffers are zero: either may be current
     // no candidates (chunk 0, or window 1): counts are zero, nothing to score
     if (cnt_out) {
       cudaError_t e = cudaMemsetAsync(cnt_out, 0, (size_t)v.H * nqb * sizeof(int32_t), s);
@@ -400,6 +400,9 @@ cudaError_t uf_launch_select(uf_ctx* c, const UfView& v, const __nv_bfloat16* q,
   c->launches += 1;
   e = cudaGetLastError();
   if (e != cudaSuccess) return e;
+  c->usage_seq = seq;
+  c->usage_n = v.n_prior;
+  for (int i = 0; i < v.n_prior; ++i) c->usage_chunk[i] = v.prior_chunk[i];
   if (want_pairs && !fuse_merge) {
     const int np_cur = (nqb + 1) / 2;
     const size_t msmem = (size_t)kMergeWarps * 2 * uf_ceil_div(v.n_cand, 32) * sizeof(uint32_t);

@@ -241,3 +241,42 @@ def test_causality_and_memory_dependence():
     zb[0] = cm.round_bf16(zb[0] + 1.0)
     a, b = cm.forward_parallel(za, cfg1, wt1), cm.forward_parallel(zb, cfg1, wt1)
     assert not np.array_equal(a[1], b[1]) and np.array_equal(a[2:], b[2:])
+
+
+def test_literal_variant_b_output_memory_differs_from_the_second_frame_on():
+    """VERDICT r2 item 8 / ADVICE r2: Alg. 2 variant B as printed stores the block OUTPUT.  With zero initial
+    memory the first frame cannot tell the two readings apart; every later frame can.  The output reading is a
+    recurrence: frame 0 still reaches frame 3 of a one-block network, where the input reading (one frame of reach per
+    block, pinned above) has forgotten it.  Both stay causal."""
+    c1 = wl.CmnWorkload("reach", 4, 3, (8,), 1, (1,), (1,), 5, 7, 2)
+    cfg, wt = _cfg(c1), _wt64(c1)
+    z = _frames64(c1, 0, 4)
+    a = cm.CausalMemStream(cfg, wt, memory="input").step(z)
+    b = cm.CausalMemStream(cfg, wt, memory="output").step(z)
+    assert np.array_equal(a, cm.forward_parallel(z, cfg, wt))
+    assert np.array_equal(a[0], b[0])
+    for t in (1, 2, 3):
+        assert not np.array_equal(a[t], b[t]), t
+    # the second frame of the output reading, restated by hand from Eq. 2: memory = the first frame's block output
+    h0 = cm.round_bf16(cm.conv3x3(z[0:1], wt["in"], wt["in.b"]))
+    h1 = cm.round_bf16(cm.conv3x3(z[1:2], wt["in"], wt["in.b"]))
+    out0 = cm.mem_block(h0, np.zeros_like(h0), wt, "s0.b0.")
+    out1 = cm.mem_block(h1, out0, wt, "s0.b0.")
+    tail = cm.round_bf16(cm.conv3x3(cm._stage_tail(out1, cfg, 0, wt), wt["out"], wt["out.b"]))
+    assert np.array_equal(tail[0], b[1])
+    # chunking does not matter (state is carried), causality holds, and the reach is unbounded
+    st = cm.CausalMemStream(cfg, wt, memory="output")
+    assert np.array_equal(np.concatenate([st.step(z[:1]), st.step(z[1:3]), st.step(z[3:])]), b)
+    z2 = z.copy()
+    z2[0] = cm.round_bf16(z2[0] + 1.0)
+    b2 = cm.CausalMemStream(cfg, wt, memory="output").step(z2)
+    assert not np.array_equal(b2[3], b[3])                     # frame 0 reaches frame 3 through the recurrence
+    z3 = z.copy()
+    z3[2] = cm.round_bf16(z3[2] + 1.0)
+    b3 = cm.CausalMemStream(cfg, wt, memory="output").step(z3)
+    assert np.array_equal(b3[:2], b[:2]) and not np.array_equal(b3[2], b[2])
+    # how far apart the two readings are on seeded weights (reported, not asserted beyond "not small")
+    rel = np.sqrt(np.mean((a[1:] - b[1:]) ** 2) / np.mean(a[1:] ** 2))
+    assert rel > 1e-3, rel
+    with pytest.raises(ValueError):
+        cm.CausalMemStream(cfg, wt, memory="both")

@@ -158,3 +158,26 @@ def test_argument_errors():
         assert e.value.code == uf.binding.UF_ERR_INVALID_ARG
     finally:
         uf.uf_cmn_destroy(net)
+
+
+def test_cmn_step_with_another_device_current():
+    """every uf_cmn_* call makes the handle's device current itself, and the dynamic-shared-memory limit of
+    the convolution kernel is raised per handle (it is a per-device attribute).  Needs two GPUs: a handle on cuda:1 is
+    set up and stepped while cuda:0 is current and must give the bits of a handle on cuda:0."""
+    import torch
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two CUDA devices")
+    c = wl.CMN_CONFIGS["cmn_tiny"]
+    zb = wl.cmn_frames(c, 0, 2)
+    outs = []
+    for dev in (0, 1):
+        torch.cuda.set_device(0)
+        net = hz.CmnCuda(c, frames_max=2, device=dev)
+        try:
+            torch.cuda.set_device(0)
+            outs.append(net.step(zb))
+            torch.cuda.set_device(0)
+            net.memory(0, 0)                              # a getter with the other device current
+        finally:
+            net.close()
+    assert np.array_equal(outs[0], outs[1])

@@ -95,3 +95,78 @@ def test_fused_full_size_1k():
         _check_cache(cu, orc, w)
     finally:
         cu.close()
+
+
+def test_fused_in_place_overlap_and_rewritten_q_out():
+    """(a) q_out == q_in (same strides) gives the bits of the out-of-place call, also inside a fused
+    [n, 3, H, d] tensor; (b) any other overlap of q_out with an input is refused and nothing is appended; (c) a q_out
+    rewritten between the fused append and the select is recognised by address only: with the shortcut on the selection
+    is the one for the ORIGINAL q_out (documented), with uf_set_pooled_q_reuse(ctx, 0) it follows the q argument."""
+    import torch
+    import paper_2606_09150_b200 as uf
+    w = wl.scaled(wl.CONFIGS["1k"], "fz_alias", n_heads=2, frames_per_chunk=2, grid_h=16, grid_w=24, capacity_chunks=3)
+    n, H, d = w.chunk_tokens, 2, 128
+    rs = None
+    outs = {}
+    for mode in ("separate", "in_place", "in_place_fused"):
+        cu = hz.CudaStream(w)
+        rs = rs or hz.RopeState(w, 64, cu.dev)
+        try:
+            for c in range(2):
+                Qb, Kb, Vb = wl.make_chunk(w, c)
+                if mode == "in_place_fused":
+                    qkv = cu.to_dev(np.ascontiguousarray(np.stack([Qb, Kb, Vb], axis=1)))
+                    q, k, v, ts = qkv[:, 0], qkv[:, 1], qkv[:, 2], 3 * H * d
+                else:
+                    q, k, v, ts = cu.to_dev(Qb), cu.to_dev(Kb), cu.to_dev(Vb), H * d
+                q_out = torch.empty((n, H, d), dtype=torch.bfloat16, device=cu.dev) if mode == "separate" else q
+                ots = H * d if mode == "separate" else ts
+                uf.uf_qkv_rope_append(cu.ctx, q, k, v, q_out, n, ts, d, ots, d, rs.d_cos, rs.d_sin, rs.d_gq, rs.d_gk,
+                                      rs.max_pos, 2 * c, w.grid_h, w.grid_w, wl.ROPE_AXIS_DIMS, 1e-6, 0, cu.stream)
+                if mode == "in_place_fused":                      # the K and V slices are inputs only
+                    torch.cuda.synchronize(cu.dev)
+                    assert np.array_equal(qkv[:, 1].contiguous().view(torch.int16).cpu().numpy().view(np.uint16), Kb)
+                    assert np.array_equal(qkv[:, 2].contiguous().view(torch.int16).cpu().numpy().view(np.uint16), Vb)
+            _, k_eff = uf.uf_query_topk(cu.ctx, -1, 50)
+            idx = torch.full((H, w.bpc, k_eff), -1, dtype=torch.int32, device=cu.dev)
+            uf.uf_select_blocks(cu.ctx, q_out, n, ots, d, -1, 50, idx, None, cu.stream)
+            torch.cuda.synchronize(cu.dev)
+            outs[mode] = (q_out.contiguous().view(torch.int16).cpu().numpy().view(np.uint16), idx.cpu().numpy())
+            if mode != "separate":
+                continue
+            # (c) rewrite q_out: the other chunk's raw Q, as if the caller had reused the buffer
+            other = cu.to_dev(wl.make_chunk(w, 7)[0])
+            fresh = other.clone()                              # same values at another address: always pooled
+            idx_fresh = torch.full_like(idx, -1)
+            uf.uf_select_blocks(cu.ctx, fresh, n, H * d, d, -1, 50, idx_fresh, None, cu.stream)
+            q_out.copy_(other)
+            idx_stale, idx_off = torch.full_like(idx, -1), torch.full_like(idx, -1)
+            l0 = uf.uf_ctx_launch_count(cu.ctx)
+            uf.uf_select_blocks(cu.ctx, q_out, n, H * d, d, -1, 50, idx_stale, None, cu.stream)
+            assert uf.uf_ctx_launch_count(cu.ctx) - l0 == 1                 # shortcut taken: no pooling pass
+            uf.uf_set_pooled_q_reuse(cu.ctx, False)
+            l0 = uf.uf_ctx_launch_count(cu.ctx)
+            uf.uf_select_blocks(cu.ctx, q_out, n, H * d, d, -1, 50, idx_off, None, cu.stream)
+            assert uf.uf_ctx_launch_count(cu.ctx) - l0 == 2                 # pooled again
+            torch.cuda.synchronize(cu.dev)
+            assert np.array_equal(idx_stale.cpu().numpy(), outs["separate"][1])      # the documented hazard
+            assert np.array_equal(idx_off.cpu().numpy(), idx_fresh.cpu().numpy())
+            assert not np.array_equal(idx_fresh.cpu().numpy(), outs["separate"][1])
+            # (b) overlaps that are refused; the ctx stays where it was
+            before = uf.uf_get_slot_map(cu.ctx, w.capacity_chunks)
+            flat = torch.zeros(4 * n * H * d, dtype=torch.bfloat16, device=cu.dev)
+            view = lambda off: flat[off:off + n * H * d].view(n, H, d)
+            a, b, cbuf = view(0), view(n * H * d), view(2 * n * H * d)
+            for qo, qi, ki, vi in ((a, b, a, cbuf),                                  # q_out == k_in
+                                   (view(H * d), a, b + 0, cbuf),                    # q_out = q_in shifted by one row
+                                   (view(n * H * d - 8), a, view(2 * n * H * d), view(3 * n * H * d))):   # tail of q_in ... head of k_in
+                with pytest.raises(uf.UFError) as ei:
+                    uf.uf_qkv_rope_append(cu.ctx, qi, ki, vi, qo, n, H * d, d, H * d, d, rs.d_cos, rs.d_sin, rs.d_gq,
+                                          rs.d_gk, rs.max_pos, 4, w.grid_h, w.grid_w, wl.ROPE_AXIS_DIMS, 1e-6, 0, cu.stream)
+                assert ei.value.code == uf.binding.UF_ERR_INVALID_ARG
+            assert uf.uf_get_slot_map(cu.ctx, w.capacity_chunks) == before
+        finally:
+            cu.close()
+    for mode in ("in_place", "in_place_fused"):
+        assert np.array_equal(outs[mode][0], outs["separate"][0]), f"{mode}: post-RoPE Q differs from the out-of-place call"
+        assert np.array_equal(outs[mode][1], outs["separate"][1]), f"{mode}: selection differs"
