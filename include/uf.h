@@ -205,7 +205,8 @@ int32_t uf_untile_tokens(uf_ctx* ctx, const void* tiled, void* raster,
  *            row y, the last dim_w/2 its column x; the cos / sin values come from the caller's tables (model state)
  *   round    to bf16 (nearest even).  Everything before it is IEEE fp32, each operation rounded once, no fused
  *            multiply-add, in the stated order (the sum of squares and the reciprocal square root run in fp64 and are
- *            rounded to fp32 once), so cache bytes and block indices are a fixed function of the input bits
+ *            rounded to fp32 once), so cache bytes and block indices are a fixed function of the input bits; against
+ *            the fp64 definition (one rounding) the result is equal or adjacent in bf16 (within one ulp)
  *   write    post-RoPE Q -> q_out; post-RoPE K and V -> the cache slot, exactly as uf_kv_append (same eviction policy,
  *            sink copy, zero pad rows); block-mean pooled K and pooled Q -> the ctx.
  * A following uf_select_blocks / uf_select_blocks_paper called with q == q_out (same strides) skips its pooling

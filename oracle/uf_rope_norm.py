@@ -17,19 +17,23 @@ R-37 ... R-40 in DESIGN.md):
             (a + ib) -> (a + ib) * exp(i * pos * theta^(-2i/D)).
         Positions: t counts latent frames from the start of the stream (chunk c starts at t0 = c * F), y, x are the
         token-grid coordinates; tokens arrive in raster (t, y, x) order.
-  R-39  The cos / sin tables are MODEL STATE (the architecture precomputes them once, in fp32), i.e. an input of the
-        step like the norm weights: `apply` takes them as arguments.  `rope_table` is the definition they must
-        satisfy (to fp32 rounding).
-  R-40  Arithmetic and rounding.  Inputs are bf16; the result is rounded to bf16 because the cache and the attention
-        kernel hold bf16.  That rounding decides cache bytes and, through pooling, block indices, so both sides take
-        it in the SAME precision, the kernel's: fp32 with every operation rounded once (IEEE, no fused multiply-add),
-        in this order (fl = round to fp32):
-            ss = sum_j x_j^2   in fp64 (each x_j^2 is exact; the sum is exact, hence order-free, as long as the
-                               squares of one token span fewer than 2^37 — else its last bit may depend on the order),
-            r  = fl(1 / sqrt(ss / C + eps))          (the fp64 operations /, +, sqrt, / rounded once each, then fl),
-            u_j = fl(fl(x_j * r) * g_j),
-            out_2i = fl(fl(u_2i * cos) - fl(u_2i+1 * sin));   out_2i+1 = fl(fl(u_2i * sin) + fl(u_2i+1 * cos)),
-            result = bf16(out)   round to nearest even (IEEE, subnormals kept).
+  R-39  The cos / sin tables are MODEL STATE (the architecture precomputes them once and stores them in fp32), i.e. an
+        input of the step like the norm weights: `apply` takes them as arguments and uses the values it is given
+        (fp32 table entries are exact in fp64).  `rope_table` is the definition they must satisfy.
+  R-40  Arithmetic and rounding.  Inputs are bf16; the result is rounded to bf16 (round to nearest even; results
+        whose magnitude is below the smallest normal bf16, 2^-126, become signed zero) because the cache and the
+        attention kernel hold bf16.  This file is the DEFINITION: fp64 throughout (BASELINE.json north_star: "NumPy in
+        fp64"), ONE rounding to bf16 at the end, every operation before it rounded once in fp64, in this order (no
+        fused multiply-add).  The CUDA kernel computes in fp32 and is compared with this file within one bf16 ulp
+        (tests/test_gpu_fused_append.py); what follows the rounding (pooling, indices, attention) is then checked
+        bit-exactly by feeding the kernel's OWN bf16 bits to oracle/uf_oracle.py (teacher forcing), because a
+        last-bit difference in a cached K legitimately moves a pooled mean.  Nothing in this file is taken from the
+        kernel's arithmetic (history: 2725cb1 wrote it, ce6d265 replaced it by a float32 mirror of the kernel, round 3
+        restored it; the mirror lives on as tests/fused_fp32_model.py, a model of the kernel, not an oracle):
+            ss = sum_j x_j^2  (each x_j^2 is exact in fp64; the sum is exact, hence order-free, as long as the
+                               squares of one token span fewer than 2^37),
+            m = ss / C;  r = 1 / sqrt(m + eps);  u_j = (x_j * r) * g_j;
+            out_2i = u_2i * cos - u_2i+1 * sin;   out_2i+1 = u_2i * sin + u_2i+1 * cos.
 """
 from __future__ import annotations
 
@@ -66,17 +70,23 @@ def raster_positions(n_tokens: int, grid_h: int, grid_w: int, t0: int):
 
 
 def round_to_bf16(y: np.ndarray) -> np.ndarray:
-    """fp32 -> nearest bf16 (ties to even), uint16 bit patterns (R-40).  On the fp32 bits: the upper 16 bits, plus one
-    when the lower 16 are above half, or exactly half with an odd upper part; the carry may run into the exponent,
-    which is the right result (also for subnormals).  No NaN / inf in the step's domain."""
-    y = np.ascontiguousarray(y, dtype=np.float32)
-    u = y.view(np.uint32)
-    upper = u >> np.uint32(16)
-    lower = u & np.uint32(0xFFFF)
-    up = (lower > np.uint32(0x8000)) | ((lower == np.uint32(0x8000)) & ((upper & np.uint32(1)) == np.uint32(1)))
-    out = upper + up.astype(np.uint32)
-    assert not ((out & np.uint32(0x7F80)) == np.uint32(0x7F80)).any(), "inf / NaN: outside the step's domain"
-    return out.astype(np.uint16)
+    """fp64 -> nearest bf16 (ties to even), returned as uint16 bit patterns; |y| < 2^-126 -> signed zero (R-40).
+    Done on the fp64 bits: keep sign, re-bias the exponent (1023 -> 127), keep the top 7 mantissa bits and round on
+    the 45 bits below them."""
+    y = np.ascontiguousarray(y, dtype=np.float64)
+    u = y.view(np.uint64)
+    sign = ((u >> np.uint64(63)) & np.uint64(1)).astype(np.uint64)
+    mag = u & np.uint64(0x7FFFFFFFFFFFFFFF)
+    keep = mag >> np.uint64(45)                                   # exponent (11 bits) + top 7 mantissa bits
+    rest = mag & np.uint64((1 << 45) - 1)
+    half = np.uint64(1 << 44)
+    up = (rest > half) | ((rest == half) & ((keep & np.uint64(1)) == np.uint64(1)))
+    keep = keep + up.astype(np.uint64)                            # a carry into the exponent is the right result
+    bias = np.uint64((1023 - 127) << 7)
+    small = keep < bias + np.uint64(1 << 7)                       # below 2^-126 after rounding: flush
+    out = np.where(small, np.uint64(0), keep - bias)
+    assert not (out >= np.uint64(0x7F80)).any(), "overflow to inf / NaN: outside the step's domain"
+    return ((sign << np.uint64(15)) | out).astype(np.uint16)
 
 
 def bf16_bits_to_f64(b: np.ndarray) -> np.ndarray:
@@ -84,26 +94,24 @@ def bf16_bits_to_f64(b: np.ndarray) -> np.ndarray:
 
 
 def rms_factor(X: np.ndarray, eps: float = EPS) -> np.ndarray:
-    """r = fl32(1 / sqrt(mean over ALL channels of the token of x^2 + eps)), the inner part in fp64 (R-37, R-40).
-    X fp64 [n, H, d] -> float32 [n]"""
+    """r = 1 / sqrt(mean over ALL channels of the token of x^2 + eps) (R-37).  X fp64 [n, H, d] -> [n]"""
     n = X.shape[0]
     C = X.shape[1] * X.shape[2]
     ss = (X * X).reshape(n, C).sum(axis=1)
-    return (1.0 / np.sqrt(ss / float(C) + eps)).astype(np.float32)
+    return 1.0 / np.sqrt(ss / float(C) + eps)
 
 
-def apply(X: np.ndarray, g: np.ndarray, cos: np.ndarray, sin: np.ndarray, pos, dims=AXIS_DIMS, eps: float = EPS):
-    """QK-norm + 3-D RoPE of one projection output.  X fp64 [n, H, d] (exact bf16 values), g float32 [H*d], cos / sin
-    float32 [max_pos, d/2], pos = (t, y, x) integer arrays [n].  Returns uint16 bf16 bits [n, H, d].  Every product and
-    sum below is ONE float32 NumPy operation, i.e. rounded once, in the order R-40 states."""
+def apply_unrounded(X: np.ndarray, g: np.ndarray, cos: np.ndarray, sin: np.ndarray, pos, dims=AXIS_DIMS,
+                    eps: float = EPS) -> np.ndarray:
+    """QK-norm + 3-D RoPE of one projection output, BEFORE the rounding to bf16.  X fp64 [n, H, d] (exact bf16 values),
+    g [H*d], cos / sin [max_pos, d/2] (any float dtype: used as fp64), pos = (t, y, x) integer arrays [n].
+    Returns fp64 [n, H, d]."""
     X = np.asarray(X, dtype=np.float64)
+    cos, sin = np.asarray(cos, dtype=np.float64), np.asarray(sin, dtype=np.float64)
     n, H, d = X.shape
-    g = np.asarray(g)
-    assert sum(dims) == d and g.shape == (H * d,) and g.dtype == np.float32
-    assert cos.dtype == np.float32 and sin.dtype == np.float32
-    r = rms_factor(X, eps)                                        # float32 [n]
-    x32 = X.astype(np.float32)                                    # exact: bf16 values
-    U = (x32 * r[:, None, None]) * g.reshape(1, H, d)             # fl(fl(x r) g)
+    assert sum(dims) == d and g.shape == (H * d,)
+    r = rms_factor(X, eps)
+    U = (X * r[:, None, None]) * np.asarray(g, dtype=np.float64).reshape(1, H, d)
     ax = pair_axis(dims)                                          # [d/2]
     P = np.stack(pos, axis=1)[:, ax]                              # [n, d/2] position that drives each pair
     col = np.arange(d // 2)[None, :]
@@ -113,5 +121,9 @@ def apply(X: np.ndarray, g: np.ndarray, cos: np.ndarray, sin: np.ndarray, pos, d
     out = np.empty_like(U)
     out[:, :, 0::2] = ue * c - uo * s
     out[:, :, 1::2] = ue * s + uo * c
-    assert out.dtype == np.float32
-    return round_to_bf16(out)
+    return out
+
+
+def apply(X: np.ndarray, g: np.ndarray, cos: np.ndarray, sin: np.ndarray, pos, dims=AXIS_DIMS, eps: float = EPS):
+    """`apply_unrounded` followed by the ONE rounding to bf16 (R-40).  Returns uint16 bf16 bits [n, H, d]."""
+    return round_to_bf16(apply_unrounded(X, g, cos, sin, pos, dims, eps))

@@ -11,7 +11,9 @@
 // contraction (__fmul_rn / __fadd_rn / __fsub_rn), in the order
 //   ss = sum x^2 (fp64, exact);  r = fl32(1 / sqrt(ss / C + eps)) (fp64 ops);  u = fl(fl(x r) g);
 //   out_e = fl(fl(u_e cos) - fl(u_o sin));  out_o = fl(fl(u_e sin) + fl(u_o cos));  result = bf16_rne(out)
-// and the oracle (oracle/uf_rope_norm.py) does the same in NumPy float32.  The pooled sums add the ROUNDED values in
+// (tests/fused_fp32_model.py restates this order in NumPy float32 for a reproducibility test; the ORACLE,
+// oracle/uf_rope_norm.py, is the fp64 definition with one rounding, and the kernel is compared with it within one bf16
+// ulp).  The pooled sums add the ROUNDED values in
 // fp64 (exact, order-free, as in uf_append.cu).
 //
 // Grid: a CLUSTER of 8 CTAs per key block of the chunk; each CTA owns B/8 consecutive rows of the block and ALL heads

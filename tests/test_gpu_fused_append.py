@@ -1,6 +1,9 @@
-"""GPU parity of the fused QK-norm + 3-D RoPE + append + pooling step (NEXT-2, uf_qkv_rope_append) against
-oracle/uf_rope_norm.py followed by the ordinary oracle: post-RoPE Q bits, cache bytes, pooled K and every selected block
-id bit-exact; attention outputs within BASELINE.json's 2e-2 / 2e-3."""
+"""GPU parity of the fused QK-norm + 3-D RoPE + append + pooling step (NEXT-2, uf_qkv_rope_append) against the fp64
+oracle oracle/uf_rope_norm.py: post-RoPE Q and cached K within ONE bf16 ulp of the fp64 definition (>= 99 % bit-equal),
+cached V the input bits; then, teacher-forced on the kernel's own bf16 bits, the ordinary oracle: slot maps, pooled K and
+every selected block id bit-exact, attention outputs within BASELINE.json's 2e-2 / 2e-3 (uf_harness.oracle_fused_step).
+A separate test compares the kernel with a float32 model of itself (tests/fused_fp32_model.py): that one shows the bits
+are reproducible, not that they are right."""
 import numpy as np
 import pytest
 
@@ -21,9 +24,7 @@ def _stream(w, n_chunks, lens=None, windows=None, fused_qkv=False, **sel):
             Qb, Kb, Vb = wl.make_chunk(w, c, n_tokens=n)
             t0 = c * w.frames_per_chunk
             got = hz.fused_step(cu, rs, Qb, Kb, Vb, t0, window=win, fused_qkv=fused_qkv, **sel)
-            ref = hz.oracle_fused_step(orc, rs, w, Qb, Kb, Vb, t0, window=win, **sel)
-            assert np.array_equal(got["q_out_bits"], ref["q_out_bits"]), \
-                f"chunk {c}: post-RoPE Q differs in {(got['q_out_bits'] != ref['q_out_bits']).sum()} elements"
+            ref = hz.oracle_fused_step(orc, rs, w, Qb, Kb, Vb, t0, got, cu, c, window=win, **sel)
             hz.compare_step(got, ref, f"[{w.name} fused chunk {c}]")
             # fused append (1) + score / top-k / pair merge (1 kernel, no pooling pass) + attention (2); chunk 0 has no candidates
             assert got["launches"] == (4 if got["k_eff"] > 0 else 3), got["launches"]
@@ -78,8 +79,9 @@ def test_fused_error_codes():
 
 
 def test_fused_full_size_1k():
-    """BASELINE.json configs[1] shapes through the fused entry: all 2 x 37.6 M post-RoPE Q elements, all selected block
-    ids, sampled cache blocks and pooled K bit-exact; attention on sampled (head, query block) pairs."""
+    """BASELINE.json configs[1] shapes through the fused entry: all 2 x 50.1 M post-RoPE Q elements and all cached K
+    within one bf16 ulp of the fp64 oracle; all selected block ids, sampled pooled K bit-exact against the oracle fed with
+    the kernel's bits; attention on sampled (head, query block) pairs."""
     w = wl.CONFIGS["1k"]
     cu, orc = hz.CudaStream(w), hz.make_oracle(w)
     rs = hz.RopeState(w, 128, cu.dev)
@@ -87,11 +89,11 @@ def test_fused_full_size_1k():
         for c in range(2):
             Qb, Kb, Vb = wl.make_chunk(w, c)
             got = hz.fused_step(cu, rs, Qb, Kb, Vb, 3 * c, topk_percent=w.topk_percent)
-            ref = hz.oracle_fused_step(orc, rs, w, Qb, Kb, Vb, 3 * c, topk_percent=w.topk_percent,
+            ref = hz.oracle_fused_step(orc, rs, w, Qb, Kb, Vb, 3 * c, got, cu, c, topk_percent=w.topk_percent,
                                        heads=[0, 5, 11], qblocks=[0, 1, 77, 190, 191], attn=(c == 1))
-            assert np.array_equal(got["q_out_bits"], ref["q_out_bits"])
             r = hz.compare_step(got, ref, f"[1k fused chunk {c}]")
-        print(f"1k fused: sampled O max-abs {r[0]:.3e} mean-abs {r[1]:.3e}, min top-k gap {ref['min_gap']:.3e}")
+        print(f"1k fused: Q / K bit-equal to the fp64 oracle's rounding {ref['eq_q']:.5f} / {ref['eq_k']:.5f}, sampled O "
+              f"max-abs {r[0]:.3e} mean-abs {r[1]:.3e}, min top-k gap {ref['min_gap']:.3e}")
         _check_cache(cu, orc, w)
     finally:
         cu.close()
@@ -170,3 +172,22 @@ def test_fused_in_place_overlap_and_rewritten_q_out():
     for mode in ("in_place", "in_place_fused"):
         assert np.array_equal(outs[mode][0], outs["separate"][0]), f"{mode}: post-RoPE Q differs from the out-of-place call"
         assert np.array_equal(outs[mode][1], outs["separate"][1]), f"{mode}: selection differs"
+
+
+def test_fused_bits_equal_the_float32_model_of_the_kernel():
+    """Reproducibility, not correctness: the kernel's post-RoPE Q bits equal tests/fused_fp32_model.py (a NumPy
+    float32 restatement of the kernel's own operation order) bit for bit, so cache bytes and block indices are a fixed
+    function of the input bits on any device."""
+    import fused_fp32_model as fm
+    w = wl.scaled(wl.CONFIGS["1k"], "fz_model", n_heads=2, frames_per_chunk=2, grid_h=13, grid_w=21, capacity_chunks=2)
+    cu = hz.CudaStream(w)
+    rs = hz.RopeState(w, 64, cu.dev)
+    try:
+        Qb, Kb, Vb = wl.make_chunk(w, 0)
+        got = hz.fused_step(cu, rs, Qb, Kb, Vb, 5, topk_count=0)
+        pos = fm.raster_positions(Qb.shape[0], w.grid_h, w.grid_w, 5)
+        assert np.array_equal(got["q_out_bits"], fm.apply(hz.bits_to_f64(Qb), rs.gq, rs.cos, rs.sin, pos))
+        k_gpu, _ = hz.cache_chunk_bits(cu, 0, Qb.shape[0])
+        assert np.array_equal(k_gpu, fm.apply(hz.bits_to_f64(Kb), rs.gk, rs.cos, rs.sin, pos))
+    finally:
+        cu.close()
