@@ -387,6 +387,7 @@ int32_t uf_select_blocks(uf_ctx* c, const void* q, int32_t n_tokens, int64_t tok
   if (k > c->kcap) return fail(c, UF_ERR_CAPACITY, "uf_select_blocks: k exceeds workspace (internal)");
   UF_CUDA(c, cudaSetDevice(c->cfg.device));
   c->skip_pool_q = c->reuse_pooled_q && (c->qbar_chunk == v.cur_chunk && c->qbar_ptr == q && c->qbar_ts == tok_stride && c->qbar_hs == head_stride);
+  if (!c->skip_pool_q) c->qbar_chunk = -1;      // this call pools q into the ctx's table: the fused call's pooled Q is gone
   cudaError_t e = uf_launch_select(c, v, (const __nv_bfloat16*)q, tok_stride, head_stride, k, idx_out, cnt_out,
                                    false, k, (cudaStream_t)stream);
   if (e != cudaSuccess) return fail_cuda(c, e, "uf_select_blocks kernel launch");
@@ -465,6 +466,7 @@ int32_t uf_select_blocks_paper(uf_ctx* c, const void* q, int32_t n_tokens, int64
     return fail(c, UF_ERR_CAPACITY, "uf_select_blocks_paper: idx_stride < min(k + 1, N_blocks)");
   UF_CUDA(c, cudaSetDevice(c->cfg.device));
   c->skip_pool_q = c->reuse_pooled_q && (c->qbar_chunk == v.cur_chunk && c->qbar_ptr == q && c->qbar_ts == tok_stride && c->qbar_hs == head_stride);
+  if (!c->skip_pool_q) c->qbar_chunk = -1;      // this call pools q into the ctx's table: the fused call's pooled Q is gone
   cudaError_t e = uf_launch_select(c, v, (const __nv_bfloat16*)q, tok_stride, head_stride, k, idx_out, cnt_out,
                                    true, idx_stride, (cudaStream_t)stream);
   if (e != cudaSuccess) return fail_cuda(c, e, "uf_select_blocks_paper kernel launch");

@@ -135,6 +135,27 @@ def test_decoder_crop_full_size():
     print("cmn_decoder_crop parity:", st)
 
 
+def test_decoder_full_1k_sampled_windows():
+    """P:347 at the size bench.py times as cmn_decoder_1k: the whole 136 x 240 HR latent, a chunk of 3 latent frames ->
+    12 frames of 1088 x 1920 x 3 (the decoder had only been run on a quarter-area, one-frame crop).  The
+    tensors are too large for the NumPy oracle as a whole (2.7 TFLOP per frame), so every layer is checked on windows:
+    the oracle's layer function on crops of the GPU's own input activations against the GPU's output, within one bf16
+    ulp and >= 99 % bit-equal per window (two opposite corners + seeded random frames and positions per layer)."""
+    c = wl.CMN_CONFIGS["cmn_decoder_1k"]
+    cm, cfg, wt = hz.cmn_oracle(c)
+    zb = wl.cmn_frames(c, 0, 3)
+    net = hz.CmnCuda(c, frames_max=3)
+    try:
+        print("cmn_decoder_1k ctx bytes:", net.uf.uf_cmn_device_bytes(net.net))
+        out_bits = net.step_bits(zb)
+        assert out_bits.shape == (12, 1088, 1920, 3)
+        assert np.isfinite(hz.bits_to_f64(out_bits[::4, ::16, ::16])).all()
+        eq = hz.cmn_layerwise_sampled(net, cm, cfg, wt, zb, out_bits, n_windows=5, win=20, seed=7, where="[cmn_decoder_1k]")
+        print(f"cmn_decoder_1k: every sampled window of every layer within one bf16 ulp, >= {eq:.4f} bit-equal")
+    finally:
+        net.close()
+
+
 def test_argument_errors():
     import paper_2606_09150_b200 as uf
     with pytest.raises(uf.UFError) as e:

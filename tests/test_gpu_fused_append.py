@@ -138,11 +138,9 @@ def test_fused_in_place_overlap_and_rewritten_q_out():
                 continue
             # (c) rewrite q_out: the other chunk's raw Q, as if the caller had reused the buffer
             other = cu.to_dev(wl.make_chunk(w, 7)[0])
-            fresh = other.clone()                              # same values at another address: always pooled
-            idx_fresh = torch.full_like(idx, -1)
-            uf.uf_select_blocks(cu.ctx, fresh, n, H * d, d, -1, 50, idx_fresh, None, cu.stream)
+            backup = q_out.clone()
             q_out.copy_(other)
-            idx_stale, idx_off = torch.full_like(idx, -1), torch.full_like(idx, -1)
+            idx_stale, idx_off, idx_fresh, idx_back = (torch.full_like(idx, -1) for _ in range(4))
             l0 = uf.uf_ctx_launch_count(cu.ctx)
             uf.uf_select_blocks(cu.ctx, q_out, n, H * d, d, -1, 50, idx_stale, None, cu.stream)
             assert uf.uf_ctx_launch_count(cu.ctx) - l0 == 1                 # shortcut taken: no pooling pass
@@ -150,10 +148,20 @@ def test_fused_in_place_overlap_and_rewritten_q_out():
             l0 = uf.uf_ctx_launch_count(cu.ctx)
             uf.uf_select_blocks(cu.ctx, q_out, n, H * d, d, -1, 50, idx_off, None, cu.stream)
             assert uf.uf_ctx_launch_count(cu.ctx) - l0 == 2                 # pooled again
+            fresh = other.clone()                              # same values at another address: always pooled
+            uf.uf_select_blocks(cu.ctx, fresh, n, H * d, d, -1, 50, idx_fresh, None, cu.stream)
+            # a select that pooled another Q has overwritten the ctx's pooled-Q table: with the shortcut back on, the
+            # original q_out must be pooled again, not matched by address against a table that no longer holds it
+            uf.uf_set_pooled_q_reuse(cu.ctx, True)
+            q_out.copy_(backup)
+            l0 = uf.uf_ctx_launch_count(cu.ctx)
+            uf.uf_select_blocks(cu.ctx, q_out, n, H * d, d, -1, 50, idx_back, None, cu.stream)
+            assert uf.uf_ctx_launch_count(cu.ctx) - l0 == 2
             torch.cuda.synchronize(cu.dev)
             assert np.array_equal(idx_stale.cpu().numpy(), outs["separate"][1])      # the documented hazard
             assert np.array_equal(idx_off.cpu().numpy(), idx_fresh.cpu().numpy())
             assert not np.array_equal(idx_fresh.cpu().numpy(), outs["separate"][1])
+            assert np.array_equal(idx_back.cpu().numpy(), outs["separate"][1])
             # (b) overlaps that are refused; the ctx stays where it was
             before = uf.uf_get_slot_map(cu.ctx, w.capacity_chunks)
             flat = torch.zeros(4 * n * H * d, dtype=torch.bfloat16, device=cu.dev)

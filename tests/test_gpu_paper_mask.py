@@ -134,9 +134,10 @@ def test_paper_mode_error_codes():
         uf.uf_ctx_destroy(ctx)
 
 
-@pytest.mark.parametrize("name", ["1k_paper", "2k_paper"])
+@pytest.mark.parametrize("name", ["1k_paper", "2k_paper", "1k_paper_native"])
 def test_full_size_paper_step(name):
-    """BASELINE.json configs[1] / configs[2] under the paper's mask at full size: ALL kept block ids and counts
+    """BASELINE.json configs[1] / configs[2] under the paper's mask at full size, and the paper's own chunking
+    (1k_paper_native: 2 latent frames of 60 x 104 tokens, 3 cached chunks, P:148 / P:343): ALL kept block ids and counts
     bit-exact; attention against the oracle on every row of two whole heads plus sampled tiles of two more; every
     row of every head against the CUDA-core kernel."""
     import torch

@@ -514,3 +514,42 @@ def test_tensor_map_cache_eviction_between_q_and_o_lookups():
             assert torch.equal(os_[i].float(), ref), f"call {i} differs from the first result"
     finally:
         cu.close()
+
+
+def test_block_column_beyond_the_exact_sum_range():
+    """ADVICE r1 item 4 / VERDICT r2 item 9: include/uf.h promises bit-exact indices "as long as the block sums are exact
+    in fp64", i.e. while one (block, head, channel) column spans fewer than 2^38 between its largest magnitude and its
+    smallest non-zero ulp; beyond that "the summation order may change the last bit of a pooled mean".  This feeds a
+    column that spans 2^74 (one 2^60 among values with ulps of 2^-14) and checks exactly that promise: the exact mean
+    (rational arithmetic) is bracketed by the GPU's and by the oracle's fp64 means within one ulp each — nothing worse
+    — every OTHER pooled value stays bit-exact, and the selection, whose top-k gaps are far above one ulp here, is
+    unchanged."""
+    from fractions import Fraction
+    w = wl.scaled(wl.CONFIGS["1k"], "widerange", n_heads=1, frames_per_chunk=1, grid_h=16, grid_w=32, capacity_chunks=2,
+                  sink_blocks=0)
+    assert w.chunk_tokens == 512 and w.bpc == 4
+    chunks = [list(wl.make_chunk(w, c)) for c in range(2)]
+    Kb = chunks[0][1]
+    blk, ch = 2, 5
+    Kb[blk * 128 + 17, 0, ch] = wl.f32_to_bf16_bits(np.array([2.0 ** 60], dtype=np.float32))[0]
+    col = hz.bits_to_f64(Kb[blk * 128:(blk + 1) * 128, 0, ch])
+    nz = np.abs(col[col != 0])
+    ulps = np.ldexp(1.0, np.frexp(nz)[1] - 8)                 # ulp of a bf16 value with exponent e (8 significant bits)
+    assert nz.max() / ulps.min() > 2.0 ** 53                  # the fp64 sum of this column cannot be exact
+    cu, orc = hz.CudaStream(w), hz.make_oracle(w)
+    try:
+        for c, (Qb, Kc, Vb) in enumerate(chunks):
+            got = cu.step(Qb, Kc, Vb, topk_count=2)
+            ref = hz.oracle_step(orc, Qb, Kc, Vb, topk_count=2)
+            hz.compare_step(got, ref, f"[widerange chunk {c}]")          # indices, counts, slot map bit-exact; O in tolerance
+        assert ref["min_gap"] > 1e-6                                      # the gaps dwarf a last-bit change of one mean
+        exact = sum(Fraction(float(x)) for x in col) / 128
+        pk = cu.pooled_k(0 * w.bpc + blk, 0)
+        ulp = np.spacing(float(exact))
+        assert abs(Fraction(float(pk[ch])) - exact) <= Fraction(ulp), (pk[ch], float(exact))
+        ok = orc.pooled_mean(hz.bits_to_f64(Kb))[0, blk]
+        assert abs(Fraction(float(ok[ch])) - exact) <= Fraction(ulp)
+        others = np.arange(128) != ch
+        assert np.array_equal(pk[others], ok[others])                     # every exact column is still bit-exact
+    finally:
+        cu.close()

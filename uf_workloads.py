@@ -95,6 +95,13 @@ CONFIGS: dict[str, Workload] = {
                          topk_count=-1, topk_percent=-1, amp=2.0, sink_blocks=0, tile=(2, 8, 8)),
     "2k_paper": Workload("2k_paper", 12, 128, 128, 3, _G2K[0], _G2K[1], capacity_chunks=3, prior_chunks=2,
                          topk_count=-1, topk_percent=-1, amp=2.0, sink_blocks=0, tile=(2, 8, 8)),
+    # the paper's OWN chunking: "streaming chunk size: 2 latent frames" at 960 x 1664
+    # -> 60 x 104 tokens per latent frame, 12 480 tokens per chunk, "KV cache: 3 temporal windows".  The
+    # (2,8,8) tiles are then full in t and 94 % full overall (1 x 8 x 13 = 104 tiles per chunk; only the last tile row
+    # is ragged: 60 = 7 * 8 + 4), the configuration section 2.3.1 was written for; BASELINE.json's 3-frame chunks leave
+    # half of the temporal tiles with one frame of two.
+    "1k_paper_native": Workload("1k_paper_native", 12, 128, 128, 2, *token_grid(960, 1664), capacity_chunks=3,
+                                prior_chunks=2, topk_count=-1, topk_percent=-1, amp=2.0, sink_blocks=0, tile=(2, 8, 8)),
 }
 
 
@@ -232,6 +239,9 @@ CMN_CONFIGS = {
     # the HR decoder, on a quarter-area crop of the 1K HR latent (the full 136 x 240 input makes
     # 1088 x 1920 x 12 frames of 64-channel activations per chunk)
     "cmn_decoder_crop": CmnWorkload("cmn_decoder_crop", 16, 3, (256, 128, 64, 64), 3, (2, 2, 2), (1, 2, 2), 68, 120, 1),
+    # PAPER.md:347 at full size: the whole 136 x 240 HR latent of the 1K workload, a chunk of 3 latent frames in ->
+    # 12 frames of 1088 x 1920 x 3 out ("8x8x4 spatiotemporal decoding"; Table 20 "HR Decoder")
+    "cmn_decoder_1k": CmnWorkload("cmn_decoder_1k", 16, 3, (256, 128, 64, 64), 3, (2, 2, 2), (1, 2, 2), 136, 240, 3),
 }
 
 
