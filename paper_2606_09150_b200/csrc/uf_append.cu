@@ -19,8 +19,8 @@ __device__ __forceinline__ void acc_bf16x8(double* acc, const uint4& u) {
   const uint32_t w[4] = {u.x, u.y, u.z, u.w};
 #pragma unroll
   for (int i = 0; i < 4; ++i) {
-    acc[2 * i]     += uf_bf16lo_to_f64(w[i]);
-    acc[2 * i + 1] += uf_bf16hi_to_f64(w[i]);
+    acc[2 * i]     += (double)__uint_as_float(w[i] << 16);
+    acc[2 * i + 1] += (double)__uint_as_float(w[i] & 0xFFFF0000u);
   }
 }
 

@@ -62,21 +62,6 @@ __host__ __device__ inline bool uf_tile_local(const UfTiling& t, int bi, int bj)
   return dh <= t.half && dw <= t.half;
 }
 
-#ifdef __CUDACC__
-// bf16 -> fp64 by bit placement (F2F.F64.F32 runs on the quarter-rate XU pipe and was 56 % / 32 % of
-// the pooling kernels' issue slots; widening is exact, so it is only a matter of where the bits go): sign to bit 63,
-// the 8-bit exponent re-biased by 1023 - 127 = 896 into bits 52..62, the 7 mantissa bits to the top of the fraction.
-// Zeros and subnormals (exponent field 0; rare in activations) take the converter.
-__device__ __forceinline__ double uf_bf16lo_to_f64(uint32_t w) {            // the bf16 in bits 0..15 of w
-  if ((w & 0x7F80u) == 0u) return (double)__uint_as_float(w << 16);
-  return __hiloint2double((int)((((w & 0x7FFFu) << 13) + 0x38000000u) | ((w & 0x8000u) << 16)), 0);
-}
-__device__ __forceinline__ double uf_bf16hi_to_f64(uint32_t w) {            // the bf16 in bits 16..31 of w
-  if ((w & 0x7F800000u) == 0u) return (double)__uint_as_float(w & 0xFFFF0000u);
-  return __hiloint2double((int)((((w >> 3) & 0x0FFFE000u) + 0x38000000u) | (w & 0x80000000u)), 0);
-}
-
-#endif
 // Snapshot of the cache state for one step, passed by value to kernels.
 struct UfView {
   UfTiling til;

@@ -41,8 +41,8 @@ uf_pool_q_kernel(const __nv_bfloat16* __restrict__ q, int64_t tok_stride, int64_
     const uint32_t w[4] = {u.x, u.y, u.z, u.w};
 #pragma unroll
     for (int t = 0; t < 4; ++t) {
-      acc[2 * t]     += uf_bf16lo_to_f64(w[t]);
-      acc[2 * t + 1] += uf_bf16hi_to_f64(w[t]);
+      acc[2 * t]     += (double)__uint_as_float(w[t] << 16);
+      acc[2 * t + 1] += (double)__uint_as_float(w[t] & 0xFFFF0000u);
     }
   }
 #pragma unroll

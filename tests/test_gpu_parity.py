@@ -540,8 +540,10 @@ def test_block_column_beyond_the_exact_sum_range():
     try:
         for c, (Qb, Kc, Vb) in enumerate(chunks):
             got = cu.step(Qb, Kc, Vb, topk_count=2)
-            ref = hz.oracle_step(orc, Qb, Kc, Vb, topk_count=2)
-            hz.compare_step(got, ref, f"[widerange chunk {c}]")          # indices, counts, slot map bit-exact; O in tolerance
+            # attention is not compared here: a 2^60 key makes logits of ~1e18, where fp32 logits have an ulp of 2^36
+            # and O is no longer within 2e-2 of the fp64 softmax (measured: max-abs 2.7); this case is about pooling
+            ref = hz.oracle_step(orc, Qb, Kc, Vb, topk_count=2, attn=False)
+            hz.compare_step(got, ref, f"[widerange chunk {c}]")          # indices, counts, slot map bit-exact
         assert ref["min_gap"] > 1e-6                                      # the gaps dwarf a last-bit change of one mean
         exact = sum(Fraction(float(x)) for x in col) / 128
         pk = cu.pooled_k(0 * w.bpc + blk, 0)
